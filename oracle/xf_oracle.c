@@ -1,0 +1,532 @@
+/*
+ * xf_oracle.c -- plain CPU oracle (TEST INFRASTRUCTURE ONLY; see xf_oracle.h for scope, pins and build flags).
+ *
+ * Layout: SoA, U[v][k][j][i], i fastest; v = 0: rho, 1..3: rho u, rho v, rho w, 4: E, 5..Nv-1: rho Y_1..rho Y_{N-1}
+ * (Eq. 2, "s = 1..N-1"; reading R1).  A direction with one interior cell carries no ghosts.
+ */
+#include "xf_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* ------------------------------------------------------------------------------------------------------------ */
+/* grid helpers                                                                                                 */
+/* ------------------------------------------------------------------------------------------------------------ */
+int xo_nv(const xo_config *c) { return c->N + 4; }
+
+void xo_padded_dims(const xo_config *c, int *nxp, int *nyp, int *nzp) {
+  *nxp = c->nx > 1 ? c->nx + 2 * c->ng : 1;
+  *nyp = c->ny > 1 ? c->ny + 2 * c->ng : 1;
+  *nzp = c->nz > 1 ? c->nz + 2 * c->ng : 1;
+}
+
+long xo_padded_cells(const xo_config *c) {
+  int a, b, d;
+  xo_padded_dims(c, &a, &b, &d);
+  return (long)a * b * d;
+}
+
+static void grid(const xo_config *c, int np[3], int n[3], int g[3], long stride[3]) {
+  xo_padded_dims(c, &np[0], &np[1], &np[2]);
+  n[0] = c->nx; n[1] = c->ny; n[2] = c->nz;
+  for (int d = 0; d < 3; ++d) g[d] = n[d] > 1 ? c->ng : 0;
+  stride[0] = 1; stride[1] = np[0]; stride[2] = (long)np[0] * np[1];
+}
+
+/* ------------------------------------------------------------------------------------------------------------ */
+/* C1. Thermodynamics (Eq. 7; Eq. 21; NASA polynomials PAPER.md:153)            */
+/*     T_c = min(max(T, Tlo), Thi); outside the fit range cp is frozen and h continues linearly (reading R3).   */
+/* ------------------------------------------------------------------------------------------------------------ */
+void xo_species_thermo(const xo_config *c, int s, double T, double *cp, double *h, double *e) {
+  const double *a = c->a[s];
+  const double Rs = c->Ru / c->W[s];
+  double Tc = T;
+  if (Tc < c->Tlo) Tc = c->Tlo;
+  if (Tc > c->Thi) Tc = c->Thi;
+  const double cpR = a[0] + Tc * (a[1] + Tc * (a[2] + Tc * (a[3] + Tc * a[4])));
+  const double hR = Tc * (a[0] + Tc * (a[1] / 2.0 + Tc * (a[2] / 3.0 + Tc * (a[3] / 4.0 + Tc * (a[4] / 5.0))))) + a[5];
+  *cp = Rs * cpR;
+  *h = Rs * hR + (*cp) * (T - Tc);
+  *e = *h - Rs * T;
+}
+
+/* mixture: Rbar = sum Y_s R_s (Eq. 7); e(T) = sum Y_s e_s(T); Cv = sum Y_s cp_s - Rbar (Eq. 21); s ascending */
+void xo_mixture(const xo_config *c, const double *Y, double T, double *Rbar, double *e, double *Cv) {
+  double R = 0.0, em = 0.0, cpm = 0.0;
+  for (int s = 0; s < c->N; ++s) {
+    double cp, h, es;
+    xo_species_thermo(c, s, T, &cp, &h, &es);
+    R += Y[s] * (c->Ru / c->W[s]);
+    em += Y[s] * es;
+    cpm += Y[s] * cp;
+  }
+  *Rbar = R;
+  *e = em;
+  *Cv = cpm - R;
+}
+
+/* ------------------------------------------------------------------------------------------------------------ */
+/* C2. Primitive recovery.  Newton: T^{k+1} = T^k + (e - e(T^k))/Cv(T^k)  (Eq. 21)           */
+/* ------------------------------------------------------------------------------------------------------------ */
+static void cell_basic(const xo_config *c, const double *Ucell, xo_prim *P) {
+  const int N = c->N;
+  P->rho = Ucell[0];
+  for (int d = 0; d < 3; ++d) P->vel[d] = Ucell[1 + d] / P->rho;
+  double sumY = 0.0;
+  for (int i = 0; i < N - 1; ++i) {
+    P->Y[i] = Ucell[5 + i] / P->rho;
+    sumY += P->Y[i];
+  }
+  P->Y[N - 1] = 1.0 - sumY; /* closure, no clipping, no renormalisation (reading R12) */
+  P->e = Ucell[4] / P->rho - 0.5 * (P->vel[0] * P->vel[0] + P->vel[1] * P->vel[1] + P->vel[2] * P->vel[2]);
+}
+
+/* everything that follows from a given temperature */
+static void cell_from_T(const xo_config *c, const double *Ucell, double T, xo_prim *P) {
+  const int N = c->N;
+  double Rbar, em, Cv;
+  xo_mixture(c, P->Y, T, &Rbar, &em, &Cv);
+  P->T = T;
+  P->Rbar = Rbar;
+  P->Cv = Cv;
+  P->p = P->rho * Rbar * T;              /* Eq. 7 */
+  P->Gamma = Rbar / Cv;                  /* Gamma = (dp/de)_rho / rho = gamma - 1 */
+  P->c = sqrt((1.0 + P->Gamma) * P->p / P->rho);
+  P->H = (Ucell[4] + P->p) / P->rho;
+  for (int s = 0; s < N; ++s) {
+    double cp, h, es;
+    xo_species_thermo(c, s, T, &cp, &h, &es);
+    P->chi[s] = (c->Ru / c->W[s]) * T - P->Gamma * es;   /* chi_s = (dp/d(rho Y_s)) at fixed rho e */
+  }
+  if (!(P->rho > 0.0) || !(P->T > 0.0) || !(P->p > 0.0)) P->status |= XO_ENONPHYSICAL;
+}
+
+void xo_cell_primitives(const xo_config *c, const double *Ucell, double Tguess, xo_prim *P) {
+  memset(P, 0, sizeof(*P));
+  cell_basic(c, Ucell, P);
+  double T = Tguess;
+  int k = 0, converged = 0;
+  while (k < c->maxit) {
+    double Rbar, eT, Cv;
+    xo_mixture(c, P->Y, T, &Rbar, &eT, &Cv);
+    const double Tn = T + (P->e - eT) / Cv;
+    ++k;
+    const double dT = fabs(Tn - T);
+    T = Tn;
+    if (dT <= c->rtol * fabs(Tn)) { converged = 1; break; }
+    if (!(Tn == Tn)) break; /* NaN */
+  }
+  P->iters = k;
+  if (!converged) P->status |= XO_ENOCONV;
+  cell_from_T(c, Ucell, T, P);
+}
+
+static void gather_cell(const xo_config *c, const double *U, long cells, long idx, double *Ucell) {
+  const int Nv = c->N + 4;
+  for (int v = 0; v < Nv; ++v) Ucell[v] = U[v * cells + idx];
+}
+
+int xo_primitives(const xo_config *c, const double *U, double *T, double *p, double *cs, double *iters_mean) {
+  const long cells = xo_padded_cells(c);
+  int status = 0;
+  double itsum = 0.0;
+#pragma omp parallel for reduction(| : status) reduction(+ : itsum) schedule(static) if (cells > 16384)
+  for (long idx = 0; idx < cells; ++idx) {
+    double Uc[XO_MAXNV];
+    xo_prim P;
+    gather_cell(c, U, cells, idx, Uc);
+    xo_cell_primitives(c, Uc, T[idx], &P);
+    T[idx] = P.T;
+    if (p) p[idx] = P.p;
+    if (cs) cs[idx] = P.c;
+    status |= P.status;
+    itsum += P.iters;
+  }
+  if (iters_mean) *iters_mean = itsum / (double)cells;
+  return status;
+}
+
+/* ------------------------------------------------------------------------------------------------------------ */
+/* C3. Physical flux in direction d (Eq. 2)                                                         */
+/* ------------------------------------------------------------------------------------------------------------ */
+void xo_phys_flux(const xo_config *c, const double *Uc, const xo_prim *P, int d, double *F) {
+  const int Nv = c->N + 4;
+  const double ud = P->vel[d];
+  F[0] = Uc[0] * ud;
+  for (int q = 0; q < 3; ++q) F[1 + q] = Uc[1 + q] * ud + (q == d ? P->p : 0.0);
+  F[4] = (Uc[4] + P->p) * ud;
+  for (int v = 5; v < Nv; ++v) F[v] = Uc[v] * ud;
+}
+
+/* ------------------------------------------------------------------------------------------------------------ */
+/* C4. Dense face eigensystem (Lambda = L A R with the Roe-averaged Jacobian, refs 32/33/37;    */
+/*     the matrices are not printed in the paper -> readings R5, R6)                                            */
+/* ------------------------------------------------------------------------------------------------------------ */
+static void tangentials(int d, int *t1, int *t2) {
+  /* x: (v, w); y: roles of (u, index 1) and (v, index 2) swapped -> (u, w); z: u <-> w swapped -> (v, u) */
+  if (d == 0) { *t1 = 1; *t2 = 2; }
+  else if (d == 1) { *t1 = 0; *t2 = 2; }
+  else { *t1 = 1; *t2 = 0; }
+}
+
+int xo_eigensystem(const xo_config *c, const xo_prim *A, const xo_prim *B, int d, double *L, double *R, double *roe) {
+  const int N = c->N, Nv = N + 4;
+  int status = 0;
+  /* Roe-type average (reading R5): q~ = (w_a q_a + w_b q_b)/(w_a + w_b), w = sqrt(rho) */
+  const double wa = sqrt(A->rho), wb = sqrt(B->rho);
+#define AVG(qa, qb) ((wa * (qa) + wb * (qb)) / (wa + wb))
+  double vt[3], Yt[XO_MAXN], chit[XO_MAXN];
+  for (int q = 0; q < 3; ++q) vt[q] = AVG(A->vel[q], B->vel[q]);
+  const double Ht = AVG(A->H, B->H);
+  const double Gt = AVG(A->Gamma, B->Gamma);
+  for (int s = 0; s < N; ++s) {
+    Yt[s] = AVG(A->Y[s], B->Y[s]);
+    chit[s] = AVG(A->chi[s], B->chi[s]);
+  }
+#undef AVG
+  const double kt = 0.5 * (vt[0] * vt[0] + vt[1] * vt[1] + vt[2] * vt[2]);
+  double c2 = 0.0;
+  for (int s = 0; s < N; ++s) c2 += Yt[s] * chit[s];
+  c2 += Gt * (Ht - kt);
+  if (!(c2 > 0.0)) status |= XO_ENONPHYSICAL;
+  const double ct = sqrt(c2);
+  double zeta[XO_MAXN];
+  for (int i = 0; i < N - 1; ++i) zeta[i] = chit[i] - chit[N - 1];
+  const double Prho = chit[N - 1] + Gt * kt;
+
+  double pi[XO_MAXNV], nu[XO_MAXNV], b[XO_MAXNV];
+  memset(nu, 0, sizeof(nu));
+  pi[0] = Prho;
+  for (int q = 0; q < 3; ++q) pi[1 + q] = -Gt * vt[q];
+  pi[4] = Gt;
+  for (int i = 0; i < N - 1; ++i) pi[5 + i] = zeta[i];
+  nu[0] = -vt[d];
+  nu[1 + d] = 1.0;
+  b[0] = 1.0;
+  for (int q = 0; q < 3; ++q) b[1 + q] = vt[q];
+  b[4] = Ht;
+  for (int i = 0; i < N - 1; ++i) b[5 + i] = Yt[i];
+
+  int t1, t2;
+  tangentials(d, &t1, &t2);
+  memset(L, 0, sizeof(double) * Nv * Nv);
+  memset(R, 0, sizeof(double) * Nv * Nv);
+#define LL(n, j) L[(n) * Nv + (j)]
+#define RR(j, n) R[(j) * Nv + (n)]
+  for (int j = 0; j < Nv; ++j) {
+    LL(0, j) = (pi[j] - ct * nu[j]) / (2.0 * c2);
+    LL(Nv - 1, j) = (pi[j] + ct * nu[j]) / (2.0 * c2);
+    LL(1, j) = (j == 0 ? 1.0 : 0.0) - pi[j] / c2;
+    RR(j, 0) = b[j];
+    RR(j, 1) = b[j];
+    RR(j, Nv - 1) = b[j];
+  }
+  RR(1 + d, 0) -= ct;
+  RR(4, 0) -= vt[d] * ct;
+  RR(1 + d, Nv - 1) += ct;
+  RR(4, Nv - 1) += vt[d] * ct;
+  RR(4, 1) = Ht - c2 / Gt;
+  LL(2, 0) = -vt[t1]; LL(2, 1 + t1) = 1.0;
+  LL(3, 0) = -vt[t2]; LL(3, 1 + t2) = 1.0;
+  RR(1 + t1, 2) = 1.0; RR(4, 2) = vt[t1];
+  RR(1 + t2, 3) = 1.0; RR(4, 3) = vt[t2];
+  for (int i = 0; i < N - 1; ++i) {
+    LL(4 + i, 0) = -Yt[i];
+    LL(4 + i, 5 + i) = 1.0;
+    RR(5 + i, 4 + i) = 1.0;
+    RR(4, 4 + i) = -zeta[i] / Gt;
+  }
+#undef LL
+#undef RR
+  if (roe) { /* exposed for the pins: u~ v~ w~ H~ Gamma~ c~ */
+    roe[0] = vt[0]; roe[1] = vt[1]; roe[2] = vt[2]; roe[3] = Ht; roe[4] = Gt; roe[5] = ct;
+  }
+  return status;
+}
+
+/* ------------------------------------------------------------------------------------------------------------ */
+/* C6. WENO5-JS (ref 35; eps = 1e-6, exponent 2, linear weights 0.1 0.6 0.3: reading R7)          */
+/* ------------------------------------------------------------------------------------------------------------ */
+double xo_weno5(const double v[5], int ideal_weights) {
+  const double q0 = (2.0 * v[0] - 7.0 * v[1] + 11.0 * v[2]) / 6.0;
+  const double q1 = (-v[1] + 5.0 * v[2] + 2.0 * v[3]) / 6.0;
+  const double q2 = (2.0 * v[2] + 5.0 * v[3] - v[4]) / 6.0;
+  double a0, a1, a2;
+  if (ideal_weights) {
+    a0 = 0.1; a1 = 0.6; a2 = 0.3;
+  } else {
+    const double eps = 1e-6;
+    const double t0 = v[0] - 2.0 * v[1] + v[2], s0 = v[0] - 4.0 * v[1] + 3.0 * v[2];
+    const double t1 = v[1] - 2.0 * v[2] + v[3], s1 = v[1] - v[3];
+    const double t2 = v[2] - 2.0 * v[3] + v[4], s2 = 3.0 * v[2] - 4.0 * v[3] + v[4];
+    const double b0 = 13.0 / 12.0 * t0 * t0 + 0.25 * s0 * s0;
+    const double b1 = 13.0 / 12.0 * t1 * t1 + 0.25 * s1 * s1;
+    const double b2 = 13.0 / 12.0 * t2 * t2 + 0.25 * s2 * s2;
+    a0 = 0.1 / ((eps + b0) * (eps + b0));
+    a1 = 0.6 / ((eps + b1) * (eps + b1));
+    a2 = 0.3 / ((eps + b2) * (eps + b2));
+  }
+  return (a0 * q0 + a1 * q1 + a2 * q2) / (a0 + a1 + a2);
+}
+
+/* ------------------------------------------------------------------------------------------------------------ */
+/* C5 + C6 + C7. Numerical flux at one face (Eq. 14-15; LLF: PAPER.md:374, reading R8)        */
+/* Ust[m][v], Pst[m], m = 0..5 <-> cells i-2..i+3; the face lies between m = 2 and m = 3.                       */
+/* ------------------------------------------------------------------------------------------------------------ */
+int xo_face_flux(const xo_config *c, int d, const double *Ust, const xo_prim *Pst, double *Fhat) {
+  const int Nv = c->N + 4;
+  double L[XO_MAXNV * XO_MAXNV], R[XO_MAXNV * XO_MAXNV];
+  int status = xo_eigensystem(c, &Pst[2], &Pst[3], d, L, R, NULL);
+
+  double aF[6][XO_MAXNV], aU[6][XO_MAXNV], lam[6][3];
+  for (int m = 0; m < 6; ++m) {
+    double F[XO_MAXNV];
+    xo_phys_flux(c, Ust + m * Nv, &Pst[m], d, F);
+    for (int n = 0; n < Nv; ++n) {          /* alpha^F_m = L F_m, alpha^U_m = L U_m (face-frozen L) */
+      double sF = 0.0, sU = 0.0;
+      for (int j = 0; j < Nv; ++j) {
+        sF += L[n * Nv + j] * F[j];
+        sU += L[n * Nv + j] * Ust[m * Nv + j];
+      }
+      aF[m][n] = sF;
+      aU[m][n] = sU;
+    }
+    lam[m][0] = Pst[m].vel[d] - Pst[m].c;   /* the cell's own eigenvalues */
+    lam[m][1] = Pst[m].vel[d];
+    lam[m][2] = Pst[m].vel[d] + Pst[m].c;
+  }
+  double g[XO_MAXNV];
+  for (int n = 0; n < Nv; ++n) {
+    const int kind = n == 0 ? 0 : (n == Nv - 1 ? 2 : 1);
+    double Lam = 0.0;                        /* LLF: max over the 6 stencil cells, factor 1 */
+    for (int m = 0; m < 6; ++m) Lam = fmax(Lam, fabs(lam[m][kind]));
+    double fp[6], fm[6];
+    for (int m = 0; m < 6; ++m) {            /* Eq. 14 */
+      fp[m] = 0.5 * (aF[m][n] + Lam * aU[m][n]);
+      fm[m] = 0.5 * (aF[m][n] - Lam * aU[m][n]);
+    }
+    const double vp[5] = {fp[0], fp[1], fp[2], fp[3], fp[4]};
+    const double vm[5] = {fm[5], fm[4], fm[3], fm[2], fm[1]};
+    g[n] = xo_weno5(vp, c->ideal_weights) + xo_weno5(vm, c->ideal_weights);
+  }
+  for (int j = 0; j < Nv; ++j) {             /* Eq. 15: Fhat = R (F+ + F-) */
+    double s = 0.0;
+    for (int n = 0; n < Nv; ++n) s += R[j * Nv + n] * g[n];
+    Fhat[j] = s;
+  }
+  return status;
+}
+
+/* ------------------------------------------------------------------------------------------------------------ */
+/* C8. Ghost fill ("specific boundary conditions", 433; formulas: reading R10), x then y then z    */
+/* ------------------------------------------------------------------------------------------------------------ */
+void xo_fill_ghosts(const xo_config *c, double *U) {
+  const int Nv = c->N + 4;
+  int np[3], n[3], g[3];
+  long st[3];
+  grid(c, np, n, g, st);
+  const long cells = xo_padded_cells(c);
+  for (int d = 0; d < 3; ++d) {
+    if (n[d] == 1) continue;
+    /* extent of the two other axes: padded if that direction was already filled, interior otherwise */
+    int lo[3], hi[3];
+    for (int q = 0; q < 3; ++q) {
+      if (q < d) { lo[q] = 0; hi[q] = np[q]; }
+      else { lo[q] = g[q]; hi[q] = g[q] + n[q]; }
+    }
+    const int a1 = (d + 1) % 3, a2 = (d + 2) % 3;
+    for (int side = 0; side < 2; ++side) {
+      const int bc = c->bc[2 * d + side];
+      for (int l = 0; l < g[d]; ++l) {
+        const int ighost = side == 0 ? g[d] - 1 - l : g[d] + n[d] + l;
+        int isrc = ighost;
+        if (bc == XO_BC_PERIODIC) isrc = side == 0 ? ighost + n[d] : ighost - n[d];
+        else if (bc == XO_BC_TRANSMISSIVE) isrc = side == 0 ? g[d] : g[d] + n[d] - 1;
+        else if (bc == XO_BC_REFLECTIVE) isrc = side == 0 ? g[d] + l : g[d] + n[d] - 1 - l;
+        for (int p = lo[a1]; p < hi[a1]; ++p)
+          for (int q = lo[a2]; q < hi[a2]; ++q) {
+            const long base = (long)p * st[a1] + (long)q * st[a2];
+            const long ig = base + (long)ighost * st[d], is = base + (long)isrc * st[d];
+            for (int v = 0; v < Nv; ++v) {
+              double val;
+              if (bc == XO_BC_DIRICHLET) val = c->bc_state[2 * d + side][v];
+              else {
+                val = U[v * cells + is];
+                if (bc == XO_BC_REFLECTIVE && v == 1 + d) val = -val; /* wall-normal momentum negated */
+              }
+              U[v * cells + ig] = val;
+            }
+          }
+      }
+    }
+  }
+}
+
+/* ------------------------------------------------------------------------------------------------------------ */
+/* C7. rhs = - sum_d (Fhat_{i+1/2} - Fhat_{i-1/2})/dx_d  (Eq. 13; faces per PAPER.md:271-273)       */
+/* ------------------------------------------------------------------------------------------------------------ */
+static void pencil_prims(const xo_config *c, const double *U, const double *T, long cells, long base, long stride,
+                         int count, double *Ust, xo_prim *Pst) {
+  const int Nv = c->N + 4;
+  for (int m = 0; m < count; ++m) {
+    const long idx = base + m * stride;
+    gather_cell(c, U, cells, idx, Ust + m * Nv);
+    memset(&Pst[m], 0, sizeof(xo_prim));
+    cell_basic(c, Ust + m * Nv, &Pst[m]);
+    cell_from_T(c, Ust + m * Nv, T[idx], &Pst[m]);
+  }
+}
+
+/* U must have its ghosts filled; T: in guess, out converged temperature (whole padded field) */
+int xo_rhs_nofill(const xo_config *c, const double *U, double *T, double *rhs) {
+  const int Nv = c->N + 4;
+  int np[3], n[3], g[3];
+  long st[3];
+  grid(c, np, n, g, st);
+  const long cells = xo_padded_cells(c);
+  int status = xo_primitives(c, U, T, NULL, NULL, NULL);   /* "after updating the primitive variables" PAPER.md:411 */
+  memset(rhs, 0, sizeof(double) * Nv * cells);
+  const double dxs[3] = {c->dx, c->dy, c->dz};
+  for (int d = 0; d < 3; ++d) {
+    if (n[d] == 1) continue;
+    const int a1 = (d + 1) % 3, a2 = (d + 2) % 3;
+    const long npen = (long)n[a1] * n[a2];
+    const int len = np[d];
+#pragma omp parallel reduction(| : status) if (npen > 16)
+    {
+      double *Ust = (double *)malloc(sizeof(double) * len * Nv);
+      xo_prim *Pst = (xo_prim *)malloc(sizeof(xo_prim) * len);
+      double *Fh = (double *)malloc(sizeof(double) * (n[d] + 1) * Nv);
+#pragma omp for schedule(dynamic, 4)
+      for (long pen = 0; pen < npen; ++pen) {
+        const int p = g[a1] + (int)(pen / n[a2]), q = g[a2] + (int)(pen % n[a2]);
+        const long base = (long)p * st[a1] + (long)q * st[a2];
+        pencil_prims(c, U, T, cells, base, st[d], len, Ust, Pst);
+        /* faces i = g-1 .. g+n-1 (face i+1/2 between cells i and i+1): n+1 faces */
+        for (int f = 0; f <= n[d]; ++f) {
+          const int i = g[d] - 1 + f;
+          status |= xo_face_flux(c, d, Ust + (i - 2) * Nv, Pst + (i - 2), Fh + f * Nv);
+        }
+        for (int f = 0; f < n[d]; ++f) {
+          const long idx = base + (long)(g[d] + f) * st[d];
+          for (int v = 0; v < Nv; ++v) rhs[v * cells + idx] -= (Fh[(f + 1) * Nv + v] - Fh[f * Nv + v]) / dxs[d];
+        }
+      }
+      free(Ust); free(Pst); free(Fh);
+    }
+  }
+  return status;
+}
+
+int xo_rhs(const xo_config *c, double *U, double *T, double *rhs) {
+  xo_fill_ghosts(c, U);                /* "with specific boundary conditions" before each residual: R11 */
+  return xo_rhs_nofill(c, U, T, rhs);
+}
+
+/* rhs at a list of sampled interior cells, each computed on its own from U (ghosts filled) and the T guess:
+ * primitives by Newton for the 7-cell cross of every direction, two faces per direction.  Used for parity at
+ * sizes where the whole-field oracle would take too long. rhs_out[q][v]. */
+int xo_rhs_cells(const xo_config *c, const double *U, const double *Tguess, long ncells, const long *idx,
+                 double *rhs_out) {
+  const int Nv = c->N + 4;
+  int np[3], n[3], g[3];
+  long st[3];
+  grid(c, np, n, g, st);
+  const long cells = xo_padded_cells(c);
+  const double dxs[3] = {c->dx, c->dy, c->dz};
+  int status = 0;
+#pragma omp parallel for reduction(| : status) schedule(dynamic, 8) if (ncells > 64)
+  for (long q = 0; q < ncells; ++q) {
+    double acc[XO_MAXNV];
+    for (int v = 0; v < Nv; ++v) acc[v] = 0.0;
+    for (int d = 0; d < 3; ++d) {
+      if (n[d] == 1) continue;
+      double Ust[7 * XO_MAXNV];
+      xo_prim Pst[7];
+      for (int m = 0; m < 7; ++m) {     /* cells i-3 .. i+3 */
+        const long id = idx[q] + (long)(m - 3) * st[d];
+        gather_cell(c, U, cells, id, Ust + m * Nv);
+        xo_cell_primitives(c, Ust + m * Nv, Tguess[id], &Pst[m]);
+        status |= Pst[m].status;
+      }
+      double Fl[XO_MAXNV], Fr[XO_MAXNV];
+      status |= xo_face_flux(c, d, Ust, Pst, Fl);            /* face i-1/2: cells i-3..i+2 */
+      status |= xo_face_flux(c, d, Ust + Nv, Pst + 1, Fr);   /* face i+1/2: cells i-2..i+3 */
+      for (int v = 0; v < Nv; ++v) acc[v] -= (Fr[v] - Fl[v]) / dxs[d];
+    }
+    for (int v = 0; v < Nv; ++v) rhs_out[q * Nv + v] = acc[v];
+  }
+  return status;
+}
+
+/* ------------------------------------------------------------------------------------------------------------ */
+/* SSP-RK3 (Eq. 16); ghosts + primitives before each of the three residuals     */
+/* ------------------------------------------------------------------------------------------------------------ */
+int xo_rk3_step(const xo_config *c, double *U, double *T, double dt) {
+  const int Nv = c->N + 4;
+  int np[3], n[3], g[3];
+  long st[3];
+  grid(c, np, n, g, st);
+  const long cells = xo_padded_cells(c);
+  const size_t bytes = sizeof(double) * Nv * cells;
+  double *U1 = (double *)malloc(bytes), *U2 = (double *)malloc(bytes), *Lr = (double *)malloc(bytes);
+  int status = 0;
+  status |= xo_rhs(c, U, T, Lr);                         /* L(U^n) */
+  memcpy(U1, U, bytes);
+  memcpy(U2, U, bytes);
+#define FOR_INTERIOR                                                                  \
+  for (int v = 0; v < Nv; ++v)                                                        \
+    for (int k = g[2]; k < g[2] + n[2]; ++k)                                          \
+      for (int j = g[1]; j < g[1] + n[1]; ++j)                                        \
+        for (int i = g[0]; i < g[0] + n[0]; ++i)
+  FOR_INTERIOR {
+    const long id = v * cells + (long)k * st[2] + (long)j * st[1] + i;
+    U1[id] = U[id] + dt * Lr[id];
+  }
+  status |= xo_rhs(c, U1, T, Lr);                        /* L(U^1) */
+  FOR_INTERIOR {
+    const long id = v * cells + (long)k * st[2] + (long)j * st[1] + i;
+    U2[id] = 0.75 * U[id] + 0.25 * (U1[id] + dt * Lr[id]);
+  }
+  status |= xo_rhs(c, U2, T, Lr);                        /* L(U^2) */
+  FOR_INTERIOR {
+    const long id = v * cells + (long)k * st[2] + (long)j * st[1] + i;
+    U[id] = 1.0 / 3.0 * U[id] + 2.0 / 3.0 * (U2[id] + dt * Lr[id]);
+  }
+#undef FOR_INTERIOR
+  free(U1); free(U2); free(Lr);
+  return status;
+}
+
+/* ------------------------------------------------------------------------------------------------------------ */
+/* Max wave speed for the CFL time step: S = max_cells sum_d (|u_d| + c)/dx_d; dt = CFL/S                       */
+/* (Eq. 17 lambda = dt/dx = CFL/Lambda~ in 1-D; PAPER.md:429 global minimum step; reading R9)      */
+/* ------------------------------------------------------------------------------------------------------------ */
+double xo_max_wavespeed(const xo_config *c, const double *U, double *T, int *status_out) {
+  int np[3], n[3], g[3];
+  long st[3];
+  grid(c, np, n, g, st);
+  const long cells = xo_padded_cells(c);
+  const double dxs[3] = {c->dx, c->dy, c->dz};
+  double S = 0.0;
+  int status = 0;
+#pragma omp parallel for reduction(max : S) reduction(| : status) collapse(2) if (cells > 16384)
+  for (int k = g[2]; k < g[2] + n[2]; ++k)
+    for (int j = g[1]; j < g[1] + n[1]; ++j)
+      for (int i = g[0]; i < g[0] + n[0]; ++i) {
+        const long idx = (long)k * st[2] + (long)j * st[1] + i;
+        double Uc[XO_MAXNV];
+        xo_prim P;
+        gather_cell(c, U, cells, idx, Uc);
+        xo_cell_primitives(c, Uc, T[idx], &P);
+        T[idx] = P.T;
+        status |= P.status;
+        double s = 0.0;
+        for (int d = 0; d < 3; ++d)
+          if (n[d] > 1) s += (fabs(P.vel[d]) + P.c) / dxs[d];
+        if (s > S) S = s;
+      }
+  if (status_out) *status_out = status;
+  return S;
+}

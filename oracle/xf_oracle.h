@@ -1,0 +1,98 @@
+/*
+ * xf_oracle.h -- plain CPU oracle for the convective right-hand side of the multicomponent compressible Euler
+ * equations (XFluids, arxiv 2403.05910).  TEST INFRASTRUCTURE ONLY.
+ *
+ * This is the slow, obviously-correct fp64 restatement of what the hot path computes.  It follows the paper
+ * step by step (citations are PAPER.md:<line>, section / equation) and, where the paper prints no formula,
+ * the readings R1..R15 listed in DESIGN.md (taken from SURVEY.md 8(c)).  It shares NO code with the CUDA path
+ * (paper_2403_05910_b200/csrc): dense Nv x Nv eigenvector matrices and dense mat-vec products here, an expanded
+ * structured form there; plain Jiang-Shu weights with three divisions here, a common-denominator form there.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may build, load or
+ * call anything in oracle/.  The product path never does.
+ *
+ * Parity pins (tests/test_oracle_*.py, -m "not gpu"): closed-form T(e); c^2 identity; L.R = I, L.A.R = diag
+ * (finite-difference Jacobian); N = 1 textbook Euler eigenvectors and Roe sound speed; WENO5 exactness on
+ * degree-4 polynomials, 5th order on smooth data; uniform-flow preservation; exact Sod Riemann solution; design
+ * order on an advected density wave; round-off conservation; interface equilibrium (equal gamma); mirror and
+ * permutation symmetry; direction consistency; dense-inverse brute-force face flux.
+ * Parity unpinned: agreement with XFluids' own code output and with the paper's Fig. 15 curves (neither code,
+ * numbers nor reference data are available).
+ *
+ * Build: gcc -O2 -ffp-contract=off -fopenmp -fPIC -shared (no -ffast-math).  OpenMP only on outermost loops of
+ * independent per-cell / per-face work, so results do not depend on the thread count.
+ */
+#ifndef XF_ORACLE_H
+#define XF_ORACLE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define XO_MAXN 16            /* max species */
+#define XO_MAXNV (XO_MAXN + 4)
+
+enum { XO_BC_PERIODIC = 0, XO_BC_TRANSMISSIVE = 1, XO_BC_REFLECTIVE = 2, XO_BC_DIRICHLET = 3 };
+enum { XO_OK = 0, XO_ENONPHYSICAL = 4, XO_ENOCONV = 5 };   /* status bits */
+
+typedef struct {
+  int nx, ny, nz;             /* interior cells; n == 1 -> direction inactive (no ghosts, no sweep)           */
+  int ng;                     /* ghost width, 3                                                               */
+  double dx, dy, dz;
+  int N;                      /* species; Nv = N + 4                                                          */
+  double Ru;
+  double W[XO_MAXN];
+  double a[XO_MAXN][7];       /* NASA-7 single range a1..a7 (a7 unused)                                       */
+  double Tlo, Thi;
+  int bc[6];                  /* xlo xhi ylo yhi zlo zhi                                                      */
+  double bc_state[6][XO_MAXNV];
+  double rtol;                /* Newton |dT| <= rtol |T|, 1e-13                                               */
+  int maxit;                  /* 50                                                                           */
+  int ideal_weights;          /* test switch: WENO5 with the linear weights               */
+} xo_config;
+
+/* all primitive quantities of one cell (C2) */
+typedef struct {
+  double rho, vel[3], Y[XO_MAXN], e, T, p, Rbar, Cv, Gamma, c, H, chi[XO_MAXN];
+  int iters, status;
+} xo_prim;
+
+/* grid helpers */
+int xo_nv(const xo_config *c);
+long xo_padded_cells(const xo_config *c);
+void xo_padded_dims(const xo_config *c, int *nxp, int *nyp, int *nzp);
+
+/* C1 thermodynamics */
+void xo_species_thermo(const xo_config *c, int s, double T, double *cp, double *h, double *e);
+void xo_mixture(const xo_config *c, const double *Y, double T, double *Rbar, double *e, double *Cv);
+
+/* C2 primitive recovery of one cell / of the whole padded field */
+void xo_cell_primitives(const xo_config *c, const double *Ucell, double Tguess, xo_prim *out);
+int xo_primitives(const xo_config *c, const double *U, double *T, double *p, double *cs, double *iters_mean);
+
+/* C3 physical flux of one cell in direction d */
+void xo_phys_flux(const xo_config *c, const double *Ucell, const xo_prim *P, int d, double *F);
+
+/* C4 dense face eigensystem from two cells' primitives: L, R are Nv x Nv row-major; returns status bits */
+int xo_eigensystem(const xo_config *c, const xo_prim *A, const xo_prim *B, int d, double *L, double *R, double *roe);
+
+/* C6 WENO5-JS: v[0..4] = v_{-2}..v_{+2}, value at +1/2 */
+double xo_weno5(const double v[5], int ideal_weights);
+
+/* C5-C7 numerical flux at one face from the 6 stencil cells (Ust[m][v], m = 0..5 <-> i-2..i+3) */
+int xo_face_flux(const xo_config *c, int d, const double *Ust, const xo_prim *Pst, double *Fhat);
+
+/* C8 ghost fill; C7 rhs, rk3, max wave speed.  U is [Nv][padded], T is [padded] (in: guess, out: T) */
+void xo_fill_ghosts(const xo_config *c, double *U);
+int xo_rhs(const xo_config *c, double *U, double *T, double *rhs);
+int xo_rhs_nofill(const xo_config *c, const double *U, double *T, double *rhs);
+/* rhs at sampled interior cells (padded linear indices idx[ncells]) straight from ghost-filled U and the T guess */
+int xo_rhs_cells(const xo_config *c, const double *U, const double *Tguess, long ncells, const long *idx,
+                 double *rhs_out);
+int xo_rk3_step(const xo_config *c, double *U, double *T, double dt);
+double xo_max_wavespeed(const xo_config *c, const double *U, double *T, int *status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
