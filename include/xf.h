@@ -1,0 +1,131 @@
+/*
+ * xf.h -- C ABI of libxf.so: the convective right-hand side of the multicomponent compressible Euler equations
+ * (the per-Runge-Kutta-stage hot path of XFluids, arxiv 2403.05910) as hand-written CUDA for sm_100a.
+ *
+ * Citations are PAPER.md:<line> (the paper) and DESIGN.md readings R1..R15 where the paper prints no formula.
+ *
+ * Conventions
+ *   Variables   Nv = N + 4 per cell: v = 0 rho, 1..3 rho u, rho v, rho w, 4 E, 5.. rho Y_1 .. rho Y_{N-1}
+ *               (Eq. 2; "s = 1..N-1"); Y_N = 1 - sum of the others.
+ *   Layout      SoA, fp64, U[v][k][j][i], i fastest.  Every ACTIVE direction (n_d > 1) carries ng = 3 ghost cells
+ *               on both sides (WENO5 stencil i-2..i+3); an inactive direction (n_d == 1) has none.
+ *               padded extent np_d = n_d + 6 (active) or 1; padded cells = npx*npy*npz; field v starts at
+ *               U + v*padded_cells.  Scalar fields (T, p, c) are [k][j][i] over the same padded box.
+ *   Memory      All field pointers are CALLER-OWNED DEVICE memory (8-byte aligned) unless the name ends in
+ *               _host.  The library allocates nothing per call; the context owns the species table, boundary
+ *               states, a status word and a few scalars.  `work` must hold xf_workspace_bytes(ctx) bytes
+ *               (xf_rhs_workspace_bytes suffices for xf_convective_rhs).
+ *   Streams     `stream` is a cudaStream_t passed as void* (NULL = default stream).  Every call is asynchronous
+ *               on that stream except xf_create / xf_destroy / xf_status / the *_host calls.
+ *   Errors      Every call returns XF_OK or a negative code.  Argument errors are detected on the host before
+ *               any launch (XF_EINVAL).  CUDA errors map to XF_ECUDA.  Physics failures (NaN, rho/T/p <= 0,
+ *               Newton not converged; the paper's error catcher) set a sticky device flag that
+ *               xf_status returns and clears.  No exceptions, no global mutable state: contexts are independent.
+ *               There is no CPU fallback: without a CUDA device xf_create fails with XF_ECUDA.
+ */
+#ifndef XF_H
+#define XF_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct xf_ctx xf_ctx; /* opaque, owned by the library */
+
+enum {
+  XF_OK = 0,
+  XF_EINVAL = -1,
+  XF_ECUDA = -2,
+  XF_ENOMEM = -3,
+  XF_ENONPHYSICAL = -4, /* NaN or rho, p, T <= 0 (or c~^2 <= 0 at a face) seen on the device */
+  XF_ENOCONV = -5       /* Newton iteration hit newton_maxit                                 */
+};
+
+enum { XF_BC_PERIODIC = 0, XF_BC_TRANSMISSIVE = 1, XF_BC_REFLECTIVE = 2, XF_BC_DIRICHLET = 3 };
+
+#define XF_MAX_SPECIES 16
+
+typedef struct {
+  int nx, ny, nz;          /* interior cells; == 1 -> direction inactive (no ghosts, no sweep)                  */
+  int ng;                  /* ghost width; must be 3 (WENO5)                                                    */
+  double dx, dy, dz;
+  int nspecies;            /* N in 1..XF_MAX_SPECIES; Nv = N + 4                                                */
+  double Ru;               /* universal gas constant in the caller's units (Eq. 7)                  */
+  const double *W;         /* host [N] molar masses                                                             */
+  const double *nasa7;     /* host [N][7] NASA-7 a1..a7, single range (a7 unused on this path)    */
+  double Tlo, Thi;         /* fit range; constant-cp continuation outside it (reading R3)                       */
+  int bc[6];               /* xlo, xhi, ylo, yhi, zlo, zhi: XF_BC_*                                             */
+  const double *bc_state;  /* host [6][Nv] conserved states of XF_BC_DIRICHLET faces, or NULL                   */
+  double newton_rtol;      /* |dT| <= rtol |T|; 0 -> 1e-13 (reading R4)                                         */
+  int newton_maxit;        /* 0 -> 50                                                                           */
+  int device;              /* CUDA ordinal                                                                      */
+} xf_config;
+
+/* Create a context: validates cfg, copies every host table, uploads boundary states.  Synchronous. */
+int xf_create(xf_ctx **out, const xf_config *cfg);
+int xf_destroy(xf_ctx *ctx);
+
+size_t xf_num_vars(const xf_ctx *ctx);            /* Nv                                                        */
+size_t xf_padded_cells(const xf_ctx *ctx);        /* product of padded extents                                 */
+size_t xf_rhs_workspace_bytes(const xf_ctx *ctx); /* scratch for xf_convective_rhs: (N + 3) fields             */
+size_t xf_workspace_bytes(const xf_ctx *ctx);     /* scratch for xf_rk3_step: the above + 3 U-sized buffers    */
+
+/* Ghost-cell fill ("specific boundary conditions"; reading R10): periodic wrap,
+ * transmissive copy of the nearest interior cell, reflective mirror with the wall-normal momentum negated, or the
+ * stored Dirichlet state; 3 layers; x, then y, then z, so that edges and corners are defined.  U in place. */
+int xf_fill_ghosts(xf_ctx *ctx, double *U, void *stream);
+
+/* Primitive recovery for every padded cell (Eq. 21): T by Newton iteration on
+ * e(T) = sum_s Y_s h_s(T) - Rbar T with Cv = sum_s Y_s cp_s - Rbar; then p = rho Rbar T (Eq. 7) and the frozen
+ * sound speed c.  T: in = starting guess, out = temperature.  p and/or c may be NULL.  U must have valid ghosts. */
+int xf_primitives(xf_ctx *ctx, const double *U, double *T, double *p, double *c, void *stream);
+
+/* One convective residual L(U) = -sum_d (Fhat_{i+1/2} - Fhat_{i-1/2})/dx_d (Eq. 13) with
+ * characteristic-wise WENO5 reconstruction, local Lax-Friedrichs splitting (Eq. 14) on the
+ * Roe-averaged eigensystem and back-projection (Eq. 15).  Does: ghost fill (U's ghosts are
+ * overwritten, interior read-only), primitives (T in/out), the x, y, z sweeps.  rhs is [Nv][padded]; only interior
+ * entries are written.  work: xf_rhs_workspace_bytes. */
+int xf_convective_rhs(xf_ctx *ctx, double *U, double *T, double *rhs, void *work, void *stream);
+
+/* One SSP-RK3 step with fixed dt (Eq. 16): three times (ghost fill, primitives, residual,
+ * stage combination).  U: in U^n, out U^{n+1} (interior; ghosts are left as filled for the last stage).
+ * work: xf_workspace_bytes. */
+int xf_rk3_step(xf_ctx *ctx, double *U, double *T, double dt, void *work, void *stream);
+
+/* As xf_rk3_step with dt = cfl / (*S_dev) read on the device (no host round trip); S_dev as written by
+ * xf_max_wavespeed on the same stream. */
+int xf_rk3_step_cfl(xf_ctx *ctx, double *U, double *T, double cfl, const double *S_dev, void *work, void *stream);
+
+/* S = max over interior cells of sum_{d active} (|u_d| + c)/dx_d, so that dt = CFL / S (Eq. 17,
+ * PAPER.md:429; reading R9).  Recovers T of the interior cells on the way (T in/out).  S_dev: 1 double, device. */
+int xf_max_wavespeed(xf_ctx *ctx, const double *U, double *T, double *S_dev, void *stream);
+
+/* Synchronises `stream`, returns XF_OK / XF_ENONPHYSICAL / XF_ENOCONV from the sticky device flag and clears it. */
+int xf_status(xf_ctx *ctx, void *stream);
+
+/* Mean Newton iteration count of the last xf_primitives launch (debug counter; synchronises the stream). */
+int xf_newton_mean_iterations(xf_ctx *ctx, void *stream, double *mean_out);
+
+/* Number of kernel launches issued through this context since xf_create (for bench.py's gpu_launches). */
+long xf_launch_count(const xf_ctx *ctx);
+
+/* HOST-buffer entry points (end-to-end measurement): copy in, run on the device, copy out.  Device scratch is
+ * allocated inside the context on first use and freed by xf_destroy.  Synchronous.
+ *   xf_convective_rhs_host: U_host [Nv][padded] in, T_host [padded] in/out, rhs_host [Nv][padded] out.
+ *   xf_rk3_steps_host:      nsteps steps with dt = cfl / S recomputed every step on the device; U_host, T_host
+ *                           in/out; *t_advanced (may be NULL) receives the sum of the time steps. */
+int xf_convective_rhs_host(xf_ctx *ctx, const double *U_host, double *T_host, double *rhs_host);
+int xf_rk3_steps_host(xf_ctx *ctx, double *U_host, double *T_host, double cfl, int nsteps, double *t_advanced);
+
+/* Measurement aid for the roofline denominator: runs a register-resident chain of dependent-free fp64 FMAs on
+ * every SM for `iters` rounds and returns the achieved TFLOP/s (2 flops per FMA) in *tflops.  Synchronous. */
+int xf_probe_fp64_peak(int device, int iters, double *tflops, double *ms);
+
+const char *xf_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* XF_H */

@@ -1,0 +1,416 @@
+// xf_api.cu -- the C ABI of libxf.so (include/xf.h): context, argument checks, launch sequencing.
+// Every step of the path runs in the kernels of this directory; nothing here computes on the host.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "xf_common.cuh"
+
+int xf_sweep_x_init();
+int xf_sweep_y_init();
+int xf_sweep_z_init();
+int xf_probe_fp64_launch(int blocks, int threads, int iters, double *sink, cudaStream_t s);
+
+struct xf_ctx {
+  XfGrid G;
+  XfThermo Th;
+  XfBc bc;
+  int N, Nv, device;
+  int *status_dev;                    // sticky flag word
+  unsigned long long *itersum_dev;    // Newton iteration counter of the last xf_primitives launch
+  double *bc_state_dev;               // [6][XF_MAXNV]
+  double *S_dev;                      // max wave speed scalar used by the host-buffer entry points
+  long launches;
+  // lazily allocated device mirrors for the *_host entry points
+  double *hU, *hT, *hR;
+  void *hW;
+};
+
+namespace {
+
+struct DeviceGuard {
+  int prev;
+  bool ok;
+  explicit DeviceGuard(int dev) : prev(-1), ok(false) {
+    if (cudaGetDevice(&prev) != cudaSuccess) return;
+    ok = prev == dev || cudaSetDevice(dev) == cudaSuccess;
+    if (prev == dev) prev = -1;
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+
+inline size_t field_bytes(const xf_ctx *c) { return sizeof(double) * (size_t)c->G.cells; }
+
+// primitive fields kept between the primitives kernel and the sweeps: p, c, Gamma, chi_1..chi_N
+struct PrimFields {
+  double *p, *c, *Gam, *chi;
+};
+inline PrimFields prim_fields(const xf_ctx *c, void *work) {
+  double *w = static_cast<double *>(work);
+  const size_t n = (size_t)c->G.cells;
+  return PrimFields{w, w + n, w + 2 * n, w + 3 * n};
+}
+
+int count_active(const XfGrid &G) { return (G.n[0] > 1) + (G.n[1] > 1) + (G.n[2] > 1); }
+
+// ghosts -> primitives -> sweeps.  E_last describes what the LAST active sweep writes (residual or RK combine);
+// earlier sweeps accumulate the partial residual in `acc`.
+int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfEpilogue &E_last, cudaStream_t s) {
+  int rc = xf_launch_ghosts(c->G, c->Nv, c->bc, c->bc_state_dev, U, s, &c->launches);
+  if (rc != XF_OK) return rc;
+  const PrimFields F = prim_fields(c, work);
+  rc = xf_launch_prim(c->G, c->Th, U, T, F.p, F.c, F.Gam, F.chi, c->status_dev, nullptr, s);
+  ++c->launches;
+  if (rc != XF_OK) return rc;
+  const int nact = count_active(c->G);
+  int done = 0;
+  for (int d = 0; d < 3; ++d) {
+    if (c->G.n[d] == 1) continue;
+    XfEpilogue E;
+    if (done == nact - 1) {
+      E = E_last;
+      E.has_acc = done > 0;
+      if (E.mode != 2) E.mode = done > 0 ? 1 : 0;
+      E.acc = acc;
+    } else {
+      memset(&E, 0, sizeof(E));
+      E.mode = done > 0 ? 1 : 0;
+      E.acc = acc;
+      E.out = acc;
+    }
+    if (d == 0) rc = xf_launch_sweep_x(c->G, c->N, U, F.p, F.c, F.Gam, F.chi, E, c->status_dev, s);
+    else if (d == 1) rc = xf_launch_sweep_y(c->G, c->N, U, F.p, F.c, F.Gam, F.chi, E, c->status_dev, s);
+    else rc = xf_launch_sweep_z(c->G, c->N, U, F.p, F.c, F.Gam, F.chi, E, c->status_dev, s);
+    ++c->launches;
+    if (rc != XF_OK) return rc;
+    ++done;
+  }
+  return XF_OK;
+}
+
+int rk3(xf_ctx *c, double *U, double *T, double dt, double cfl, const double *S_dev, void *work, cudaStream_t s) {
+  const size_t n = (size_t)c->G.cells;
+  double *w = static_cast<double *>(work);
+  double *U1 = w + (size_t)(c->N + 3) * n;
+  double *U2 = U1 + (size_t)c->Nv * n;
+  double *acc = U2 + (size_t)c->Nv * n;
+  XfEpilogue E;
+  memset(&E, 0, sizeof(E));
+  E.mode = 2;
+  E.dt = dt;
+  E.cfl = cfl;
+  E.S_dev = S_dev;
+  E.Un = U;
+  // Eq. 16: U1 = Un + dt L(Un); U2 = 3/4 Un + 1/4 (U1 + dt L(U1)); Un+1 = 1/3 Un + 2/3 (U2 + dt L(U2))
+  E.alpha = 0.0; E.beta = 1.0; E.out = U1;
+  int rc = residual(c, U, T, work, acc, E, s);
+  if (rc != XF_OK) return rc;
+  E.alpha = 0.75; E.beta = 0.25; E.out = U2;
+  rc = residual(c, U1, T, work, acc, E, s);
+  if (rc != XF_OK) return rc;
+  E.alpha = 1.0 / 3.0; E.beta = 2.0 / 3.0; E.out = U;
+  return residual(c, U2, T, work, acc, E, s);
+}
+
+int ensure_host_mirrors(xf_ctx *c) {
+  if (c->hU) return XF_OK;
+  const size_t fb = field_bytes(c);
+  if (cudaMalloc(&c->hU, fb * c->Nv) != cudaSuccess) return XF_ENOMEM;
+  if (cudaMalloc(&c->hT, fb) != cudaSuccess) return XF_ENOMEM;
+  if (cudaMalloc(&c->hR, fb * c->Nv) != cudaSuccess) return XF_ENOMEM;
+  if (cudaMalloc(&c->hW, xf_workspace_bytes(c)) != cudaSuccess) return XF_ENOMEM;
+  return XF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int xf_create(xf_ctx **out, const xf_config *cfg) {
+  if (!out || !cfg) return XF_EINVAL;
+  *out = nullptr;
+  const int N = cfg->nspecies;
+  if (cfg->ng != XF_NG || N < 1 || N > XF_MAXN || cfg->nx < 1 || cfg->ny < 1 || cfg->nz < 1) return XF_EINVAL;
+  if (!cfg->W || !cfg->nasa7 || !(cfg->Ru > 0.0) || !(cfg->Thi > cfg->Tlo)) return XF_EINVAL;
+  const int n[3] = {cfg->nx, cfg->ny, cfg->nz};
+  const double dxs[3] = {cfg->dx, cfg->dy, cfg->dz};
+  for (int d = 0; d < 3; ++d) {
+    if (n[d] == 1) continue;
+    if (!(dxs[d] > 0.0)) return XF_EINVAL;
+    if (n[d] < XF_NG) return XF_EINVAL;  // ghost layers are copies of interior layers: need >= 3 of them
+    for (int side = 0; side < 2; ++side) {
+      const int b = cfg->bc[2 * d + side];
+      if (b < XF_BC_PERIODIC || b > XF_BC_DIRICHLET) return XF_EINVAL;
+      if (b == XF_BC_DIRICHLET && !cfg->bc_state) return XF_EINVAL;
+    }
+    if ((cfg->bc[2 * d] == XF_BC_PERIODIC) != (cfg->bc[2 * d + 1] == XF_BC_PERIODIC)) return XF_EINVAL;
+  }
+  for (int s = 0; s < N; ++s)
+    if (!(cfg->W[s] > 0.0)) return XF_EINVAL;
+  if (n[0] == 1 && n[1] == 1 && n[2] == 1) return XF_EINVAL;
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev) return XF_ECUDA;
+  DeviceGuard guard(cfg->device);
+  if (!guard.ok) return XF_ECUDA;
+
+  xf_ctx *c = new (std::nothrow) xf_ctx;
+  if (!c) return XF_ENOMEM;
+  memset(c, 0, sizeof(*c));
+  c->N = N;
+  c->Nv = N + 4;
+  c->device = cfg->device;
+  XfGrid &G = c->G;
+  for (int d = 0; d < 3; ++d) {
+    G.n[d] = n[d];
+    G.g[d] = n[d] > 1 ? XF_NG : 0;
+    G.np[d] = n[d] + 2 * G.g[d];
+    G.inv_d[d] = n[d] > 1 ? 1.0 / dxs[d] : 0.0;
+  }
+  G.st[0] = 1;
+  G.st[1] = G.np[0];
+  G.st[2] = (long long)G.np[0] * G.np[1];
+  G.cells = (long long)G.np[0] * G.np[1] * G.np[2];
+
+  XfThermo &Th = c->Th;
+  Th.N = N;
+  Th.Tlo = cfg->Tlo;
+  Th.Thi = cfg->Thi;
+  Th.rtol = cfg->newton_rtol > 0.0 ? cfg->newton_rtol : 1e-13;
+  Th.maxit = cfg->newton_maxit > 0 ? cfg->newton_maxit : 50;
+  for (int s = 0; s < N; ++s) {
+    const double *a = cfg->nasa7 + 7 * s;
+    Th.Rs[s] = cfg->Ru / cfg->W[s];
+    for (int q = 0; q < 6; ++q) Th.a[s][q] = a[q];
+    for (int q = 0; q < 4; ++q) Th.b[s][q] = a[q + 1] / (double)(q + 2);
+  }
+  for (int q = 0; q < 6; ++q) c->bc.kind[q] = cfg->bc[q];
+
+  bool ok = cudaMalloc(&c->status_dev, sizeof(int)) == cudaSuccess &&
+            cudaMalloc(&c->itersum_dev, sizeof(unsigned long long)) == cudaSuccess &&
+            cudaMalloc(&c->bc_state_dev, sizeof(double) * 6 * XF_MAXNV) == cudaSuccess &&
+            cudaMalloc(&c->S_dev, sizeof(double)) == cudaSuccess;
+  if (ok) {
+    double bs[6 * XF_MAXNV];
+    memset(bs, 0, sizeof(bs));
+    if (cfg->bc_state)
+      for (int q = 0; q < 6; ++q)
+        for (int v = 0; v < c->Nv; ++v) bs[q * XF_MAXNV + v] = cfg->bc_state[q * c->Nv + v];
+    ok = cudaMemcpy(c->bc_state_dev, bs, sizeof(bs), cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemset(c->status_dev, 0, sizeof(int)) == cudaSuccess &&
+         cudaMemset(c->itersum_dev, 0, sizeof(unsigned long long)) == cudaSuccess;
+  }
+  if (ok) ok = xf_sweep_x_init() == XF_OK && xf_sweep_y_init() == XF_OK && xf_sweep_z_init() == XF_OK;
+  if (!ok) {
+    xf_destroy(c);
+    return XF_ECUDA;
+  }
+  *out = c;
+  return XF_OK;
+}
+
+int xf_destroy(xf_ctx *c) {
+  if (!c) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  cudaFree(c->status_dev);
+  cudaFree(c->itersum_dev);
+  cudaFree(c->bc_state_dev);
+  cudaFree(c->S_dev);
+  cudaFree(c->hU);
+  cudaFree(c->hT);
+  cudaFree(c->hR);
+  cudaFree(c->hW);
+  delete c;
+  return XF_OK;
+}
+
+size_t xf_num_vars(const xf_ctx *c) { return c ? (size_t)c->Nv : 0; }
+size_t xf_padded_cells(const xf_ctx *c) { return c ? (size_t)c->G.cells : 0; }
+size_t xf_rhs_workspace_bytes(const xf_ctx *c) { return c ? field_bytes(c) * (size_t)(c->N + 3) : 0; }
+size_t xf_workspace_bytes(const xf_ctx *c) {
+  return c ? field_bytes(c) * (size_t)(c->N + 3 + 3 * c->Nv) : 0;
+}
+
+int xf_fill_ghosts(xf_ctx *c, double *U, void *stream) {
+  if (!c || !U) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  return xf_launch_ghosts(c->G, c->Nv, c->bc, c->bc_state_dev, U, static_cast<cudaStream_t>(stream), &c->launches);
+}
+
+int xf_primitives(xf_ctx *c, const double *U, double *T, double *p, double *cs, void *stream) {
+  if (!c || !U || !T) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (cudaMemsetAsync(c->itersum_dev, 0, sizeof(unsigned long long), s) != cudaSuccess) return XF_ECUDA;
+  ++c->launches;
+  return xf_launch_prim(c->G, c->Th, U, T, p, cs, nullptr, nullptr, c->status_dev, c->itersum_dev, s);
+}
+
+int xf_convective_rhs(xf_ctx *c, double *U, double *T, double *rhs, void *work, void *stream) {
+  if (!c || !U || !T || !rhs || !work) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  XfEpilogue E;
+  memset(&E, 0, sizeof(E));
+  E.mode = 0;
+  E.out = rhs;
+  return residual(c, U, T, work, rhs, E, static_cast<cudaStream_t>(stream));
+}
+
+int xf_rk3_step(xf_ctx *c, double *U, double *T, double dt, void *work, void *stream) {
+  if (!c || !U || !T || !work || !(dt == dt)) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  return rk3(c, U, T, dt, 0.0, nullptr, work, static_cast<cudaStream_t>(stream));
+}
+
+int xf_rk3_step_cfl(xf_ctx *c, double *U, double *T, double cfl, const double *S_dev, void *work, void *stream) {
+  if (!c || !U || !T || !work || !S_dev || !(cfl > 0.0)) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  return rk3(c, U, T, 0.0, cfl, S_dev, work, static_cast<cudaStream_t>(stream));
+}
+
+int xf_max_wavespeed(xf_ctx *c, const double *U, double *T, double *S_dev, void *stream) {
+  if (!c || !U || !T || !S_dev) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  ++c->launches;
+  return xf_launch_wavespeed(c->G, c->Th, U, T, S_dev, c->status_dev, static_cast<cudaStream_t>(stream));
+}
+
+int xf_status(xf_ctx *c, void *stream) {
+  if (!c) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  int flag = 0;
+  if (cudaMemcpyAsync(&flag, c->status_dev, sizeof(int), cudaMemcpyDeviceToHost, s) != cudaSuccess) return XF_ECUDA;
+  if (cudaMemsetAsync(c->status_dev, 0, sizeof(int), s) != cudaSuccess) return XF_ECUDA;
+  if (cudaStreamSynchronize(s) != cudaSuccess) return XF_ECUDA;
+  if (flag & XF_FLAG_NONPHYSICAL) return XF_ENONPHYSICAL;
+  if (flag & XF_FLAG_NOCONV) return XF_ENOCONV;
+  return XF_OK;
+}
+
+int xf_newton_mean_iterations(xf_ctx *c, void *stream, double *mean_out) {
+  if (!c || !mean_out) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  unsigned long long sum = 0;
+  if (cudaMemcpyAsync(&sum, c->itersum_dev, sizeof(sum), cudaMemcpyDeviceToHost, s) != cudaSuccess) return XF_ECUDA;
+  if (cudaStreamSynchronize(s) != cudaSuccess) return XF_ECUDA;
+  *mean_out = (double)sum / (double)c->G.cells;
+  return XF_OK;
+}
+
+long xf_launch_count(const xf_ctx *c) { return c ? c->launches : 0; }
+
+int xf_convective_rhs_host(xf_ctx *c, const double *U_host, double *T_host, double *rhs_host) {
+  if (!c || !U_host || !T_host || !rhs_host) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  int rc = ensure_host_mirrors(c);
+  if (rc != XF_OK) return rc;
+  const size_t fb = field_bytes(c);
+  cudaStream_t s = nullptr;
+  if (cudaMemcpyAsync(c->hU, U_host, fb * c->Nv, cudaMemcpyHostToDevice, s) != cudaSuccess) return XF_ECUDA;
+  if (cudaMemcpyAsync(c->hT, T_host, fb, cudaMemcpyHostToDevice, s) != cudaSuccess) return XF_ECUDA;
+  if (cudaMemsetAsync(c->hR, 0, fb * c->Nv, s) != cudaSuccess) return XF_ECUDA;
+  XfEpilogue E;
+  memset(&E, 0, sizeof(E));
+  E.out = c->hR;
+  rc = residual(c, c->hU, c->hT, c->hW, c->hR, E, s);
+  if (rc != XF_OK) return rc;
+  if (cudaMemcpyAsync(rhs_host, c->hR, fb * c->Nv, cudaMemcpyDeviceToHost, s) != cudaSuccess) return XF_ECUDA;
+  if (cudaMemcpyAsync(T_host, c->hT, fb, cudaMemcpyDeviceToHost, s) != cudaSuccess) return XF_ECUDA;
+  return cudaStreamSynchronize(s) == cudaSuccess ? XF_OK : XF_ECUDA;
+}
+
+int xf_rk3_steps_host(xf_ctx *c, double *U_host, double *T_host, double cfl, int nsteps, double *t_advanced) {
+  if (!c || !U_host || !T_host || !(cfl > 0.0) || nsteps < 0) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  int rc = ensure_host_mirrors(c);
+  if (rc != XF_OK) return rc;
+  const size_t fb = field_bytes(c);
+  cudaStream_t s = nullptr;
+  if (cudaMemcpyAsync(c->hU, U_host, fb * c->Nv, cudaMemcpyHostToDevice, s) != cudaSuccess) return XF_ECUDA;
+  if (cudaMemcpyAsync(c->hT, T_host, fb, cudaMemcpyHostToDevice, s) != cudaSuccess) return XF_ECUDA;
+  double t = 0.0;
+  for (int k = 0; k < nsteps; ++k) {
+    ++c->launches;
+    rc = xf_launch_wavespeed(c->G, c->Th, c->hU, c->hT, c->S_dev, c->status_dev, s);
+    if (rc != XF_OK) return rc;
+    rc = rk3(c, c->hU, c->hT, 0.0, cfl, c->S_dev, c->hW, s);
+    if (rc != XF_OK) return rc;
+    if (t_advanced) {
+      double S = 0.0;
+      if (cudaMemcpyAsync(&S, c->S_dev, sizeof(double), cudaMemcpyDeviceToHost, s) != cudaSuccess) return XF_ECUDA;
+      if (cudaStreamSynchronize(s) != cudaSuccess) return XF_ECUDA;
+      t += cfl / S;
+    }
+  }
+  if (cudaMemcpyAsync(U_host, c->hU, fb * c->Nv, cudaMemcpyDeviceToHost, s) != cudaSuccess) return XF_ECUDA;
+  if (cudaMemcpyAsync(T_host, c->hT, fb, cudaMemcpyDeviceToHost, s) != cudaSuccess) return XF_ECUDA;
+  if (cudaStreamSynchronize(s) != cudaSuccess) return XF_ECUDA;
+  if (t_advanced) *t_advanced = t;
+  return XF_OK;
+}
+
+int xf_probe_fp64_peak(int device, int iters, double *tflops, double *ms_out) {
+  if (!tflops || iters < 1) return XF_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return XF_ECUDA;
+  DeviceGuard guard(device);
+  if (!guard.ok) return XF_ECUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return XF_ECUDA;
+  const int threads = 256, blocks = prop.multiProcessorCount * 8;
+  double *sink = nullptr;
+  if (cudaMalloc(&sink, sizeof(double) * (size_t)blocks * threads) != cudaSuccess) return XF_ENOMEM;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  int rc = xf_probe_fp64_launch(blocks, threads, iters / 8 + 1, sink, nullptr);  // warm-up
+  float best = 1e30f;
+  for (int rep = 0; rep < 5 && rc == XF_OK; ++rep) {
+    cudaEventRecord(e0, nullptr);
+    rc = xf_probe_fp64_launch(blocks, threads, iters, sink, nullptr);
+    cudaEventRecord(e1, nullptr);
+    if (cudaEventSynchronize(e1) != cudaSuccess) rc = XF_ECUDA;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (ms < best) best = ms;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(sink);
+  if (rc != XF_OK) return rc;
+  // 16 independent chains x 8 FMAs per round x 2 flops
+  const double flops = 2.0 * 16.0 * 8.0 * (double)iters * (double)blocks * (double)threads;
+  *tflops = flops / ((double)best * 1e-3) * 1e-12;
+  if (ms_out) *ms_out = best;
+  return XF_OK;
+}
+
+const char *xf_strerror(int code) {
+  switch (code) {
+    case XF_OK: return "ok";
+    case XF_EINVAL: return "invalid argument";
+    case XF_ECUDA: return "CUDA error (no device, bad device ordinal or launch failure)";
+    case XF_ENOMEM: return "out of device memory";
+    case XF_ENONPHYSICAL: return "non-physical state on the device (NaN or rho, p, T <= 0)";
+    case XF_ENOCONV: return "Newton iteration for T(e) did not converge";
+    default: return "unknown error";
+  }
+}
+
+}  // extern "C"

@@ -1,0 +1,81 @@
+// xf_common.cuh -- shared declarations of the CUDA path (sm_100a).  No code is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/xf.h"
+
+#define XF_NG 3
+#define XF_MAXN XF_MAX_SPECIES
+#define XF_MAXNV (XF_MAXN + 4)
+
+// status bits on the device (sticky word owned by the context)
+#define XF_FLAG_NONPHYSICAL 1
+#define XF_FLAG_NOCONV 2
+
+// Grid geometry handed to every kernel by value (lives in the kernel-parameter constant bank).
+struct XfGrid {
+  int n[3];        // interior cells per direction
+  int np[3];       // padded extents
+  int g[3];        // ghost width per direction (0 if inactive)
+  long long st[3]; // element strides of i, j, k
+  long long cells; // padded cells
+  double inv_d[3]; // 1/dx, 1/dy, 1/dz
+};
+
+// Species table in evaluation form, handed to the thermo kernels by value (constant bank, <= 4 KB):
+//   cp_s/R_s = a0 + a1 T + a2 T^2 + a3 T^3 + a4 T^4            (NASA polynomials; Horner)
+//   h_s/R_s  = T (a0 + b1 T + b2 T^2 + b3 T^3 + b4 T^4) + a5,   b_k = a_k/(k+1)
+struct XfThermo {
+  double Rs[XF_MAXN];
+  double a[XF_MAXN][6];  // a0..a4, a5 (enthalpy constant)
+  double b[XF_MAXN][4];  // a1/2, a2/3, a3/4, a4/5
+  double Tlo, Thi;
+  double rtol;
+  int maxit;
+  int N;
+};
+
+struct XfBc {
+  int kind[6];
+};
+
+// How a sweep writes its flux divergence: out = alpha*Un + beta*(Us + dt*(acc + div)).
+struct XfEpilogue {
+  int mode;           // 0: out = div (first sweep of a plain rhs); 1: out = acc + div; 2: RK stage combine
+  int has_acc;        // mode 2: whether a previous sweep left a partial rhs in `acc`
+  double alpha, beta; // mode 2: stage weights of Eq. 16
+  double dt;          // mode 2: time step, used when S_dev == nullptr
+  double cfl;         // mode 2: dt = cfl / *S_dev otherwise
+  const double *S_dev;
+  const double *acc;  // partial rhs of earlier sweeps [Nv][padded]
+  const double *Un;   // U^n  [Nv][padded] (mode 2)
+  double *out;        // rhs or U^{s+1} [Nv][padded]
+};
+
+// launch helpers implemented per translation unit
+int xf_launch_prim(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *p, double *c,
+                   double *Gam, double *chi, int *status, unsigned long long *itersum, cudaStream_t s);
+int xf_launch_wavespeed(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *S_dev, int *status,
+                        cudaStream_t s);
+int xf_launch_ghosts(const XfGrid &G, int Nv, const XfBc &bc, const double *bc_state_dev, double *U, cudaStream_t s,
+                     long *launches);
+int xf_launch_sweep_x(const XfGrid &G, int N, const double *U, const double *p, const double *c, const double *Gam,
+                      const double *chi, const XfEpilogue &E, int *status, cudaStream_t s);
+int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *p, const double *c, const double *Gam,
+                      const double *chi, const XfEpilogue &E, int *status, cudaStream_t s);
+int xf_launch_sweep_z(const XfGrid &G, int N, const double *U, const double *p, const double *c, const double *Gam,
+                      const double *chi, const XfEpilogue &E, int *status, cudaStream_t s);
+int xf_sweeps_init();  // opt in to large dynamic shared memory once per process
+
+// fp64 reciprocal: MUFU.RCP64H seed + two Newton steps (4 DFMA); relative error <= ~2 ulp for normal inputs.
+// The path is bound by the fp64 pipe, and an IEEE division costs about three times as many pipe slots.
+__device__ __forceinline__ double xf_rcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  return r;
+}

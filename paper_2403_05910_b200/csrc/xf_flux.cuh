@@ -1,0 +1,212 @@
+// xf_flux.cuh -- directional reconstruct-and-flux sweeps for sm_100a (the hot loop: Eq. 13-15).
+//
+// One thread computes one face flux Fhat_{i+1/2} = R (F+ + F-) from the six stencil cells staged in shared memory:
+//   * Roe-type average of the two adjacent cells (reading R5), c~^2 from the identity that makes L R = I;
+//   * the eigenvector matrices are never formed: L V needs one dense functional pi.V (Nv FMAs) plus sparse rows,
+//     and because F_m = u_m U_m + p_m (e_n + u_m e_E), the projected flux L F_m is u_m (L U_m) plus a pressure term
+//     that is non-zero only for the two acoustic fields and the entropy field -- so the flux is never projected;
+//   * local Lax-Friedrichs splitting (Eq. 14; reading R8), WENO5-JS in a common-denominator form with a single
+//     reciprocal per reconstruction (reading R7), back-projection with the structure of R (Eq. 15);
+//   * the face fluxes of a chunk go to shared memory, the flux difference (Eq. 13) is formed per cell and written
+//     out either as a residual or directly as the Runge-Kutta stage combination (Eq. 16).
+// The fp64 pipe bounds this path, so the code minimises fp64 instructions, not bytes.
+#pragma once
+#include "xf_common.cuh"
+
+namespace xf {
+
+// WENO5-JS value at +1/2 from point values v0..v4 = v_{-2}..v_{+2} (Jiang & Shu; eps = 1e-6, exponent 2).
+// Written on first differences D_k; smoothness indicators scaled by 4 (cancels in the weights);
+//   result = v2 + (D2 + 2 D3)/6 + [ (2/3) P0 (d0 - d1) + P2 (d1 - d2) ] / [ 2 P0 + 12 P1 + 6 P2 ],
+// with P0 = (s1 s2)^2, P1 = (s0 s2)^2, P2 = (s0 s1)^2, s_k = 4 (eps + beta_k): the Jiang-Shu weights
+// d_k/(eps+beta_k)^2 brought to a common denominator, so one reciprocal instead of four divisions.
+__device__ __forceinline__ double weno5(double v0, double v1, double v2, double v3, double v4) {
+  const double D1 = v1 - v0, D2 = v2 - v1, D3 = v3 - v2, D4 = v4 - v3;
+  const double d0 = D2 - D1, d1 = D3 - D2, d2 = D4 - D3;
+  const double e0 = fma(3.0, D2, -D1);   // v0 - 4 v1 + 3 v2
+  const double e1 = D2 + D3;             // v3 - v1
+  const double e2 = fma(-3.0, D3, D4);   // 3 v2 - 4 v3 + v4
+  const double k133 = 13.0 / 3.0, eps4 = 4.0e-6;
+  const double s0 = fma(e0, e0, fma(k133 * d0, d0, eps4));
+  const double s1 = fma(e1, e1, fma(k133 * d1, d1, eps4));
+  const double s2 = fma(e2, e2, fma(k133 * d2, d2, eps4));
+  const double p12 = s1 * s2, p02 = s0 * s2, p01 = s0 * s1;
+  const double P0 = p12 * p12, P1 = p02 * p02, P2 = p01 * p01;
+  const double num = fma(P0 * (d0 - d1), 2.0 / 3.0, P2 * (d1 - d2));
+  const double den = fma(2.0, P0, fma(12.0, P1, 6.0 * P2));
+  const double base = fma(fma(2.0, D3, D2), 1.0 / 6.0, v2);
+  return fma(num, xf_rcp(den), base);
+}
+
+template <int DIR> struct Axes;
+template <> struct Axes<0> { static constexpr int nd = 0, t1 = 1, t2 = 2; };
+template <> struct Axes<1> { static constexpr int nd = 1, t1 = 0, t2 = 2; };
+template <> struct Axes<2> { static constexpr int nd = 2, t1 = 1, t2 = 0; };
+
+// Shared-memory cell fields: 0..Nv-1 conserved variables, then p, c, u_n (normal velocity), 1/rho, sqrt(rho).
+__host__ __device__ constexpr int nfields(int N) { return N + 4 + 5; }
+
+// Numerical flux at one face.  sm: staged fields, field f of stencil cell m at sm[f*FS + o[m]] (m = 0..5 <-> i-2..i+3,
+// the face lies between m = 2 and m = 3).  ga, gb: global cell indices of those two cells (for Gamma, chi_s, which
+// are only needed at the two adjacent cells and are read straight from global memory).  Writes Fhat_v to fout[v*FOS].
+template <int N_T, int DIR>
+__device__ __forceinline__ void face_flux(const int N, const double *__restrict__ sm, const int FS, const int (&o)[6],
+                                          const double *__restrict__ Gam, const double *__restrict__ chi,
+                                          const long long ga, const long long gb, const long long cells,
+                                          double *__restrict__ fout, const int FOS, int *__restrict__ status) {
+  constexpr int nd = Axes<DIR>::nd, t1 = Axes<DIR>::t1, t2 = Axes<DIR>::t2;
+  const int Nv = N + 4;
+  const int FP = Nv, FC = Nv + 1, FUD = Nv + 2, FRI = Nv + 3, FSR = Nv + 4;
+#define XS(f, m) sm[(f) * FS + o[m]]
+
+  // ---- Roe-type average (reading R5): q~ = (w_a q_a + w_b q_b)/(w_a + w_b), w = sqrt(rho)
+  const double wa = XS(FSR, 2), wb = XS(FSR, 3);
+  const double winv = xf_rcp(wa + wb);
+  const double oa = wa * winv, ob = wb * winv;
+  const double oma = oa * XS(FRI, 2), omb = ob * XS(FRI, 3);  // weights acting on conserved quantities
+  double ut[3];
+#pragma unroll
+  for (int q = 0; q < 3; ++q) ut[q] = fma(oma, XS(1 + q, 2), omb * XS(1 + q, 3));
+  const double Ht = fma(oma, XS(4, 2) + XS(FP, 2), omb * (XS(4, 3) + XS(FP, 3)));
+  const double Gt = fma(oa, Gam[ga], ob * Gam[gb]);
+  const double kt = 0.5 * fma(ut[0], ut[0], fma(ut[1], ut[1], ut[2] * ut[2]));
+  const double chiN = fma(oa, chi[(N - 1) * cells + ga], ob * chi[(N - 1) * cells + gb]);
+
+  // ---- the dense functional pi.U_m for the six stencil cells; species part first
+  double rho[6], piU[6];
+#pragma unroll
+  for (int m = 0; m < 6; ++m) {
+    rho[m] = XS(0, m);
+    piU[m] = 0.0;
+  }
+  double c2acc = 0.0;
+#pragma unroll 3
+  for (int i = 0; i < N - 1; ++i) {
+    const double zeta = fma(oa, chi[i * cells + ga], ob * chi[i * cells + gb]) - chiN;
+    double y[6];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) y[m] = XS(5 + i, m);
+    const double Yt = fma(oma, y[2], omb * y[3]);
+    c2acc = fma(Yt, zeta, c2acc);
+#pragma unroll
+    for (int m = 0; m < 6; ++m) piU[m] = fma(zeta, y[m], piU[m]);
+  }
+  // c~^2 = sum_s Y~_s chi~_s + Gamma~ (H~ - k~), with Y~_N = 1 - sum_{i<N} Y~_i
+  const double c2 = chiN + c2acc + Gt * (Ht - kt);
+  if (!(c2 > 0.0)) atomicOr(status, XF_FLAG_NONPHYSICAL);
+  const double ct = sqrt(c2);
+  const double h = 0.5 * xf_rcp(c2);  // 1/(2 c~^2)
+  const double Prho = fma(Gt, kt, chiN);
+
+  double nuU[6], ud[6], qp[6], rp[6];
+  double lam_m = 0.0, lam_0 = 0.0, lam_p = 0.0;  // LLF: max over the stencil of |u-c|, |u|, |u+c| (reading R8)
+#pragma unroll
+  for (int m = 0; m < 6; ++m) {
+    const double mdot = fma(ut[0], XS(1, m), fma(ut[1], XS(2, m), ut[2] * XS(3, m)));
+    piU[m] += fma(Prho, rho[m], Gt * (XS(4, m) - mdot));
+    nuU[m] = fma(-ut[nd], rho[m], XS(1 + nd, m));
+    ud[m] = XS(FUD, m);
+    const double cm = XS(FC, m);
+    lam_m = fmax(lam_m, fabs(ud[m] - cm));
+    lam_0 = fmax(lam_0, fabs(ud[m]));
+    lam_p = fmax(lam_p, fabs(ud[m] + cm));
+    const double ph = 0.5 * XS(FP, m) * h;             // p_m / (4 c~^2)
+    qp[m] = Gt * (ud[m] - ut[nd]) * ph;                // pressure terms of L F_m
+    rp[m] = ct * ph;
+  }
+
+  // ---- acoustic (u-c), entropy (u) and acoustic (u+c) fields
+  double g0, g1, gL;
+  {
+    double fp[6], fm[6];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) {
+      const double a = h * fma(-ct, nuU[m], piU[m]);
+      const double pt = qp[m] - rp[m];
+      fp[m] = fma(0.5 * (ud[m] + lam_m), a, pt);
+      fm[m] = fma(0.5 * (ud[m] - lam_m), a, pt);
+    }
+    g0 = weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + weno5(fm[5], fm[4], fm[3], fm[2], fm[1]);
+#pragma unroll
+    for (int m = 0; m < 6; ++m) {
+      const double a = h * fma(ct, nuU[m], piU[m]);
+      const double pt = qp[m] + rp[m];
+      fp[m] = fma(0.5 * (ud[m] + lam_p), a, pt);
+      fm[m] = fma(0.5 * (ud[m] - lam_p), a, pt);
+    }
+    gL = weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + weno5(fm[5], fm[4], fm[3], fm[2], fm[1]);
+  }
+  double ap[6], am[6];  // (u_m +- Lambda_u)/2 for all fields that travel with u
+#pragma unroll
+  for (int m = 0; m < 6; ++m) {
+    ap[m] = 0.5 * (ud[m] + lam_0);
+    am[m] = 0.5 * (ud[m] - lam_0);
+  }
+  {
+    double fp[6], fm[6];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) {
+      const double a = fma(-2.0 * h, piU[m], rho[m]);
+      const double pt = -2.0 * qp[m];
+      fp[m] = fma(ap[m], a, pt);
+      fm[m] = fma(am[m], a, pt);
+    }
+    g1 = weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + weno5(fm[5], fm[4], fm[3], fm[2], fm[1]);
+  }
+
+  // ---- back-projection Fhat = R g (Eq. 15), structured
+  const double s = g0 + g1 + gL;
+  const double delta = ct * (gL - g0);
+  const double invG = xf_rcp(Gt);
+  double F4 = fma(Ht, s, fma(ut[nd], delta, -(c2 * invG) * g1));
+  fout[0] = s;
+  fout[(1 + nd) * FOS] = fma(ut[nd], s, delta);
+
+  // ---- fields travelling with u: two shear fields, N-1 species fields.  alpha_m = V_m - C rho_m with
+  //      C = Roe average of V/rho; L F_m = u_m alpha_m, so f+-_m = (u_m +- Lambda)/2 * alpha_m.
+#define XF_LINEAR_FIELD(VIDX, DEXPR)                                                                   \
+  {                                                                                                    \
+    double V[6], fp[6], fm[6];                                                                         \
+    _Pragma("unroll") for (int m = 0; m < 6; ++m) V[m] = XS(VIDX, m);                                  \
+    const double C = fma(oma, V[2], omb * V[3]);                                                       \
+    _Pragma("unroll") for (int m = 0; m < 6; ++m) {                                                    \
+      const double a = fma(-C, rho[m], V[m]);                                                          \
+      fp[m] = ap[m] * a;                                                                               \
+      fm[m] = am[m] * a;                                                                               \
+    }                                                                                                  \
+    const double g = weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + weno5(fm[5], fm[4], fm[3], fm[2], fm[1]); \
+    fout[(VIDX) * FOS] = fma(C, s, g);                                                                 \
+    F4 = fma((DEXPR), g, F4);                                                                          \
+  }
+  XF_LINEAR_FIELD(1 + t1, C)
+  XF_LINEAR_FIELD(1 + t2, C)
+#pragma unroll 1
+  for (int i = 0; i < N - 1; ++i) {
+    const double zeta = fma(oa, chi[i * cells + ga], ob * chi[i * cells + gb]) - chiN;
+    XF_LINEAR_FIELD(5 + i, -zeta * invG)
+  }
+#undef XF_LINEAR_FIELD
+  fout[4 * FOS] = F4;
+#undef XS
+}
+
+// per-cell derived fields computed once at staging time
+__device__ __forceinline__ void derive_cell(double rho, double mn, double &ud, double &ri, double &sr) {
+  ri = xf_rcp(rho);
+  ud = mn * ri;
+  sr = sqrt(rho);
+}
+
+// out = alpha*Un + beta*(Us + dt*(acc + div)) or plain residual accumulation (see XfEpilogue)
+__device__ __forceinline__ void write_out(const XfEpilogue &E, double dt, long long gi, double div, double us) {
+  if (E.mode == 0) {
+    E.out[gi] = div;
+  } else if (E.mode == 1) {
+    E.out[gi] = E.acc[gi] + div;
+  } else {
+    const double L = E.has_acc ? E.acc[gi] + div : div;
+    E.out[gi] = fma(E.alpha, E.Un[gi], E.beta * fma(dt, L, us));
+  }
+}
+
+}  // namespace xf

@@ -1,0 +1,233 @@
+"""Thin ctypes binding of libxf.so (include/xf.h): argument marshalling only -- every step of the path runs in the
+CUDA kernels of csrc/.  PyTorch supplies device memory and streams; there is no CPU fallback: if the library is
+missing or no CUDA device is present, loading / ``xf_create`` fails loudly.
+
+Function names follow the C ABI (``xf_create``, ``xf_primitives``, ``xf_convective_rhs``, ``xf_rk3_step``,
+``xf_max_wavespeed`` ...); ``Context`` is a small RAII convenience around them.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+LIB_PATH = _HERE / "libxf.so"
+
+XF_OK, XF_EINVAL, XF_ECUDA, XF_ENOMEM, XF_ENONPHYSICAL, XF_ENOCONV = 0, -1, -2, -3, -4, -5
+XF_BC_PERIODIC, XF_BC_TRANSMISSIVE, XF_BC_REFLECTIVE, XF_BC_DIRICHLET = 0, 1, 2, 3
+XF_MAX_SPECIES = 16
+
+# every symbol include/xf.h declares (tests check that the library exports all of them)
+ABI_SYMBOLS = (
+    "xf_create", "xf_destroy", "xf_num_vars", "xf_padded_cells", "xf_rhs_workspace_bytes", "xf_workspace_bytes",
+    "xf_fill_ghosts", "xf_primitives", "xf_convective_rhs", "xf_rk3_step", "xf_rk3_step_cfl", "xf_max_wavespeed",
+    "xf_status", "xf_newton_mean_iterations", "xf_launch_count", "xf_convective_rhs_host", "xf_rk3_steps_host",
+    "xf_probe_fp64_peak", "xf_strerror",
+)
+
+
+class XfConfig(C.Structure):
+    _fields_ = [
+        ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("ng", C.c_int),
+        ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double),
+        ("nspecies", C.c_int), ("Ru", C.c_double),
+        ("W", C.POINTER(C.c_double)), ("nasa7", C.POINTER(C.c_double)),
+        ("Tlo", C.c_double), ("Thi", C.c_double),
+        ("bc", C.c_int * 6), ("bc_state", C.POINTER(C.c_double)),
+        ("newton_rtol", C.c_double), ("newton_maxit", C.c_int), ("device", C.c_int),
+    ]
+
+
+class XfError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {strerror(code)} ({code})")
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load libxf.so (built in-tree by ``paper_2403_05910_b200.build``).  Raises if it is not there."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2403_05910_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(str(LIB_PATH))
+        vp, dp, ctx = C.c_void_p, C.c_void_p, C.c_void_p
+        L.xf_create.argtypes = [C.POINTER(ctx), C.POINTER(XfConfig)]
+        L.xf_destroy.argtypes = [ctx]
+        for name in ("xf_num_vars", "xf_padded_cells", "xf_rhs_workspace_bytes", "xf_workspace_bytes"):
+            getattr(L, name).argtypes = [ctx]
+            getattr(L, name).restype = C.c_size_t
+        L.xf_fill_ghosts.argtypes = [ctx, dp, vp]
+        L.xf_primitives.argtypes = [ctx, dp, dp, dp, dp, vp]
+        L.xf_convective_rhs.argtypes = [ctx, dp, dp, dp, vp, vp]
+        L.xf_rk3_step.argtypes = [ctx, dp, dp, C.c_double, vp, vp]
+        L.xf_rk3_step_cfl.argtypes = [ctx, dp, dp, C.c_double, dp, vp, vp]
+        L.xf_max_wavespeed.argtypes = [ctx, dp, dp, dp, vp]
+        L.xf_status.argtypes = [ctx, vp]
+        L.xf_newton_mean_iterations.argtypes = [ctx, vp, C.POINTER(C.c_double)]
+        L.xf_launch_count.argtypes = [ctx]
+        L.xf_launch_count.restype = C.c_long
+        L.xf_convective_rhs_host.argtypes = [ctx, dp, dp, dp]
+        L.xf_rk3_steps_host.argtypes = [ctx, dp, dp, C.c_double, C.c_int, C.POINTER(C.c_double)]
+        L.xf_probe_fp64_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.xf_strerror.argtypes = [C.c_int]
+        L.xf_strerror.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def strerror(code: int) -> str:
+    return lib().xf_strerror(int(code)).decode()
+
+
+def _check(code: int, where: str) -> None:
+    if code != XF_OK:
+        raise XfError(code, where)
+
+
+def _ptr(t) -> int:
+    """Device (torch.Tensor) or host (numpy.ndarray) fp64 contiguous buffer -> raw address; None -> NULL."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        assert t.dtype == np.float64 and t.flags["C_CONTIGUOUS"]
+        return t.ctypes.data
+    import torch
+
+    assert isinstance(t, torch.Tensor) and t.is_contiguous()
+    assert t.dtype in (torch.float64, torch.uint8)
+    return t.data_ptr()
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+
+        return torch.cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+def xf_probe_fp64_peak(device: int = 0, iters: int = 4096):
+    """-> (TFLOP/s, ms) of the register-resident fp64 FMA probe kernel."""
+    tf, ms = C.c_double(), C.c_double()
+    _check(lib().xf_probe_fp64_peak(int(device), int(iters), C.byref(tf), C.byref(ms)), "xf_probe_fp64_peak")
+    return tf.value, ms.value
+
+
+class Context:
+    """Owns one ``xf_ctx``.  Methods are the C-ABI calls with the context bound; tensors are caller-owned."""
+
+    def __init__(self, nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, W: Sequence[float], nasa7, Ru: float,
+                 Tlo: float, Thi: float, bc=(0,) * 6, bc_state=None, newton_rtol: float = 0.0, newton_maxit: int = 0,
+                 device: int = 0):
+        W = np.ascontiguousarray(W, dtype=np.float64)
+        nasa7 = np.ascontiguousarray(nasa7, dtype=np.float64)
+        n = int(W.shape[0])
+        assert nasa7.shape == (n, 7)
+        cfg = XfConfig()
+        cfg.nx, cfg.ny, cfg.nz, cfg.ng = int(nx), int(ny), int(nz), 3
+        cfg.dx, cfg.dy, cfg.dz = float(dx), float(dy), float(dz)
+        cfg.nspecies, cfg.Ru = n, float(Ru)
+        cfg.W = W.ctypes.data_as(C.POINTER(C.c_double))
+        cfg.nasa7 = nasa7.ctypes.data_as(C.POINTER(C.c_double))
+        cfg.Tlo, cfg.Thi = float(Tlo), float(Thi)
+        for q in range(6):
+            cfg.bc[q] = int(bc[q])
+        bs = None
+        if bc_state is not None:
+            bs = np.ascontiguousarray(bc_state, dtype=np.float64)
+            assert bs.shape == (6, n + 4)
+            cfg.bc_state = bs.ctypes.data_as(C.POINTER(C.c_double))
+        cfg.newton_rtol, cfg.newton_maxit, cfg.device = float(newton_rtol), int(newton_maxit), int(device)
+        self._h = C.c_void_p()
+        _check(lib().xf_create(C.byref(self._h), C.byref(cfg)), "xf_create")
+        self.device = int(device)
+        self.N, self.Nv = n, n + 4
+        self.cells = int(lib().xf_padded_cells(self._h))
+        self.shape = (nz + 6 if nz > 1 else 1, ny + 6 if ny > 1 else 1, nx + 6 if nx > 1 else 1)
+        self.interior_cells = int(nx) * int(ny) * int(nz)
+        self.rhs_workspace_bytes = int(lib().xf_rhs_workspace_bytes(self._h))
+        self.workspace_bytes = int(lib().xf_workspace_bytes(self._h))
+
+    @classmethod
+    def from_workload(cls, wl, **kw) -> "Context":
+        t = wl.table
+        return cls(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, t.W, t.nasa7, t.Ru, t.Tlo, t.Thi, wl.bc, wl.bc_state, **kw)
+
+    def close(self) -> None:
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().xf_destroy(self._h)
+            self._h = C.c_void_p()
+
+    __del__ = close
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # ---- device-memory helpers (plumbing) ----
+    def empty_fields(self, nfields: Optional[int] = None):
+        import torch
+
+        shape = self.shape if nfields is None else (nfields,) + self.shape
+        return torch.empty(shape, dtype=torch.float64, device=f"cuda:{self.device}")
+
+    def workspace(self, rhs_only: bool = False):
+        import torch
+
+        nbytes = self.rhs_workspace_bytes if rhs_only else self.workspace_bytes
+        return torch.empty(nbytes // 8, dtype=torch.float64, device=f"cuda:{self.device}")
+
+    # ---- the C-ABI calls ----
+    def xf_fill_ghosts(self, U, stream=None) -> None:
+        _check(lib().xf_fill_ghosts(self._h, _ptr(U), _stream(stream)), "xf_fill_ghosts")
+
+    def xf_primitives(self, U, T, p=None, c=None, stream=None) -> None:
+        _check(lib().xf_primitives(self._h, _ptr(U), _ptr(T), _ptr(p), _ptr(c), _stream(stream)), "xf_primitives")
+
+    def xf_convective_rhs(self, U, T, rhs, work, stream=None) -> None:
+        assert work.numel() * work.element_size() >= self.rhs_workspace_bytes
+        _check(lib().xf_convective_rhs(self._h, _ptr(U), _ptr(T), _ptr(rhs), _ptr(work), _stream(stream)),
+               "xf_convective_rhs")
+
+    def xf_rk3_step(self, U, T, dt: float, work, stream=None) -> None:
+        assert work.numel() * work.element_size() >= self.workspace_bytes
+        _check(lib().xf_rk3_step(self._h, _ptr(U), _ptr(T), float(dt), _ptr(work), _stream(stream)), "xf_rk3_step")
+
+    def xf_rk3_step_cfl(self, U, T, cfl: float, S_dev, work, stream=None) -> None:
+        assert work.numel() * work.element_size() >= self.workspace_bytes
+        _check(lib().xf_rk3_step_cfl(self._h, _ptr(U), _ptr(T), float(cfl), _ptr(S_dev), _ptr(work), _stream(stream)),
+               "xf_rk3_step_cfl")
+
+    def xf_max_wavespeed(self, U, T, S_dev, stream=None) -> None:
+        _check(lib().xf_max_wavespeed(self._h, _ptr(U), _ptr(T), _ptr(S_dev), _stream(stream)), "xf_max_wavespeed")
+
+    def xf_status(self, stream=None) -> int:
+        return int(lib().xf_status(self._h, _stream(stream)))
+
+    def xf_newton_mean_iterations(self, stream=None) -> float:
+        m = C.c_double()
+        _check(lib().xf_newton_mean_iterations(self._h, _stream(stream), C.byref(m)), "xf_newton_mean_iterations")
+        return m.value
+
+    def xf_launch_count(self) -> int:
+        return int(lib().xf_launch_count(self._h))
+
+    def xf_convective_rhs_host(self, U_host: np.ndarray, T_host: np.ndarray, rhs_host: np.ndarray) -> None:
+        _check(lib().xf_convective_rhs_host(self._h, _ptr(U_host), _ptr(T_host), _ptr(rhs_host)),
+               "xf_convective_rhs_host")
+
+    def xf_rk3_steps_host(self, U_host: np.ndarray, T_host: np.ndarray, cfl: float, nsteps: int) -> float:
+        t = C.c_double()
+        _check(lib().xf_rk3_steps_host(self._h, _ptr(U_host), _ptr(T_host), float(cfl), int(nsteps), C.byref(t)),
+               "xf_rk3_steps_host")
+        return t.value

@@ -1,0 +1,337 @@
+"""-m gpu parity tests: the CUDA path (through the C-ABI binding) against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star, reading R14): relative 1e-12 per RHS evaluation and
+1e-9 after 200 steps, per variable, normalised by that variable's max magnitude over the field (the three momentum
+components share one scale so that an identically zero component does not divide by zero).  Integer / copy work
+(ghost fill) is bit-exact.
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from paper_2403_05910_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+RHS_TOL = 1e-12
+STEPS_TOL = 1e-9
+
+
+def _gpu(w, **kw):
+    from gpu_helpers import GpuRun
+
+    return GpuRun(w, **kw)
+
+
+def field_err(a: np.ndarray, b: np.ndarray) -> np.ndarray:
+    """per-variable max|a-b| / scale_v with b the oracle; momentum components share their scale (R14)."""
+    nv = a.shape[0]
+    a2, b2 = a.reshape(nv, -1), b.reshape(nv, -1)
+    num = np.abs(a2 - b2).max(axis=1)
+    den = np.abs(b2).max(axis=1)
+    den[1:4] = den[1:4].max()
+    return num / np.maximum(den, 1e-300)
+
+
+def state_err(w, a: np.ndarray, b: np.ndarray, cmax: float) -> np.ndarray:
+    nv = a.shape[0]
+    ai, bi = w.interior(a).reshape(nv, -1), w.interior(b).reshape(nv, -1)
+    num = np.abs(ai - bi).max(axis=1)
+    den = np.abs(bi).max(axis=1)
+    den[1:4] = np.abs(bi[0]).max() * cmax
+    return num / np.maximum(den, 1e-300)
+
+
+# ------------------------------------------------------------------------------------------------------------
+# ghost fill: bit-exact
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape", [(17, 1, 1), (9, 12, 1), (8, 5, 7), (5, 1, 6), (1, 7, 9)])
+@pytest.mark.parametrize("bc", [(0, 0, 0, 0, 0, 0), (1, 1, 2, 2, 1, 2), (3, 1, 2, 1, 3, 3), (2, 3, 1, 1, 2, 2)])
+def test_ghost_fill_bit_exact(oracle_mod, shape, bc):
+    import torch
+
+    w = wl.random_smooth_box(*shape, nspecies=3, seed=11, bc=bc)
+    rng = np.random.default_rng(5)
+    w.bc_state = rng.uniform(0.5, 2.0, (6, w.nvars))
+    U0 = rng.uniform(-1.0, 1.0, w.U.shape)       # ghosts hold garbage that must be overwritten
+    orc = oracle_mod.Oracle.from_workload(w)
+    Uo = U0.copy()
+    orc.fill_ghosts(Uo)
+    g = _gpu(w)
+    g.U.copy_(torch.from_numpy(U0))
+    g.ctx.xf_fill_ghosts(g.U)
+    assert np.array_equal(g.host_U(), Uo)
+    g.close()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# primitives and the max wave speed
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 7, 10])
+def test_primitives_parity(oracle_mod, n):
+    import torch
+
+    w = wl.random_smooth_box(19, 11, 6, nspecies=n, seed=100 + n)
+    orc = oracle_mod.Oracle.from_workload(w)
+    Uo, To = w.U.copy(), w.T_guess.copy()
+    orc.fill_ghosts(Uo)
+    po, co = np.zeros_like(To), np.zeros_like(To)
+    st, iters = orc.primitives(Uo, To, po, co)
+    assert st == 0
+    g = _gpu(w)
+    g.ctx.xf_fill_ghosts(g.U)
+    p, c = torch.zeros_like(g.T), torch.zeros_like(g.T)
+    g.ctx.xf_primitives(g.U, g.T, p, c)
+    assert g.ctx.xf_status() == 0
+    assert abs(g.ctx.xf_newton_mean_iterations() - iters) < 0.05
+    for a, b in ((g.host_T(), To), (p.cpu().numpy(), po), (c.cpu().numpy(), co)):
+        assert np.max(np.abs(a - b) / np.abs(b)) < 1e-13
+    g.close()
+
+
+def test_primitives_outside_fit_range_and_constant_cp(oracle_mod):
+    """continuation branch (reading R3): temperatures below Tlo and above Thi, wild guesses."""
+    w = wl.config5_random_states(24, 16, 12)
+    orc = oracle_mod.Oracle.from_workload(w)
+    Uo, To = w.U.copy(), w.T_guess.copy()
+    orc.fill_ghosts(Uo)
+    st, _ = orc.primitives(Uo, To)
+    assert st == 0
+    frac_out = np.mean((To < 200.0) | (To > 3000.0))
+    assert frac_out > 0.01, "workload must exercise the continuation branch"
+    g = _gpu(w)
+    g.ctx.xf_fill_ghosts(g.U)
+    g.ctx.xf_primitives(g.U, g.T)
+    assert g.ctx.xf_status() == 0
+    assert np.max(np.abs(g.host_T() - To) / To) < 1e-13
+    g.close()
+
+
+@pytest.mark.parametrize("shape,n", [((64, 1, 1), 2), ((33, 20, 1), 3), ((21, 10, 9), 10)])
+def test_max_wavespeed_parity(oracle_mod, shape, n):
+    w = wl.random_smooth_box(*shape, nspecies=n, seed=7)
+    orc = oracle_mod.Oracle.from_workload(w)
+    So = orc.max_wavespeed(w.U.copy(), w.T_guess.copy())
+    g = _gpu(w)
+    S = g.max_wavespeed()
+    assert abs(S - So) <= 1e-13 * So
+    g.close()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# one convective RHS: every species-count instantiation, 1-D / 2-D / 3-D, ragged sizes spanning several tiles
+# ------------------------------------------------------------------------------------------------------------
+RHS_CASES = [
+    ((400, 1, 1), 1, (0,) * 6), ((1030, 1, 1), 2, (1, 1, 0, 0, 0, 0)), ((7, 1, 1), 3, (2, 2, 0, 0, 0, 0)),
+    ((1, 70, 1), 2, (0,) * 6), ((1, 1, 45), 4, (0, 0, 0, 0, 2, 1)),
+    ((150, 37, 1), 3, (3, 1, 2, 2, 0, 0)), ((37, 1, 29), 2, (0, 0, 0, 0, 1, 1)), ((1, 40, 33), 5, (0,) * 6),
+    ((45, 19, 23), 4, (3, 1, 0, 0, 0, 0)), ((70, 9, 8), 10, (3, 1, 2, 2, 2, 2)), ((33, 35, 37), 1, (0,) * 6),
+    ((20, 18, 40), 7, (1, 2, 2, 1, 0, 0)), ((131, 6, 5), 16, (0,) * 6),
+]
+
+
+@pytest.mark.parametrize("shape,n,bc", RHS_CASES)
+def test_rhs_parity_small(oracle_mod, shape, n, bc):
+    if shape[0] > 1000:
+        # a long pencil (several x-sweep segments).  A smooth low-mode field on 1000+ cells is over-resolved: the
+        # RHS is a difference quotient whose round-off, eps*|F|/dx, is then ~1e-12 of max|rhs| on BOTH sides
+        # (DESIGN.md "Tolerances"), so the long-pencil case uses the shock-tube data of config 1 instead.
+        w = wl.config1_shock_tube(nx=shape[0])
+    else:
+        w = wl.random_smooth_box(*shape, nspecies=n, seed=1000 + n + shape[0], bc=bc)
+    orc = oracle_mod.Oracle.from_workload(w)
+    Uo, To = w.U.copy(), w.T_guess.copy()
+    ro = orc.rhs(Uo, To)
+    assert orc.last_status == 0
+    g = _gpu(w)
+    r = g.rhs()
+    err = field_err(w.interior(r), w.interior(ro))
+    assert err.max() < RHS_TOL, err
+    assert np.array_equal(g.host_U(), Uo)                     # ghosts filled identically, interior untouched
+    assert np.max(np.abs(g.host_T() - To) / To) < 1e-13
+    g.close()
+
+
+def test_rhs_parity_shocked_states(oracle_mod):
+    """discontinuous data: WENO weights far from the linear ones, LLF maxima switching cells."""
+    w = wl.config3_shock_bubble_3d(24)
+    orc = oracle_mod.Oracle.from_workload(w)
+    ro = orc.rhs(w.U.copy(), w.T_guess.copy())
+    g = _gpu(w)
+    err = field_err(w.interior(g.rhs()), w.interior(ro))
+    assert err.max() < RHS_TOL, err
+    g.close()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# config 1 (BASELINE.json configs[0]): the full 200-step run, every step's dt from the device reduction
+# ------------------------------------------------------------------------------------------------------------
+def test_config1_200_steps(oracle_mod):
+    w = wl.config1_shock_tube()
+    orc = oracle_mod.Oracle.from_workload(w)
+    Uo, To = w.U.copy(), w.T_guess.copy()
+    g = _gpu(w)
+    worst = 0.0
+    for step in range(w.steps):
+        So = orc.max_wavespeed(Uo, To)
+        S = g.max_wavespeed()
+        assert abs(S - So) <= 1e-11 * So
+        if step in (0, 50, 199):                              # per-RHS parity on the evolving states
+            ro = orc.rhs(Uo.copy(), To.copy())
+            keepU, keepT = g.U.clone(), g.T.clone()
+            g.U.copy_(g.torch.from_numpy(Uo))
+            g.T.copy_(g.torch.from_numpy(To))
+            err = field_err(w.interior(g.rhs()), w.interior(ro))
+            assert err.max() < RHS_TOL, (step, err)
+            g.U.copy_(keepU)
+            g.T.copy_(keepT)
+        dt = w.cfl / So                                       # the same dt on both sides
+        assert orc.rk3_step(Uo, To, dt) == 0
+        g.step(dt)
+        cmax = So * w.dx
+        worst = max(worst, state_err(w, g.host_U(), Uo, cmax).max())
+    assert g.ctx.xf_status() == 0
+    assert worst < STEPS_TOL, worst
+    g.close()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# configs 2-4 at reduced size (same generator, same set-up), multi-step; config 5 sub-block, one RK3 step
+# ------------------------------------------------------------------------------------------------------------
+def _multi_step(oracle_mod, w, steps):
+    orc = oracle_mod.Oracle.from_workload(w)
+    Uo, To = w.U.copy(), w.T_guess.copy()
+    g = _gpu(w)
+    worst = 0.0
+    for _ in range(steps):
+        So = orc.max_wavespeed(Uo, To)
+        S = g.max_wavespeed()
+        assert abs(S - So) <= 1e-10 * So
+        dt = w.cfl / So
+        assert orc.rk3_step(Uo, To, dt) == 0
+        g.step(dt)
+        cmax = So * min(w.dx, w.dy, w.dz)
+        worst = max(worst, state_err(w, g.host_U(), Uo, cmax).max())
+    assert g.ctx.xf_status() == 0
+    g.close()
+    return worst
+
+
+def test_config2_reduced_200_steps(oracle_mod):
+    assert _multi_step(oracle_mod, wl.config2_shock_bubble_2d(256, 128), 200) < STEPS_TOL
+
+
+def test_config3_reduced_steps(oracle_mod):
+    assert _multi_step(oracle_mod, wl.config3_shock_bubble_3d(40), 40) < STEPS_TOL
+
+
+def test_config4_reduced_steps(oracle_mod):
+    assert _multi_step(oracle_mod, wl.config4_shock_bubble_3d_10sp(64, 32, 32), 20) < STEPS_TOL
+
+
+def test_config5_subblock_one_rk3_step(oracle_mod):
+    """BASELINE.json configs[4] parity recipe at reduced box size: the GPU advances the periodic box, the oracle a
+    (16+18)^3 cut around a seeded origin; the inner 16^3 cells are compared."""
+    w = wl.config5_random_states(48, 40, 36)
+    g = _gpu(w)
+    S = g.max_wavespeed()
+    dt = w.cfl / S
+    g.step(dt)
+    assert g.ctx.xf_status() == 0
+    Ug = w.interior(g.host_U())
+    rng = np.random.default_rng(wl.SEED_BASE + 55)
+    origin = (int(rng.integers(0, w.nx)), int(rng.integers(0, w.ny)), int(rng.integers(0, w.nz)))
+    size, margin = 16, 9
+    sub = wl.periodic_subblock(w, origin, size, margin)
+    orc = oracle_mod.Oracle.from_workload(sub)
+    Uo, To = sub.U.copy(), sub.T_guess.copy()
+    orc.rk3_step(Uo, To, dt)
+    inner_o = sub.interior(Uo)[:, margin:margin + size, margin:margin + size, margin:margin + size]
+    ix = (np.arange(size) + origin[0]) % w.nx
+    iy = (np.arange(size) + origin[1]) % w.ny
+    iz = (np.arange(size) + origin[2]) % w.nz
+    inner_g = Ug[:, iz][:, :, iy][:, :, :, ix]
+    nv = w.nvars
+    num = np.abs(inner_g - inner_o).reshape(nv, -1).max(axis=1)
+    den = np.abs(inner_o).reshape(nv, -1).max(axis=1)
+    den[1:4] = np.abs(inner_o[0]).max() * S * w.dx
+    assert (num / den).max() < STEPS_TOL
+    g.close()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# API behaviour
+# ------------------------------------------------------------------------------------------------------------
+def test_rk3_step_cfl_matches_host_dt():
+    w = wl.random_smooth_box(40, 12, 10, nspecies=3, seed=3)
+    a, b = _gpu(w), _gpu(w)
+    S = a.max_wavespeed()
+    a.step(0.4 / S)
+    b.max_wavespeed()
+    b.ctx.xf_rk3_step_cfl(b.U, b.T, 0.4, b.S, b.work)
+    assert np.array_equal(a.host_U(), b.host_U())
+    a.close()
+    b.close()
+
+
+def test_host_entry_points_match_device_calls():
+    w = wl.random_smooth_box(30, 14, 9, nspecies=4, seed=8)
+    g = _gpu(w)
+    r_dev = g.rhs()
+    Uh, Th = w.U.copy(), w.T_guess.copy()
+    rh = np.zeros_like(Uh)
+    g.ctx.xf_convective_rhs_host(Uh, Th, rh)
+    assert np.array_equal(w.interior(rh), w.interior(r_dev))
+    g.reset()
+    t = 0.0
+    for _ in range(3):
+        S = g.max_wavespeed()
+        g.ctx.xf_rk3_step_cfl(g.U, g.T, 0.5, g.S, g.work)
+        t += 0.5 / S
+    Uh, Th = w.U.copy(), w.T_guess.copy()
+    t_host = g.ctx.xf_rk3_steps_host(Uh, Th, 0.5, 3)
+    assert np.array_equal(w.interior(Uh), w.interior(g.host_U()))
+    assert abs(t_host - t) <= 1e-14 * t
+    g.close()
+
+
+def test_status_flags_nonphysical_and_noconv():
+    from paper_2403_05910_b200 import xf
+
+    w = wl.random_smooth_box(16, 8, 1, nspecies=2, seed=4)
+    g = _gpu(w)
+    g.U[0, 0, 5, 7] = -1.0                                    # negative density in one interior cell
+    g.ctx.xf_fill_ghosts(g.U)
+    g.ctx.xf_primitives(g.U, g.T)
+    assert g.ctx.xf_status() == xf.XF_ENONPHYSICAL
+    assert g.ctx.xf_status() == xf.XF_OK                      # the flag is cleared by reading it
+    g.close()
+    g = _gpu(w, newton_maxit=1, newton_rtol=1e-15)
+    g.ctx.xf_primitives(g.U, g.T)
+    assert g.ctx.xf_status() == xf.XF_ENOCONV
+    g.close()
+
+
+def test_conservation_and_two_contexts_on_two_streams():
+    import torch
+
+    w1 = wl.random_smooth_box(32, 16, 12, nspecies=3, seed=21)
+    w2 = wl.random_smooth_box(24, 20, 1, nspecies=10, seed=22)
+    g1, g2 = _gpu(w1), _gpu(w2)
+    ref1, ref2 = _gpu(w1), _gpu(w2)
+    for g in (ref1, ref2):
+        g.step(1e-4)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    g1.ctx.xf_rk3_step(g1.U, g1.T, 1e-4, g1.work, stream=s1)
+    g2.ctx.xf_rk3_step(g2.U, g2.T, 1e-4, g2.work, stream=s2)
+    torch.cuda.synchronize()
+    assert np.array_equal(g1.host_U(), ref1.host_U())
+    assert np.array_equal(g2.host_U(), ref2.host_U())
+    tot0 = w1.interior(w1.U).reshape(w1.nvars, -1).sum(axis=1)
+    tot1 = w1.interior(g1.host_U()).reshape(w1.nvars, -1).sum(axis=1)
+    scale = np.abs(w1.interior(w1.U)).reshape(w1.nvars, -1).sum(axis=1)
+    assert np.max(np.abs(tot1 - tot0) / scale) < 1e-13        # periodic box: round-off conservation
+    for g in (g1, g2, ref1, ref2):
+        g.close()
