@@ -1,0 +1,385 @@
+#!/usr/bin/env python
+"""bench.py -- the headline measurement: fp64 cell-updates/s per RK stage of the convective RHS on one B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl b200|reference] [--workload config4]
+
+A "step" is one pass of the whole hot path over the workload: xf_max_wavespeed (the CFL reduction) followed by
+xf_rk3_step_cfl -- three times (ghost fill, primitives, x/y/z sweeps with the flux divergence and the fused
+SSP-RK3 stage combination).  One step is therefore 3 convective-RHS evaluations of every interior cell, and
+
+    value = interior cells x 3 x K x N / time          [cell-updates/s per RK stage, whole job]
+
+Default workload: BASELINE.json configs[3] (3-D 10-species shock-bubble, 512x256x256), the configuration the
+north-star target is quoted on.  The state advances from step to step (a real simulation), inputs are synthetic
+and seeded, each U copy is 4 GB >> the 126 MB L2, so no L2 flush is needed.
+
+N > 1 (torchrun): the path has no exchange step on one GPU (replicas only), so every rank
+runs an independent replica of the same problem, no data-path collective; timing is max over ranks; "weak".
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded sample of the same
+workload; it is a deliberately plain program -- parity and the roofline fraction are the headline, not that ratio.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "fp64 cell-updates/s per RK stage (convective RHS)"
+UNIT = "cell-updates/s"
+
+WORKLOADS = {
+    # name: (generator, full grid, grid of the bounded oracle sample for cpu_baseline, grid of a --impl reference step)
+    "config4": ("config4_shock_bubble_3d_10sp", (512, 256, 256), (192, 96, 96), (128, 64, 64)),
+    "config3": ("config3_shock_bubble_3d", (256, 256, 256), (128, 128, 128), (96, 96, 96)),
+    "config2": ("config2_shock_bubble_2d", (2048, 1024, 1), (1024, 512, 1), (1024, 512, 1)),
+}
+
+
+def make_workload(name: str, grid):
+    from paper_2403_05910_b200 import workloads as wl
+
+    gen = getattr(wl, WORKLOADS[name][0])
+    if name == "config3":
+        return gen(grid[0])
+    if name == "config2":
+        return gen(grid[0], grid[1])
+    return gen(*grid)
+
+
+def flops_per_face(N: int) -> int:
+    """Algorithmic fp64 flops of one face flux + its share of the divergence."""
+    return 222 * N + 954
+
+
+def flops_per_cell_rhs(N: int, D: int, newton_its: float) -> float:
+    return D * flops_per_face(N) + 24 * N * newton_its + 3 * N + 40
+
+
+def bytes_per_cell_rhs(N: int) -> int:
+    """Compulsory HBM bytes of one RHS evaluation: read U, write rhs/U', read the T guess, write T."""
+    return (2 * (N + 4) + 2) * 8
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# clocks: nvidia-smi sampled DURING the timed region (B200_PROFILING.md "clocks line")
+# ---------------------------------------------------------------------------------------------------------------
+_CLK_FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+               "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+               "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+
+class ClockSampler:
+    def __init__(self, gpu_index: int):
+        self.path = Path(tempfile.gettempdir()) / f"xf_clocks_{os.getpid()}.csv"
+        self.gpu = gpu_index
+        self.proc = None
+
+    def start(self):
+        try:
+            self.fh = open(self.path, "w")
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={_CLK_FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"], stdout=self.fh,
+                                         stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.fh.close()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.path.read_text().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                smax.append(float(f[2]))
+                power.append(float(f[3]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        try:
+            self.path.unlink()
+        except OSError:
+            pass
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(smax), power_w_max=max(power), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the CPU oracle legs (cpu_baseline of the main arm; the whole --impl reference arm)
+# ---------------------------------------------------------------------------------------------------------------
+def oracle_threads() -> int:
+    env = os.environ.get("OMP_NUM_THREADS")
+    return int(env) if env and env.isdigit() else (os.cpu_count() or 1)
+
+
+def oracle_step_seconds(w, steps: int, warmup: int = 0):
+    """Times `steps` hot-path steps (max wave speed + one RK3 step = 3 RHS) of the oracle on workload w."""
+    import oracle
+
+    O = oracle.Oracle.from_workload(w)
+    U, T = w.U.copy(), w.T_guess.copy()
+    for _ in range(warmup):
+        S = O.max_wavespeed(U, T)
+        O.rk3_step(U, T, w.cfl / S)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        S = O.max_wavespeed(U, T)
+        O.rk3_step(U, T, w.cfl / S)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(name: str) -> dict:
+    grid = WORKLOADS[name][2]
+    w = make_workload(name, grid)
+    sec = oracle_step_seconds(w, 1)
+    return {"value": w.interior_cells * 3 / sec, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle",
+            "sample": f"1 step (max wave speed + RK3 = 3 RHS) of {name} generated at {grid[0]}x{grid[1]}x{grid[2]} "
+                      f"(same set-up, reduced grid), {sec:.1f} s, oracle/xf_oracle.c with OpenMP"}
+
+
+def run_reference(args, rank: int, world: int) -> None:
+    if rank != 0:
+        return
+    name = args.workload
+    grid = WORKLOADS[name][3]
+    w = make_workload(name, grid)
+    sec = oracle_step_seconds(w, args.steps, args.warmup)
+    value = w.interior_cells * 3 * args.steps / sec
+    sample = (f"each step = max wave speed + RK3 (3 RHS) of {name} generated at {grid[0]}x{grid[1]}x{grid[2]} "
+              f"(bounded sample of the {'x'.join(map(str, WORKLOADS[name][1]))} workload)")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sec / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": name, "grid": list(WORKLOADS[name][1]), "nspecies": w.nspecies, "sample_grid": list(grid)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the B200 arm
+# ---------------------------------------------------------------------------------------------------------------
+def measured_peaks() -> dict:
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return {"hbm_gbs": float(d["hbm_gbs"]), "hbm_source": "MEASURED_PEAKS.json (of measured)"}
+    return {"hbm_gbs": 6650.0, "hbm_source": "B200_PROFILING.md fallback (of fallback)"}
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
+# capture (profiles/); None until a capture of that (workload, kernel) exists.
+NCU_TRAFFIC_BYTES = {}
+
+
+def run_b200(args, rank: int, local_rank: int, world: int) -> None:
+    import numpy as np
+    import torch
+
+    from paper_2403_05910_b200 import xf
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU path")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    name = args.workload
+    grid = tuple(args.grid) if args.grid else WORKLOADS[name][1]
+    w = make_workload(name, grid)
+    N, Nv, cells = w.nspecies, w.nvars, w.interior_cells
+    D = sum(1 for n in (w.nx, w.ny, w.nz) if n > 1)
+    ctx = xf.Context.from_workload(w, device=local_rank)
+    U = torch.from_numpy(w.U).to(dev)
+    T = torch.from_numpy(w.T_guess).to(dev)
+    work = ctx.workspace()
+    S = torch.zeros(1, dtype=torch.float64, device=dev)
+    cfl = float(w.cfl)
+
+    # fp64-pipe peak measured on this GPU, now (the denominator of the "alu" roofline)
+    peak_tf, probe_ms = xf.xf_probe_fp64_peak(local_rank, 60000)
+
+    def step():
+        ctx.xf_max_wavespeed(U, T, S)
+        ctx.xf_rk3_step_cfl(U, T, cfl, S, work)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    if ctx.xf_status() != 0:
+        raise RuntimeError("non-physical state or Newton failure during warm-up")
+
+    ctx.xf_timing_enable(32 * args.steps + 32)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    launches0 = ctx.xf_launch_count()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms_total = max_over_ranks(float(e0.elapsed_time(e1)))
+    launches = ctx.xf_launch_count() - launches0
+    ktimes = ctx.xf_timing_read()
+    ctx.xf_timing_enable(0)
+    status = ctx.xf_status()
+    if status != 0:
+        raise RuntimeError(f"xf_status = {status} after the timed region")
+    # mean Newton iteration count of the state the timed region ended on (debug counter; outside the timed region)
+    ctx.xf_fill_ghosts(U)
+    Tn = T.clone()
+    ctx.xf_primitives(U, Tn)
+    newton_its = ctx.xf_newton_mean_iterations()
+    del Tn
+
+    ms_per_step = ms_total / args.steps
+    value = cells * 3 * world / (ms_per_step * 1e-3)
+
+    # ---- roofline of the dominant kernel (per launch, CUDA events on the launching stream inside the timed region)
+    peaks = measured_peaks()
+    sweeps = {k: v for k, v in ktimes.items() if k.startswith("sweep") and v[1] > 0}
+    dom = max(sweeps, key=lambda k: sweeps[k][0])
+    dom_ms = sweeps[dom][0] / sweeps[dom][1]
+    alg_flops = flops_per_face(N) * cells                      # one sweep launch = every face of one direction
+    # bytes one sweep launch must move in THIS design: U (Nv) + p, c, Gamma, chi_s (N + 3) read, the partial residual
+    # read (all but the first sweep) and one write of Nv fields
+    first = dom == "sweep_x"
+    alg_bytes = ((Nv + N + 3) + (0 if first else Nv) + Nv) * 8 * cells
+    achieved_tf = alg_flops / (dom_ms * 1e-3) * 1e-12
+    kernel_sum_ms = sum(v[0] for v in ktimes.values())
+    roofline = {
+        "bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
+        "traffic": NCU_TRAFFIC_BYTES.get((name, dom)),
+        "kernel": dom, "launch_ms": dom_ms, "launches_timed": sweeps[dom][1],
+        "algorithmic_flops_per_launch": alg_flops, "algorithmic_bytes_per_launch": alg_bytes,
+        "hbm_gbs_achieved": alg_bytes / (dom_ms * 1e-3) * 1e-9, "hbm_gbs_peak": peaks["hbm_gbs"],
+        "hbm_frac": alg_bytes / (dom_ms * 1e-3) * 1e-9 / peaks["hbm_gbs"],
+        "peak_source": f"xf_probe_fp64_peak on this GPU in this run ({probe_ms:.1f} ms of register-resident DFMA); "
+                       f"HBM: {peaks['hbm_source']}",
+        "kernel_share_of_step": {k: v[0] / kernel_sum_ms for k, v in ktimes.items() if v[1] > 0},
+        "kernel_ms_per_launch": {k: v[0] / v[1] for k, v in ktimes.items() if v[1] > 0},
+    }
+    # whole step against the north-star roofline: the slower of bytes / HBM BW and fp64 flops / fp64 peak
+    step_flops = flops_per_cell_rhs(N, D, newton_its) * cells * 3
+    step_bytes = bytes_per_cell_rhs(N) * cells * 3
+    t_alu, t_hbm = step_flops / (peak_tf * 1e12), step_bytes / (peaks["hbm_gbs"] * 1e9)
+    step_roofline = {"t_roof_ms": max(t_alu, t_hbm) * 1e3, "t_alu_ms": t_alu * 1e3, "t_hbm_ms": t_hbm * 1e3,
+                     "frac": max(t_alu, t_hbm) * 1e3 / ms_per_step, "newton_mean_iterations": newton_its,
+                     "flops_per_cell_rhs": flops_per_cell_rhs(N, D, newton_its),
+                     "bytes_per_cell_rhs": bytes_per_cell_rhs(N)}
+
+    # ---- end to end through the host-buffer C-ABI call: pinned host U, T -> device -> one step -> host, every step
+    del U, T, work
+    torch.cuda.empty_cache()
+    Uh = torch.empty(w.U.shape, dtype=torch.float64, pin_memory=True)
+    Th = torch.empty(w.T_guess.shape, dtype=torch.float64, pin_memory=True)
+    Uh.copy_(torch.from_numpy(w.U))
+    Th.copy_(torch.from_numpy(w.T_guess))
+    Uh_np, Th_np = Uh.numpy(), Th.numpy()
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    ctx.xf_rk3_steps_host(Uh_np, Th_np, cfl, 1)                # warm-up: allocates the device mirrors
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        ctx.xf_rk3_steps_host(Uh_np, Th_np, cfl, 1)
+    torch.cuda.synchronize()
+    e2e_s = max_over_ranks(time.perf_counter() - t0)
+    barrier()
+    io_bytes = (Nv + 1) * ctx.cells * 8
+    e2e = {"value": cells * 3 * world * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": io_bytes,
+           "d2h_bytes_per_step": io_bytes, "steps": e2e_steps, "ms_per_step": e2e_s / e2e_steps * 1e3,
+           "api": "xf_rk3_steps_host (pinned host U, T in and out every step)"}
+    if ctx.xf_status() != 0:
+        raise RuntimeError("non-physical state during the end-to-end run")
+    ctx.close()
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": name, "grid": list(grid), "nspecies": N, "nvars": Nv, "interior_cells": cells,
+                       "step": "xf_max_wavespeed + xf_rk3_step_cfl = 3 x (ghost fill, primitives, x/y/z sweeps, "
+                               "RK combine)", "rhs_per_step": 3, "l2": "inputs larger than L2 (one U copy = "
+                               f"{Nv * ctx.cells * 8 / 1e9:.2f} GB), no flush", "parallelism": "replicas"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+            "step_roofline": step_roofline,
+        }
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = cpu_baseline(name)
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=("b200", "reference"))
+    ap.add_argument("--workload", default="config4", choices=sorted(WORKLOADS))
+    ap.add_argument("--grid", type=int, nargs=3, default=None, help="override the grid (debugging only)")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.warmup < 3:
+        args.warmup = 3 if args.impl == "b200" else args.warmup
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_b200(args, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    main()

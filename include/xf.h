@@ -111,6 +111,17 @@ int xf_newton_mean_iterations(xf_ctx *ctx, void *stream, double *mean_out);
 /* Number of kernel launches issued through this context since xf_create (for bench.py's gpu_launches). */
 long xf_launch_count(const xf_ctx *ctx);
 
+/* Per-kernel device timing for the roofline report (bench.py): after xf_timing_enable(ctx, max_records) every
+ * kernel the context launches is bracketed by a CUDA event pair on the caller's stream (up to max_records pairs
+ * between two reads; further launches go untimed).  xf_timing_read synchronises `stream`, adds up the elapsed
+ * milliseconds and the number of records per kernel kind into ms_out[XF_K_COUNT] / count_out[XF_K_COUNT], and
+ * resets the record list.  max_records = 0 switches timing off.  The ghost fill (one launch per active direction)
+ * is timed as one record. */
+enum { XF_K_GHOST = 0, XF_K_PRIM = 1, XF_K_SWEEP_X = 2, XF_K_SWEEP_Y = 3, XF_K_SWEEP_Z = 4, XF_K_WAVESPEED = 5,
+       XF_K_COUNT = 6 };
+int xf_timing_enable(xf_ctx *ctx, int max_records);
+int xf_timing_read(xf_ctx *ctx, void *stream, double *ms_out, long *count_out);
+
 /* HOST-buffer entry points (end-to-end measurement): copy in, run on the device, copy out.  Device scratch is
  * allocated inside the context on first use and freed by xf_destroy.  Synchronous.
  *   xf_convective_rhs_host: U_host [Nv][padded] in, T_host [padded] in/out, rhs_host [Nv][padded] out.

@@ -26,6 +26,10 @@ struct xf_ctx {
   // lazily allocated device mirrors for the *_host entry points
   double *hU, *hT, *hR;
   void *hW;
+  // optional per-kernel timing (xf_timing_enable): event pairs recorded around every launch on the caller's stream
+  int timing_cap, timing_n;
+  cudaEvent_t *ev0, *ev1;
+  int *ev_kind;
 };
 
 namespace {
@@ -55,15 +59,52 @@ inline PrimFields prim_fields(const xf_ctx *c, void *work) {
   return PrimFields{w, w + n, w + 2 * n, w + 3 * n};
 }
 
+// Brackets one kernel (or the ghost-fill group) with an event pair when timing is on; free otherwise.
+struct Timed {
+  xf_ctx *c;
+  cudaStream_t s;
+  int slot;
+  Timed(xf_ctx *ctx, int kind, cudaStream_t st) : c(ctx), s(st), slot(-1) {
+    if (c->timing_cap > 0 && c->timing_n < c->timing_cap) {
+      slot = c->timing_n++;
+      c->ev_kind[slot] = kind;
+      cudaEventRecord(c->ev0[slot], s);
+    }
+  }
+  ~Timed() {
+    if (slot >= 0) cudaEventRecord(c->ev1[slot], s);
+  }
+};
+
+void timing_free(xf_ctx *c) {
+  for (int q = 0; q < c->timing_cap; ++q) {
+    cudaEventDestroy(c->ev0[q]);
+    cudaEventDestroy(c->ev1[q]);
+  }
+  free(c->ev0);
+  free(c->ev1);
+  free(c->ev_kind);
+  c->ev0 = c->ev1 = nullptr;
+  c->ev_kind = nullptr;
+  c->timing_cap = c->timing_n = 0;
+}
+
 int count_active(const XfGrid &G) { return (G.n[0] > 1) + (G.n[1] > 1) + (G.n[2] > 1); }
 
 // ghosts -> primitives -> sweeps.  E_last describes what the LAST active sweep writes (residual or RK combine);
 // earlier sweeps accumulate the partial residual in `acc`.
 int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfEpilogue &E_last, cudaStream_t s) {
-  int rc = xf_launch_ghosts(c->G, c->Nv, c->bc, c->bc_state_dev, U, s, &c->launches);
+  int rc;
+  {
+    Timed t(c, XF_K_GHOST, s);
+    rc = xf_launch_ghosts(c->G, c->Nv, c->bc, c->bc_state_dev, U, s, &c->launches);
+  }
   if (rc != XF_OK) return rc;
   const PrimFields F = prim_fields(c, work);
-  rc = xf_launch_prim(c->G, c->Th, U, T, F.p, F.c, F.Gam, F.chi, c->status_dev, nullptr, s);
+  {
+    Timed t(c, XF_K_PRIM, s);
+    rc = xf_launch_prim(c->G, c->Th, U, T, F.p, F.c, F.Gam, F.chi, c->status_dev, nullptr, s);
+  }
   ++c->launches;
   if (rc != XF_OK) return rc;
   const int nact = count_active(c->G);
@@ -82,6 +123,7 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
       E.acc = acc;
       E.out = acc;
     }
+    Timed t(c, XF_K_SWEEP_X + d, s);
     if (d == 0) rc = xf_launch_sweep_x(c->G, c->N, U, F.p, F.c, F.Gam, F.chi, E, c->status_dev, s);
     else if (d == 1) rc = xf_launch_sweep_y(c->G, c->N, U, F.p, F.c, F.Gam, F.chi, E, c->status_dev, s);
     else rc = xf_launch_sweep_z(c->G, c->N, U, F.p, F.c, F.Gam, F.chi, E, c->status_dev, s);
@@ -224,6 +266,7 @@ int xf_destroy(xf_ctx *c) {
   cudaFree(c->hT);
   cudaFree(c->hR);
   cudaFree(c->hW);
+  timing_free(c);
   delete c;
   return XF_OK;
 }
@@ -282,6 +325,7 @@ int xf_max_wavespeed(xf_ctx *c, const double *U, double *T, double *S_dev, void 
   DeviceGuard guard(c->device);
   if (!guard.ok) return XF_ECUDA;
   ++c->launches;
+  Timed t(c, XF_K_WAVESPEED, static_cast<cudaStream_t>(stream));
   return xf_launch_wavespeed(c->G, c->Th, U, T, S_dev, c->status_dev, static_cast<cudaStream_t>(stream));
 }
 
@@ -312,6 +356,49 @@ int xf_newton_mean_iterations(xf_ctx *c, void *stream, double *mean_out) {
 }
 
 long xf_launch_count(const xf_ctx *c) { return c ? c->launches : 0; }
+
+int xf_timing_enable(xf_ctx *c, int max_records) {
+  if (!c || max_records < 0) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  timing_free(c);
+  if (max_records == 0) return XF_OK;
+  c->ev0 = static_cast<cudaEvent_t *>(calloc(max_records, sizeof(cudaEvent_t)));
+  c->ev1 = static_cast<cudaEvent_t *>(calloc(max_records, sizeof(cudaEvent_t)));
+  c->ev_kind = static_cast<int *>(calloc(max_records, sizeof(int)));
+  if (!c->ev0 || !c->ev1 || !c->ev_kind) {
+    timing_free(c);
+    return XF_ENOMEM;
+  }
+  for (int q = 0; q < max_records; ++q) {
+    if (cudaEventCreate(&c->ev0[q]) != cudaSuccess || cudaEventCreate(&c->ev1[q]) != cudaSuccess) {
+      c->timing_cap = q;
+      timing_free(c);
+      return XF_ECUDA;
+    }
+    c->timing_cap = q + 1;
+  }
+  return XF_OK;
+}
+
+int xf_timing_read(xf_ctx *c, void *stream, double *ms_out, long *count_out) {
+  if (!c || !ms_out || !count_out) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  if (cudaStreamSynchronize(static_cast<cudaStream_t>(stream)) != cudaSuccess) return XF_ECUDA;
+  for (int k = 0; k < XF_K_COUNT; ++k) {
+    ms_out[k] = 0.0;
+    count_out[k] = 0;
+  }
+  for (int q = 0; q < c->timing_n; ++q) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, c->ev0[q], c->ev1[q]) != cudaSuccess) return XF_ECUDA;
+    ms_out[c->ev_kind[q]] += (double)ms;
+    ++count_out[c->ev_kind[q]];
+  }
+  c->timing_n = 0;
+  return XF_OK;
+}
 
 int xf_convective_rhs_host(xf_ctx *c, const double *U_host, double *T_host, double *rhs_host) {
   if (!c || !U_host || !T_host || !rhs_host) return XF_EINVAL;
@@ -347,7 +434,10 @@ int xf_rk3_steps_host(xf_ctx *c, double *U_host, double *T_host, double cfl, int
   double t = 0.0;
   for (int k = 0; k < nsteps; ++k) {
     ++c->launches;
-    rc = xf_launch_wavespeed(c->G, c->Th, c->hU, c->hT, c->S_dev, c->status_dev, s);
+    {
+      Timed tm(c, XF_K_WAVESPEED, s);
+      rc = xf_launch_wavespeed(c->G, c->Th, c->hU, c->hT, c->S_dev, c->status_dev, s);
+    }
     if (rc != XF_OK) return rc;
     rc = rk3(c, c->hU, c->hT, 0.0, cfl, c->S_dev, c->hW, s);
     if (rc != XF_OK) return rc;

@@ -25,8 +25,9 @@ ABI_SYMBOLS = (
     "xf_create", "xf_destroy", "xf_num_vars", "xf_padded_cells", "xf_rhs_workspace_bytes", "xf_workspace_bytes",
     "xf_fill_ghosts", "xf_primitives", "xf_convective_rhs", "xf_rk3_step", "xf_rk3_step_cfl", "xf_max_wavespeed",
     "xf_status", "xf_newton_mean_iterations", "xf_launch_count", "xf_convective_rhs_host", "xf_rk3_steps_host",
-    "xf_probe_fp64_peak", "xf_strerror",
+    "xf_probe_fp64_peak", "xf_strerror", "xf_timing_enable", "xf_timing_read",
 )
+KERNEL_KINDS = ("ghost_fill", "primitives", "sweep_x", "sweep_y", "sweep_z", "max_wavespeed")  # XF_K_* of xf.h
 
 
 class XfConfig(C.Structure):
@@ -77,6 +78,8 @@ def lib() -> C.CDLL:
         L.xf_convective_rhs_host.argtypes = [ctx, dp, dp, dp]
         L.xf_rk3_steps_host.argtypes = [ctx, dp, dp, C.c_double, C.c_int, C.POINTER(C.c_double)]
         L.xf_probe_fp64_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.xf_timing_enable.argtypes = [ctx, C.c_int]
+        L.xf_timing_read.argtypes = [ctx, vp, C.POINTER(C.c_double), C.POINTER(C.c_long)]
         L.xf_strerror.argtypes = [C.c_int]
         L.xf_strerror.restype = C.c_char_p
         _lib = L
@@ -221,6 +224,16 @@ class Context:
 
     def xf_launch_count(self) -> int:
         return int(lib().xf_launch_count(self._h))
+
+    def xf_timing_enable(self, max_records: int) -> None:
+        _check(lib().xf_timing_enable(self._h, int(max_records)), "xf_timing_enable")
+
+    def xf_timing_read(self, stream=None) -> dict:
+        """-> {kernel kind: (total ms, records)} since the last read."""
+        n = len(KERNEL_KINDS)
+        ms, cnt = (C.c_double * n)(), (C.c_long * n)()
+        _check(lib().xf_timing_read(self._h, _stream(stream), ms, cnt), "xf_timing_read")
+        return {k: (ms[q], cnt[q]) for q, k in enumerate(KERNEL_KINDS)}
 
     def xf_convective_rhs_host(self, U_host: np.ndarray, T_host: np.ndarray, rhs_host: np.ndarray) -> None:
         _check(lib().xf_convective_rhs_host(self._h, _ptr(U_host), _ptr(T_host), _ptr(rhs_host)),
