@@ -49,16 +49,6 @@ struct DeviceGuard {
 
 inline size_t field_bytes(const xf_ctx *c) { return sizeof(double) * (size_t)c->G.cells; }
 
-// primitive fields kept between the primitives kernel and the sweeps: p, c, Gamma, chi_1..chi_N
-struct PrimFields {
-  double *p, *c, *Gam, *chi;
-};
-inline PrimFields prim_fields(const xf_ctx *c, void *work) {
-  double *w = static_cast<double *>(work);
-  const size_t n = (size_t)c->G.cells;
-  return PrimFields{w, w + n, w + 2 * n, w + 3 * n};
-}
-
 // Brackets one kernel (or the ghost-fill group) with an event pair when timing is on; free otherwise.
 struct Timed {
   xf_ctx *c;
@@ -100,10 +90,10 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
     rc = xf_launch_ghosts(c->G, c->Nv, c->bc, c->bc_state_dev, U, s, &c->launches);
   }
   if (rc != XF_OK) return rc;
-  const PrimFields F = prim_fields(c, work);
+  double *prim = static_cast<double *>(work);  // p, c, 1/rho, sqrt(rho), Gamma, chi_1..chi_N
   {
     Timed t(c, XF_K_PRIM, s);
-    rc = xf_launch_prim(c->G, c->Th, U, T, F.p, F.c, F.Gam, F.chi, c->status_dev, nullptr, s);
+    rc = xf_launch_prim(c->G, c->Th, U, T, prim, nullptr, nullptr, c->status_dev, nullptr, s);
   }
   ++c->launches;
   if (rc != XF_OK) return rc;
@@ -124,9 +114,9 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
       E.out = acc;
     }
     Timed t(c, XF_K_SWEEP_X + d, s);
-    if (d == 0) rc = xf_launch_sweep_x(c->G, c->N, U, F.p, F.c, F.Gam, F.chi, E, c->status_dev, s);
-    else if (d == 1) rc = xf_launch_sweep_y(c->G, c->N, U, F.p, F.c, F.Gam, F.chi, E, c->status_dev, s);
-    else rc = xf_launch_sweep_z(c->G, c->N, U, F.p, F.c, F.Gam, F.chi, E, c->status_dev, s);
+    if (d == 0) rc = xf_launch_sweep_x(c->G, c->N, U, prim, E, c->status_dev, s);
+    else if (d == 1) rc = xf_launch_sweep_y(c->G, c->N, U, prim, E, c->status_dev, s);
+    else rc = xf_launch_sweep_z(c->G, c->N, U, prim, E, c->status_dev, s);
     ++c->launches;
     if (rc != XF_OK) return rc;
     ++done;
@@ -137,7 +127,7 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
 int rk3(xf_ctx *c, double *U, double *T, double dt, double cfl, const double *S_dev, void *work, cudaStream_t s) {
   const size_t n = (size_t)c->G.cells;
   double *w = static_cast<double *>(work);
-  double *U1 = w + (size_t)(c->N + 3) * n;
+  double *U1 = w + (size_t)(c->N + 5) * n;
   double *U2 = U1 + (size_t)c->Nv * n;
   double *acc = U2 + (size_t)c->Nv * n;
   XfEpilogue E;
@@ -194,6 +184,7 @@ int xf_create(xf_ctx **out, const xf_config *cfg) {
   for (int s = 0; s < N; ++s)
     if (!(cfg->W[s] > 0.0)) return XF_EINVAL;
   if (n[0] == 1 && n[1] == 1 && n[2] == 1) return XF_EINVAL;
+  if (n[1] > 65535 || n[2] > 65535) return XF_EINVAL;  // they index the y dimension of the y/z sweep grids
 
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev) return XF_ECUDA;
@@ -273,9 +264,9 @@ int xf_destroy(xf_ctx *c) {
 
 size_t xf_num_vars(const xf_ctx *c) { return c ? (size_t)c->Nv : 0; }
 size_t xf_padded_cells(const xf_ctx *c) { return c ? (size_t)c->G.cells : 0; }
-size_t xf_rhs_workspace_bytes(const xf_ctx *c) { return c ? field_bytes(c) * (size_t)(c->N + 3) : 0; }
+size_t xf_rhs_workspace_bytes(const xf_ctx *c) { return c ? field_bytes(c) * (size_t)(c->N + 5) : 0; }
 size_t xf_workspace_bytes(const xf_ctx *c) {
-  return c ? field_bytes(c) * (size_t)(c->N + 3 + 3 * c->Nv) : 0;
+  return c ? field_bytes(c) * (size_t)(c->N + 5 + 3 * c->Nv) : 0;
 }
 
 int xf_fill_ghosts(xf_ctx *c, double *U, void *stream) {
@@ -292,7 +283,7 @@ int xf_primitives(xf_ctx *c, const double *U, double *T, double *p, double *cs, 
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (cudaMemsetAsync(c->itersum_dev, 0, sizeof(unsigned long long), s) != cudaSuccess) return XF_ECUDA;
   ++c->launches;
-  return xf_launch_prim(c->G, c->Th, U, T, p, cs, nullptr, nullptr, c->status_dev, c->itersum_dev, s);
+  return xf_launch_prim(c->G, c->Th, U, T, nullptr, p, cs, c->status_dev, c->itersum_dev, s);
 }
 
 int xf_convective_rhs(xf_ctx *c, double *U, double *T, double *rhs, void *work, void *stream) {

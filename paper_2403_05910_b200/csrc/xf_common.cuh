@@ -54,19 +54,20 @@ struct XfEpilogue {
 };
 
 // launch helpers implemented per translation unit
-int xf_launch_prim(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *p, double *c,
-                   double *Gam, double *chi, int *status, unsigned long long *itersum, cudaStream_t s);
+// prim: the N + 5 workspace fields p, c, 1/rho, sqrt(rho), Gamma, chi_1..chi_N ([field][padded cells]); NULL = do
+// not store them (xf_primitives), p_out / c_out: optional separate copies of p and c for the caller.
+int xf_launch_prim(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *prim, double *p_out,
+                   double *c_out, int *status, unsigned long long *itersum, cudaStream_t s);
 int xf_launch_wavespeed(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *S_dev, int *status,
                         cudaStream_t s);
 int xf_launch_ghosts(const XfGrid &G, int Nv, const XfBc &bc, const double *bc_state_dev, double *U, cudaStream_t s,
                      long *launches);
-int xf_launch_sweep_x(const XfGrid &G, int N, const double *U, const double *p, const double *c, const double *Gam,
-                      const double *chi, const XfEpilogue &E, int *status, cudaStream_t s);
-int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *p, const double *c, const double *Gam,
-                      const double *chi, const XfEpilogue &E, int *status, cudaStream_t s);
-int xf_launch_sweep_z(const XfGrid &G, int N, const double *U, const double *p, const double *c, const double *Gam,
-                      const double *chi, const XfEpilogue &E, int *status, cudaStream_t s);
-int xf_sweeps_init();  // opt in to large dynamic shared memory once per process
+int xf_launch_sweep_x(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
+                      cudaStream_t s);
+int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
+                      cudaStream_t s);
+int xf_launch_sweep_z(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
+                      cudaStream_t s);
 
 // fp64 reciprocal: MUFU.RCP64H seed + two Newton steps (4 DFMA); relative error <= ~2 ulp for normal inputs.
 // The path is bound by the fp64 pipe, and an IEEE division costs about three times as many pipe slots.

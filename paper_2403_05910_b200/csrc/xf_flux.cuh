@@ -1,4 +1,5 @@
-// xf_flux.cuh -- directional reconstruct-and-flux sweeps for sm_100a (the hot loop: Eq. 13-15).
+// xf_flux.cuh -- the per-face numerical flux of the directional sweeps for sm_100a (the hot loop: PAPER.md:98-107,
+// Eq. 13-15).
 //
 // One thread computes one face flux Fhat_{i+1/2} = R (F+ + F-) from the six stencil cells staged in shared memory:
 //   * Roe-type average of the two adjacent cells (reading R5), c~^2 from the identity that makes L R = I;
@@ -7,8 +8,8 @@
 //     that is non-zero only for the two acoustic fields and the entropy field -- so the flux is never projected;
 //   * local Lax-Friedrichs splitting (Eq. 14; reading R8), WENO5-JS in a common-denominator form with a single
 //     reciprocal per reconstruction (reading R7), back-projection with the structure of R (Eq. 15);
-//   * the face fluxes of a chunk go to shared memory, the flux difference (Eq. 13) is formed per cell and written
-//     out either as a residual or directly as the Runge-Kutta stage combination (Eq. 16).
+//   * every component of Fhat is handed to `emit` the moment it is final, so the caller can difference it against
+//     the neighbouring face (Eq. 13) and write it out without holding all Nv components in registers.
 // The fp64 pipe bounds this path, so the code minimises fp64 instructions, not bytes.
 #pragma once
 #include "xf_common.cuh"
@@ -43,20 +44,20 @@ template <> struct Axes<0> { static constexpr int nd = 0, t1 = 1, t2 = 2; };
 template <> struct Axes<1> { static constexpr int nd = 1, t1 = 0, t2 = 2; };
 template <> struct Axes<2> { static constexpr int nd = 2, t1 = 1, t2 = 0; };
 
-// Shared-memory cell fields: 0..Nv-1 conserved variables, then p, c, u_n (normal velocity), 1/rho, sqrt(rho).
-__host__ __device__ constexpr int nfields(int N) { return N + 4 + 5; }
+// Staged cell fields, in this order: the Nv conserved variables, then the N + 5 fields the primitives kernel leaves
+// in the workspace: p, c, 1/rho, sqrt(rho), Gamma, chi_1..chi_N.
+__host__ __device__ constexpr int nstaged(int N) { return 2 * N + 9; }
+__host__ __device__ constexpr int nprimfields(int N) { return N + 5; }
 
-// Numerical flux at one face.  sm: staged fields, field f of stencil cell m at sm[f*FS + o[m]] (m = 0..5 <-> i-2..i+3,
-// the face lies between m = 2 and m = 3).  ga, gb: global cell indices of those two cells (for Gamma, chi_s, which
-// are only needed at the two adjacent cells and are read straight from global memory).  Writes Fhat_v to fout[v*FOS].
-template <int N_T, int DIR>
-__device__ __forceinline__ void face_flux(const int N, const double *__restrict__ sm, const int FS, const int (&o)[6],
-                                          const double *__restrict__ Gam, const double *__restrict__ chi,
-                                          const long long ga, const long long gb, const long long cells,
-                                          double *__restrict__ fout, const int FOS, int *__restrict__ status) {
+// Numerical flux at one face.  sm: staged fields, field f of stencil cell m at sm[f*FS + o[m]] (m = 0..5 <-> i-2..i+3;
+// the face lies between m = 2 and m = 3).  emit(v, Fhat_v, vnext) is called once per component, in the order
+// 0, 1+nd, 1+t1, 1+t2, 5, ..., Nv-1, 4 (vnext = the component that follows, -1 after the last).
+// Returns false if the Roe-averaged c~^2 is not positive.
+template <int DIR, class Emit>
+__device__ __forceinline__ bool face_flux(const int N, const double *sm, const int FS, const int (&o)[6], Emit &emit) {
   constexpr int nd = Axes<DIR>::nd, t1 = Axes<DIR>::t1, t2 = Axes<DIR>::t2;
   const int Nv = N + 4;
-  const int FP = Nv, FC = Nv + 1, FUD = Nv + 2, FRI = Nv + 3, FSR = Nv + 4;
+  const int FP = Nv, FC = Nv + 1, FRI = Nv + 2, FSR = Nv + 3, FG = Nv + 4, FCHI = Nv + 5;
 #define XS(f, m) sm[(f) * FS + o[m]]
 
   // ---- Roe-type average (reading R5): q~ = (w_a q_a + w_b q_b)/(w_a + w_b), w = sqrt(rho)
@@ -68,9 +69,9 @@ __device__ __forceinline__ void face_flux(const int N, const double *__restrict_
 #pragma unroll
   for (int q = 0; q < 3; ++q) ut[q] = fma(oma, XS(1 + q, 2), omb * XS(1 + q, 3));
   const double Ht = fma(oma, XS(4, 2) + XS(FP, 2), omb * (XS(4, 3) + XS(FP, 3)));
-  const double Gt = fma(oa, Gam[ga], ob * Gam[gb]);
+  const double Gt = fma(oa, XS(FG, 2), ob * XS(FG, 3));
   const double kt = 0.5 * fma(ut[0], ut[0], fma(ut[1], ut[1], ut[2] * ut[2]));
-  const double chiN = fma(oa, chi[(N - 1) * cells + ga], ob * chi[(N - 1) * cells + gb]);
+  const double chiN = fma(oa, XS(FCHI + N - 1, 2), ob * XS(FCHI + N - 1, 3));
 
   // ---- the dense functional pi.U_m for the six stencil cells; species part first
   double rho[6], piU[6];
@@ -82,7 +83,7 @@ __device__ __forceinline__ void face_flux(const int N, const double *__restrict_
   double c2acc = 0.0;
 #pragma unroll 3
   for (int i = 0; i < N - 1; ++i) {
-    const double zeta = fma(oa, chi[i * cells + ga], ob * chi[i * cells + gb]) - chiN;
+    const double zeta = fma(oa, XS(FCHI + i, 2), ob * XS(FCHI + i, 3)) - chiN;
     double y[6];
 #pragma unroll
     for (int m = 0; m < 6; ++m) y[m] = XS(5 + i, m);
@@ -93,7 +94,6 @@ __device__ __forceinline__ void face_flux(const int N, const double *__restrict_
   }
   // c~^2 = sum_s Y~_s chi~_s + Gamma~ (H~ - k~), with Y~_N = 1 - sum_{i<N} Y~_i
   const double c2 = chiN + c2acc + Gt * (Ht - kt);
-  if (!(c2 > 0.0)) atomicOr(status, XF_FLAG_NONPHYSICAL);
   const double ct = sqrt(c2);
   const double h = 0.5 * xf_rcp(c2);  // 1/(2 c~^2)
   const double Prho = fma(Gt, kt, chiN);
@@ -102,10 +102,11 @@ __device__ __forceinline__ void face_flux(const int N, const double *__restrict_
   double lam_m = 0.0, lam_0 = 0.0, lam_p = 0.0;  // LLF: max over the stencil of |u-c|, |u|, |u+c| (reading R8)
 #pragma unroll
   for (int m = 0; m < 6; ++m) {
-    const double mdot = fma(ut[0], XS(1, m), fma(ut[1], XS(2, m), ut[2] * XS(3, m)));
+    const double mn = XS(1 + nd, m);
+    const double mdot = fma(ut[nd], mn, fma(ut[t1], XS(1 + t1, m), ut[t2] * XS(1 + t2, m)));
     piU[m] += fma(Prho, rho[m], Gt * (XS(4, m) - mdot));
-    nuU[m] = fma(-ut[nd], rho[m], XS(1 + nd, m));
-    ud[m] = XS(FUD, m);
+    nuU[m] = fma(-ut[nd], rho[m], mn);
+    ud[m] = mn * XS(FRI, m);
     const double cm = XS(FC, m);
     lam_m = fmax(lam_m, fabs(ud[m] - cm));
     lam_0 = fmax(lam_0, fabs(ud[m]));
@@ -159,12 +160,12 @@ __device__ __forceinline__ void face_flux(const int N, const double *__restrict_
   const double delta = ct * (gL - g0);
   const double invG = xf_rcp(Gt);
   double F4 = fma(Ht, s, fma(ut[nd], delta, -(c2 * invG) * g1));
-  fout[0] = s;
-  fout[(1 + nd) * FOS] = fma(ut[nd], s, delta);
+  emit(0, s, 1 + nd);
+  emit(1 + nd, fma(ut[nd], s, delta), 1 + t1);
 
   // ---- fields travelling with u: two shear fields, N-1 species fields.  alpha_m = V_m - C rho_m with
   //      C = Roe average of V/rho; L F_m = u_m alpha_m, so f+-_m = (u_m +- Lambda)/2 * alpha_m.
-#define XF_LINEAR_FIELD(VIDX, DEXPR)                                                                   \
+#define XF_LINEAR_FIELD(VIDX, DEXPR, VNEXT)                                                            \
   {                                                                                                    \
     double V[6], fp[6], fm[6];                                                                         \
     _Pragma("unroll") for (int m = 0; m < 6; ++m) V[m] = XS(VIDX, m);                                  \
@@ -175,38 +176,20 @@ __device__ __forceinline__ void face_flux(const int N, const double *__restrict_
       fm[m] = am[m] * a;                                                                               \
     }                                                                                                  \
     const double g = weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + weno5(fm[5], fm[4], fm[3], fm[2], fm[1]); \
-    fout[(VIDX) * FOS] = fma(C, s, g);                                                                 \
     F4 = fma((DEXPR), g, F4);                                                                          \
+    emit(VIDX, fma(C, s, g), VNEXT);                                                                   \
   }
-  XF_LINEAR_FIELD(1 + t1, C)
-  XF_LINEAR_FIELD(1 + t2, C)
+  XF_LINEAR_FIELD(1 + t1, C, 1 + t2)
+  XF_LINEAR_FIELD(1 + t2, C, N > 1 ? 5 : 4)
 #pragma unroll 1
   for (int i = 0; i < N - 1; ++i) {
-    const double zeta = fma(oa, chi[i * cells + ga], ob * chi[i * cells + gb]) - chiN;
-    XF_LINEAR_FIELD(5 + i, -zeta * invG)
+    const double zeta = fma(oa, XS(FCHI + i, 2), ob * XS(FCHI + i, 3)) - chiN;
+    XF_LINEAR_FIELD(5 + i, -zeta * invG, i + 2 < N ? 6 + i : 4)
   }
 #undef XF_LINEAR_FIELD
-  fout[4 * FOS] = F4;
+  emit(4, F4, -1);
 #undef XS
-}
-
-// per-cell derived fields computed once at staging time
-__device__ __forceinline__ void derive_cell(double rho, double mn, double &ud, double &ri, double &sr) {
-  ri = xf_rcp(rho);
-  ud = mn * ri;
-  sr = sqrt(rho);
-}
-
-// out = alpha*Un + beta*(Us + dt*(acc + div)) or plain residual accumulation (see XfEpilogue)
-__device__ __forceinline__ void write_out(const XfEpilogue &E, double dt, long long gi, double div, double us) {
-  if (E.mode == 0) {
-    E.out[gi] = div;
-  } else if (E.mode == 1) {
-    E.out[gi] = E.acc[gi] + div;
-  } else {
-    const double L = E.has_acc ? E.acc[gi] + div : div;
-    E.out[gi] = fma(E.alpha, E.Un[gi], E.beta * fma(dt, L, us));
-  }
+  return c2 > 0.0;
 }
 
 }  // namespace xf

@@ -91,8 +91,8 @@ __device__ __forceinline__ double newton_T(const XfThermo &th, int N, const Cell
 template <int N_T>
 __global__ void __launch_bounds__(256)
 prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *__restrict__ U, double *__restrict__ T,
-            double *__restrict__ p_out, double *__restrict__ c_out, double *__restrict__ Gam_out,
-            double *__restrict__ chi_out, int *__restrict__ status, unsigned long long *__restrict__ itersum) {
+            double *__restrict__ prim, double *__restrict__ p_out, double *__restrict__ c_out,
+            int *__restrict__ status, unsigned long long *__restrict__ itersum) {
   const int N = N_T > 0 ? N_T : th.N;
   const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   int it = 0;
@@ -123,11 +123,15 @@ prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *_
     T[idx] = Tn;
     if (p_out) p_out[idx] = pr;
     if (c_out) c_out[idx] = cs;
-    if (Gam_out) Gam_out[idx] = Gam;
-    if (chi_out) {
+    if (prim) {  // what the sweeps stage per cell: p, c, 1/rho, sqrt(rho), Gamma, chi_s
+      prim[idx] = pr;
+      prim[G.cells + idx] = cs;
+      prim[2 * G.cells + idx] = xf_rcp(S.rho);
+      prim[3 * G.cells + idx] = sqrt(S.rho);
+      prim[4 * G.cells + idx] = Gam;
 #pragma unroll
       for (int s = 0; s < CellState<N_T>::NS; ++s)
-        if (s < N) chi_out[s * G.cells + idx] = th.Rs[s] * fma(-Gam, esR[s], Tn);  // chi_s = R_s T - Gamma e_s
+        if (s < N) prim[(5 + s) * G.cells + idx] = th.Rs[s] * fma(-Gam, esR[s], Tn);  // chi_s = R_s T - Gamma e_s
     }
     int flag = 0;
     if (!(S.rho > 0.0) || !(Tn > 0.0) || !(pr > 0.0)) flag |= XF_FLAG_NONPHYSICAL;
@@ -212,11 +216,11 @@ wavespeed_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const doub
     default: { CALL(0); break; }      \
   }
 
-int xf_launch_prim(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *p, double *c, double *Gam,
-                   double *chi, int *status, unsigned long long *itersum, cudaStream_t s) {
+int xf_launch_prim(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *prim, double *p,
+                   double *c, int *status, unsigned long long *itersum, cudaStream_t s) {
   const int threads = 256;
   const unsigned blocks = (unsigned)((G.cells + threads - 1) / threads);
-#define CALL(NT) prim_kernel<NT><<<blocks, threads, 0, s>>>(G, Th, U, T, p, c, Gam, chi, status, itersum)
+#define CALL(NT) prim_kernel<NT><<<blocks, threads, 0, s>>>(G, Th, U, T, prim, p, c, status, itersum)
   XF_DISPATCH_N(Th.N, CALL)
 #undef CALL
   return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;

@@ -1,23 +1,19 @@
 // xf_sweep_y.cu -- instantiations and launcher of the y-direction sweep (see xf_sweeps.cuh).
 #include "xf_sweeps.cuh"
 
-static int seg_len_for(const XfGrid &G, int n, long long columns) {
-  // split long columns when the grid alone cannot fill 148 SMs x 2 blocks; each split costs one extra face
-  int nseg = 1;
-  while (columns * nseg < 592 && n / (nseg * 2) >= 16) nseg *= 2;
-  return (n + nseg - 1) / nseg;
-}
-
-int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *p, const double *c, const double *Gam,
-                      const double *chi, const XfEpilogue &E, int *status, cudaStream_t s) {
+int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
+                      cudaStream_t s) {
   using namespace xf;
   constexpr int DIR = 1, OD = DIR == 1 ? 2 : 1;
-  const int strips = (G.n[0] + 31) / 32;
-  const int seg_len = seg_len_for(G, G.n[DIR], (long long)strips * G.n[OD]);
-  const int nseg = (G.n[DIR] + seg_len - 1) / seg_len;
-  const dim3 grid(strips, G.n[OD], nseg), block(32, YZ_W);
-  const size_t smem = sweep_yz_smem(N);
-#define CALL(NT) sweep_yz_kernel<NT, DIR><<<grid, block, smem, s>>>(G, N, U, p, c, Gam, chi, E, status, seg_len)
+  const int groups = (G.n[0] + YZ_LI - 1) / YZ_LI;
+  // one warp marches a whole column unless it is very long; each split costs one extra face row
+  const int n = G.n[DIR];
+  const int max_len = YZ_MAXCH * YZ_LJ - 1;
+  const int nseg = (n + max_len - 1) / max_len;
+  const int seg_len = (n + nseg - 1) / nseg;
+  const dim3 grid(groups, G.n[OD], nseg);
+  const size_t smem = sizeof(double) * warp_smem_doubles(N, YZ_LI, YZ_LJ);
+#define CALL(NT) sweep_kernel<NT, DIR, YZ_LI, YZ_LJ><<<grid, 32, smem, s>>>(G, N, U, prim, E, status, seg_len)
   XF_DISPATCH_SWEEP_N(N, CALL)
 #undef CALL
   return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
@@ -26,9 +22,9 @@ int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *p, 
 int xf_sweep_y_init() {
   using namespace xf;
   cudaError_t e = cudaSuccess;
-#define CALL(NT)                                                                                          \
-  e = cudaFuncSetAttribute(sweep_yz_kernel<NT, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,         \
-                           (int)sweep_yz_smem(NT > 0 ? NT : XF_MAXN));                                    \
+#define CALL(NT)                                                                                               \
+  e = cudaFuncSetAttribute(sweep_kernel<NT, 1, YZ_LI, YZ_LJ>, cudaFuncAttributeMaxDynamicSharedMemorySize,     \
+                           (int)(sizeof(double) * warp_smem_doubles(NT > 0 ? NT : XF_MAXN, YZ_LI, YZ_LJ)));   \
   if (e != cudaSuccess) return XF_ECUDA;
   CALL(0) CALL(1) CALL(2) CALL(3) CALL(4) CALL(10)
 #undef CALL

@@ -1,175 +1,216 @@
-// xf_sweeps.cuh -- the marching sweep kernels built around xf::face_flux (see xf_flux.cuh).
+// xf_sweeps.cuh -- the marching sweep kernel built around xf::face_flux (see xf_flux.cuh).
 //
-// x sweep: lanes run ALONG the stencil.  All interior rows of one k-plane are contiguous in memory (row pitch =
-//   padded nx), so a plane is swept as ONE long flat pencil; the few faces whose stencil straddles a row end are
-//   computed on valid (ghost) data and never used (5 of every nx+6).  A block marches a segment of that pencil in
-//   chunks of TX faces: stage TX+5 cells in shared memory, one face per thread, fluxes to shared memory, one cell
-//   update per thread; the last face of a chunk is carried to the next, so no face is computed twice.
-// y / z sweeps: lanes run ACROSS 32 neighbouring pencils (consecutive i -> coalesced), warps along the stencil.
-//   A block marches a column in chunks of W faces over a ring of W+5 staged rows.
+// Every WARP is autonomous: it owns a private ring of staged stencil rows in shared memory, fills it with
+// cp.async (LDGSTS) one chunk ahead of the arithmetic, exchanges face fluxes with warp shuffles, and never meets
+// a block-wide barrier -- the fp64 pipe is the bound and must not wait on memory.
+//
+// A warp's 32 lanes are laid out LI (contiguous, along i) x LJ (along the sweep direction); one lane = one face.
+//   x sweep: LI = 1, LJ = 32.  All interior rows of one k-plane are contiguous in memory (row pitch = padded nx),
+//     so a plane is swept as ONE long flat pencil; the few faces whose stencil straddles a row end are computed
+//     on valid (ghost) data and never used (5 of every nx+6).
+//   y / z sweeps: LI x LJ = 4 x 8: four neighbouring pencils (one 32-byte sector per row) marched 8 faces at a time.
+// A chunk of LJ face rows needs LJ + 5 stencil rows; the ring holds 2 LJ + 5 rows so that the LJ new rows of the
+// next chunk land while the current chunk is computed.  Face row f of a segment is the lower face of cell f; its
+// stencil is rows f .. f+5; the lane that owns face f updates cell f-1 from its own flux and that of face f-1
+// (the lane LI below it, or the carry left in shared memory by the previous chunk).
 #pragma once
 #include "xf_flux.cuh"
 
 namespace xf {
 
-constexpr int TX = 128;        // x sweep: faces per chunk = threads per block
-constexpr int XCHUNKS = 8;     // x sweep: chunks per block segment (segment = XCHUNKS*TX - 1 cells)
-constexpr int YZ_W = 8;        // y/z sweeps: warps per block = faces per chunk
-constexpr int YZ_R = YZ_W + 5; // ring rows
+constexpr int X_LI = 1, X_LJ = 32, X_NCH = 16;   // x sweep: segment = X_NCH chunks = 32*X_NCH faces, 32*X_NCH - 1 cells
+constexpr int YZ_LI = 4, YZ_LJ = 8, YZ_MAXCH = 64;
 
-template <int N_T>
-__host__ __device__ constexpr int nspec_static() { return N_T > 0 ? N_T : XF_MAXN; }
-
-__host__ inline size_t sweep_x_smem(int N) {
-  return sizeof(double) * ((size_t)nfields(N) * (TX + 5) + (size_t)(N + 4) * (TX + 1));
-}
-__host__ inline size_t sweep_yz_smem(int N) {
-  return sizeof(double) * ((size_t)nfields(N) * YZ_R * 32 + (size_t)(N + 4) * (YZ_W + 1) * 32);
+__host__ __device__ constexpr int ring_rows(int LJ) { return 2 * LJ + 5; }
+__host__ __device__ inline size_t warp_smem_doubles(int N, int LI, int LJ) {
+  return (size_t)nstaged(N) * ring_rows(LJ) * LI + 2 * (size_t)(N + 4) * LI;
 }
 
-template <int N_T>
-__global__ void __launch_bounds__(TX)
-sweep_x_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const double *__restrict__ P,
-               const double *__restrict__ Cs, const double *__restrict__ Gam, const double *__restrict__ chi,
-               const XfEpilogue E, int *__restrict__ status, const int segs_per_plane) {
-  const int N = N_T > 0 ? N_T : Nrt;
-  const int Nv = N + 4, NF = nfields(N);
-  extern __shared__ double smem[];
-  constexpr int CS = TX + 5;          // cell slots per field
-  constexpr int FSL = TX + 1;         // flux slots per variable
-  double *sm = smem;
-  double *fb = smem + (size_t)NF * CS;
+__device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int NPENDING>
+__device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;" ::"n"(NPENDING) : "memory");
+}
 
-  const int t = threadIdx.x;
-  const int plane = blockIdx.x / segs_per_plane;            // interior k
-  const int seg = blockIdx.x - plane * segs_per_plane;
-  const long long L = (long long)G.n[1] * G.np[0];          // flat cells of the plane's interior rows
-  const long long base = (long long)(plane + G.g[2]) * G.st[2] + (long long)G.g[1] * G.st[1];
-  constexpr int SEG = XCHUNKS * TX - 1;
-  const long long c0 = (long long)seg * SEG;                // first cell of this block's segment
-  const long long c1 = c0 + SEG < L ? c0 + SEG : L;         // one past the last cell
-  const double dt = E.mode == 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
-  const double ninv = -G.inv_d[0];
+// Differences each flux component against the face below (Eq. 13) and writes the cell value: a plain residual,
+// an accumulated residual, or the Runge-Kutta stage combination out = alpha*Un + beta*(Us + dt*(acc + div)) (Eq. 16).
+// The acc / Un operands of the NEXT component are fetched while the current one is being reconstructed.
+template <int LI>
+struct CellWriter {
+  const XfEpilogue &E;
+  const double *sm_us;    // staged U^s of the cell this lane updates: sm_us[v * FS]
+  double *carry_rd, *carry_wr;
+  long long gi, cells;
+  double dt, ninv, nacc, nun;
+  int FS, li;
+  bool write_ok, first_row, last_row, need_acc, need_un;
 
-  for (int q = 0; q < XCHUNKS; ++q) {
-    const long long f0 = c0 + (long long)q * TX;            // first face of the chunk (face f = left face of cell f)
-    if (f0 > c1) break;
-    // ---- stage cells f0-3 .. f0+TX+1 (slot x <-> cell f0-3+x)
-    for (int x = t; x < CS; x += TX) {
-      long long gi = base + f0 - 3 + x;
-      gi = gi < 0 ? 0 : (gi >= G.cells ? G.cells - 1 : gi);  // garbage faces at the very ends stay in bounds
-      for (int v = 0; v < Nv; ++v) sm[v * CS + x] = U[v * G.cells + gi];
-      sm[Nv * CS + x] = P[gi];
-      sm[(Nv + 1) * CS + x] = Cs[gi];
-      double ud, ri, sr;
-      derive_cell(sm[x], sm[1 * CS + x], ud, ri, sr);
-      sm[(Nv + 2) * CS + x] = ud;
-      sm[(Nv + 3) * CS + x] = ri;
-      sm[(Nv + 4) * CS + x] = sr;
+  __device__ __forceinline__ void preload(int v) {
+    if (write_ok) {
+      if (need_acc) nacc = E.acc[v * cells + gi];
+      if (need_un) nun = E.Un[v * cells + gi];
     }
-    __syncthreads();
-    // ---- one face per thread: face f0+t between cells f0+t-1 (slot t+2) and f0+t (slot t+3)
-    const long long f = f0 + t;
-    if (f <= c1) {
-      const int o[6] = {t, t + 1, t + 2, t + 3, t + 4, t + 5};
-      long long ga = base + f - 1, gb = base + f;
-      ga = ga < 0 ? 0 : ga;
-      gb = gb >= G.cells ? G.cells - 1 : gb;
-      face_flux<N_T, 0>(N, sm, CS, o, Gam, chi, ga, gb, G.cells, fb + (t + 1), FSL, status);
-    }
-    __syncthreads();
-    // ---- one cell per thread: cell f0+t-1 from the faces in flux slots t and t+1
-    const long long cc = f0 + t - 1;
-    if (cc >= c0 && cc < c1) {
-      const int i = (int)(cc % G.np[0]);
-      if (i >= G.g[0] && i < G.g[0] + G.n[0]) {
-        const long long gi = base + cc;
-        for (int v = 0; v < Nv; ++v) {
-          const double div = (fb[v * FSL + t + 1] - fb[v * FSL + t]) * ninv;
-          write_out(E, dt, v * G.cells + gi, div, sm[v * CS + t + 2]);
-        }
+  }
+  __device__ __forceinline__ void operator()(int v, double F, int vnext) {
+    double prev = __shfl_up_sync(0xffffffffu, F, LI);
+    if (first_row) prev = carry_rd[v * LI + li];
+    if (last_row) carry_wr[v * LI + li] = F;
+    const double a = nacc, un = nun;
+    if (vnext >= 0) preload(vnext);
+    if (write_ok) {
+      const double div = (F - prev) * ninv;
+      const long long idx = v * cells + gi;
+      if (E.mode == 0) {
+        E.out[idx] = div;
+      } else if (E.mode == 1) {
+        E.out[idx] = a + div;
+      } else {
+        const double L = need_acc ? a + div : div;
+        const double us = sm_us[v * FS];
+        E.out[idx] = need_un ? fma(E.alpha, un, E.beta * fma(dt, L, us)) : E.beta * fma(dt, L, us);
       }
     }
-    __syncthreads();
-    if (t < Nv) fb[t * FSL] = fb[t * FSL + TX];             // carry the last face to the next chunk
   }
-}
+};
 
-// DIR = 1 (y) or 2 (z).  Block (32, YZ_W): lane <-> i, warp <-> face within the chunk.
-template <int N_T, int DIR>
-__global__ void __launch_bounds__(32 * YZ_W)
-sweep_yz_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const double *__restrict__ P,
-                const double *__restrict__ Cs, const double *__restrict__ Gam, const double *__restrict__ chi,
-                const XfEpilogue E, int *__restrict__ status, const int seg_len) {
+// One warp = one segment of one pencil group.  DIR = 0: blockIdx.x enumerates (k-plane, segment of the flat pencil).
+// DIR = 1, 2: blockIdx = (group of LI pencils along i, index along the other transverse direction, segment).
+template <int N_T, int DIR, int LI, int LJ>
+__global__ void __launch_bounds__(32, 12)
+sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const double *__restrict__ prim,
+             const XfEpilogue E, int *__restrict__ status, const int seg_param) {
+  static_assert(LI * LJ == 32, "one lane per face");
   const int N = N_T > 0 ? N_T : Nrt;
-  const int Nv = N + 4, NF = nfields(N);
+  const int Nv = N + 4, NST = nstaged(N);
+  constexpr int RR = ring_rows(LJ);
+  constexpr int FS = RR * LI;
   extern __shared__ double smem[];
-  constexpr int CS = YZ_R * 32;
-  constexpr int FSL = (YZ_W + 1) * 32;
   double *sm = smem;
-  double *fb = smem + (size_t)NF * CS;
+  double *carry = smem + (size_t)NST * FS;
 
-  const int lane = threadIdx.x, w = threadIdx.y;
-  constexpr int OD = DIR == 1 ? 2 : 1;                      // the other transverse direction
-  const int i = G.g[0] + blockIdx.x * 32 + lane;
-  const bool lane_ok = i < G.g[0] + G.n[0];
-  const int ic = lane_ok ? i : G.g[0] + G.n[0] - 1;         // clamped: idle lanes stage valid data
-  const long long colbase = (long long)(blockIdx.y + G.g[OD]) * G.st[OD] + ic;
-  const long long sst = G.st[DIR];
-  const int n = G.n[DIR];
-  const int q0 = blockIdx.z * seg_len;                      // first interior cell of this block's segment
-  const int q1 = q0 + seg_len < n ? q0 + seg_len : n;       // one past the last
-  const double dt = E.mode == 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
-  const double ninv = -G.inv_d[DIR];
+  const int lane = threadIdx.x;
+  const int li = lane % LI, lj = lane / LI;
 
-  // stage padded row r into ring slot r % YZ_R (each warp stages whole rows: 32 consecutive i per field)
-  auto stage_row = [&](int r) {
-    const int x = (r % YZ_R) * 32 + lane;
-    const long long gi = colbase + (long long)r * sst;
-    for (int v = 0; v < Nv; ++v) sm[v * CS + x] = U[v * G.cells + gi];
-    sm[Nv * CS + x] = P[gi];
-    sm[(Nv + 1) * CS + x] = Cs[gi];
-    double ud, ri, sr;
-    derive_cell(sm[x], sm[(1 + DIR) * CS + x], ud, ri, sr);
-    sm[(Nv + 2) * CS + x] = ud;
-    sm[(Nv + 3) * CS + x] = ri;
-    sm[(Nv + 4) * CS + x] = sr;
+  // ---- this warp's segment: faces f_begin .. f_end (inclusive), cells f_begin .. f_end - 1
+  long long base;      // global index of stencil row 0 at li = 0 (may be negative for the x sweep: clamped on use)
+  long long sst;       // stride between stencil rows
+  int f_begin, f_end;
+  int i0 = 0, imax = 0;  // y/z: first i of this pencil group, last valid i
+  if (DIR == 0) {
+    const int segs_per_plane = seg_param;
+    const int plane = blockIdx.x / segs_per_plane;
+    const int seg = blockIdx.x - plane * segs_per_plane;
+    const int L = G.n[1] * G.np[0];                          // flat cells of the plane's interior rows
+    constexpr int SEGC = X_NCH * 32 - 1;
+    f_begin = seg * SEGC;
+    f_end = f_begin + SEGC < L ? f_begin + SEGC : L;
+    base = (long long)(plane + G.g[2]) * G.st[2] + (long long)G.g[1] * G.st[1] - 3;  // row r <-> flat cell r - 3
+    sst = 1;
+  } else {
+    constexpr int OD = DIR == 1 ? 2 : 1;                     // the other transverse direction
+    const int seg_len = seg_param;
+    i0 = G.g[0] + blockIdx.x * LI;
+    imax = G.g[0] + G.n[0] - 1;
+    base = (long long)(blockIdx.y + G.g[OD]) * G.st[OD];     // + i, + r * sst
+    sst = G.st[DIR];
+    f_begin = blockIdx.z * seg_len;
+    f_end = f_begin + seg_len < G.n[DIR] ? f_begin + seg_len : G.n[DIR];
+  }
+  auto row_addr = [&](int r, int l) -> long long {           // global cell index of stencil row r, lane column l
+    if (DIR == 0) {
+      long long gi = base + r;
+      return gi < 0 ? 0 : (gi >= G.cells ? G.cells - 1 : gi);  // garbage faces at the very ends stay in bounds
+    }
+    const int ii = i0 + l < imax ? i0 + l : imax;            // idle lanes stage valid data
+    const int rr = r < G.np[DIR] ? r : G.np[DIR] - 1;        // rows past the last chunk's needs stay in bounds
+    return base + ii + (long long)rr * sst;
+  };
+  auto stage = [&](int slot, long long gi) {
+    double *dst = sm + slot;
+#pragma unroll
+    for (int f = 0; f < (N_T > 0 ? nstaged(N_T) : 1); ++f) {
+      if (N_T > 0) cp_async8(dst + f * FS, (f < Nv ? U + (size_t)f * G.cells : prim + (size_t)(f - Nv) * G.cells) + gi);
+    }
+    if (N_T == 0) {
+      for (int f = 0; f < NST; ++f)
+        cp_async8(dst + f * FS, (f < Nv ? U + (size_t)f * G.cells : prim + (size_t)(f - Nv) * G.cells) + gi);
+    }
   };
 
-  const int nfaces = q1 - q0 + 1;                           // faces q0 .. q1 (face f lies between padded rows f+2, f+3)
-  const int nchunks = (nfaces + YZ_W - 1) / YZ_W;
-  for (int c = 0; c < nchunks; ++c) {
-    const int f0 = q0 + c * YZ_W;
-    // ---- rows needed by this chunk: f0 .. f0+W+4; all but the last W are already in the ring (except chunk 0)
-    if (c == 0) {
-      for (int r = f0 + w; r < f0 + 5; r += YZ_W) stage_row(r);
-    }
-    {
-      const int r = f0 + 5 + w;
-      if (r <= q1 + 5) stage_row(r);
-    }
-    __syncthreads();
-    const int f = f0 + w;
-    if (f <= q1 && lane_ok) {
-      int o[6];
-#pragma unroll
-      for (int m = 0; m < 6; ++m) o[m] = ((f + m) % YZ_R) * 32 + lane;
-      const long long ga = colbase + (long long)(f + 2) * sst, gb = ga + sst;
-      face_flux<N_T, DIR>(N, sm, CS, o, Gam, chi, ga, gb, G.cells, fb + (w + 1) * 32 + lane, FSL, status);
-    }
-    __syncthreads();
-    const int qq = f - 1;                                   // cell between faces qq (slot w) and qq+1 (slot w+1)
-    if (qq >= q0 && qq < q1 && lane_ok) {
-      const long long gi = colbase + (long long)(qq + 3) * sst;
-      const int x = ((qq + 3) % YZ_R) * 32 + lane;
-      for (int v = 0; v < Nv; ++v) {
-        const double div = (fb[v * FSL + (w + 1) * 32 + lane] - fb[v * FSL + w * 32 + lane]) * ninv;
-        write_out(E, dt, v * G.cells + gi, div, sm[v * CS + x]);
-      }
-    }
-    __syncthreads();
-    for (int v = w; v < Nv; v += YZ_W) fb[v * FSL + lane] = fb[v * FSL + YZ_W * 32 + lane];  // carry the last face
+  // ---- prologue: rows f_begin .. f_begin + LJ + 4 into ring slots 0 .. LJ + 4
+  for (int idx = lane; idx < (LJ + 5) * LI; idx += 32) {
+    const int r = idx / LI, l = idx - r * LI;
+    stage(r * LI + l, row_addr(f_begin + r, l));
   }
+  cp_async_commit();
+
+  const double dt = E.mode == 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
+  CellWriter<LI> W{E};
+  W.cells = G.cells;
+  W.dt = dt;
+  W.ninv = -G.inv_d[DIR];
+  W.FS = FS;
+  W.li = li;
+  W.first_row = lj == 0;
+  W.last_row = lj == LJ - 1;
+  W.need_acc = E.mode == 1 || (E.mode == 2 && E.has_acc);
+  W.need_un = E.mode == 2 && E.alpha != 0.0;
+  W.nacc = 0.0;
+  W.nun = 0.0;
+  const bool lane_ok = DIR == 0 || i0 + li <= imax;
+
+  int rb = 0;       // ring slot (row) of stencil row fc
+  int par = 0;
+  bool bad = false;
+  for (int fc = f_begin; fc <= f_end; fc += LJ) {
+    // ---- prefetch the LJ new rows of the next chunk: rows fc + LJ + 5 + lj
+    if (fc + LJ <= f_end) {
+      int slot = rb + LJ + 5 + lj;
+      slot -= slot >= RR ? RR : 0;
+      stage(slot * LI + li, row_addr(fc + LJ + 5 + lj, li));
+    }
+    cp_async_commit();
+    cp_async_wait<1>();   // everything but the group just committed has landed
+    __syncwarp();
+
+    const int f = fc + lj;
+    int o[6];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) {
+      int s = rb + lj + m;
+      s -= s >= RR ? RR : 0;
+      o[m] = s * LI + li;
+    }
+    // the cell this lane updates: f - 1 (between faces f - 1 and f), staged at stencil row f + 2 (m = 2)
+    bool ok = lane_ok && f > f_begin && f <= f_end;
+    long long gi;
+    if (DIR == 0) {
+      const int cc = f - 1;
+      const int i = cc % G.np[0];
+      ok = ok && i >= G.g[0] && i < G.g[0] + G.n[0];
+      gi = base + 3 + cc;
+    } else {
+      gi = base + (i0 + li) + (long long)(f + 2) * sst;
+    }
+    W.write_ok = ok;
+    W.gi = gi;
+    W.sm_us = sm + o[2];
+    W.carry_rd = carry + par * Nv * LI;
+    W.carry_wr = carry + (par ^ 1) * Nv * LI;
+    W.preload(0);
+    const bool c2ok = face_flux<DIR>(N, sm, FS, o, W);
+    bad = bad || (!c2ok && lane_ok && f <= f_end);
+    __syncwarp();         // all lanes are done with the rows the next iteration's prefetch overwrites
+    rb += LJ;
+    rb -= rb >= RR ? RR : 0;
+    par ^= 1;
+  }
+  cp_async_wait<0>();
+  if (bad) atomicOr(status, XF_FLAG_NONPHYSICAL);
 }
 
 }  // namespace xf
