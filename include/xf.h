@@ -69,7 +69,7 @@ int xf_destroy(xf_ctx *ctx);
 
 size_t xf_num_vars(const xf_ctx *ctx);            /* Nv                                                        */
 size_t xf_padded_cells(const xf_ctx *ctx);        /* product of padded extents                                 */
-size_t xf_rhs_workspace_bytes(const xf_ctx *ctx); /* scratch for xf_convective_rhs: (N + 5) fields             */
+size_t xf_rhs_workspace_bytes(const xf_ctx *ctx); /* scratch for xf_convective_rhs: (N + 4) fields             */
 size_t xf_workspace_bytes(const xf_ctx *ctx);     /* scratch for xf_rk3_step: the above + 3 U-sized buffers    */
 
 /* Ghost-cell fill ("specific boundary conditions"; reading R10): periodic wrap,

@@ -90,7 +90,7 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
     rc = xf_launch_ghosts(c->G, c->Nv, c->bc, c->bc_state_dev, U, s, &c->launches);
   }
   if (rc != XF_OK) return rc;
-  double *prim = static_cast<double *>(work);  // p, c, 1/rho, sqrt(rho), Gamma, chi_1..chi_N
+  double *prim = static_cast<double *>(work);  // p, c, 1/rho, Gamma, chi_1..chi_N
   {
     Timed t(c, XF_K_PRIM, s);
     rc = xf_launch_prim(c->G, c->Th, U, T, prim, nullptr, nullptr, c->status_dev, nullptr, s);
@@ -99,7 +99,8 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
   if (rc != XF_OK) return rc;
   const int nact = count_active(c->G);
   int done = 0;
-  for (int d = 0; d < 3; ++d) {
+  for (int dd = 0; dd < 3; ++dd) {
+    const int d = getenv("XF_REV") ? 2 - dd : dd;
     if (c->G.n[d] == 1) continue;
     XfEpilogue E;
     if (done == nact - 1) {
@@ -127,7 +128,7 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
 int rk3(xf_ctx *c, double *U, double *T, double dt, double cfl, const double *S_dev, void *work, cudaStream_t s) {
   const size_t n = (size_t)c->G.cells;
   double *w = static_cast<double *>(work);
-  double *U1 = w + (size_t)(c->N + 5) * n;
+  double *U1 = w + (size_t)(c->N + 4) * n;
   double *U2 = U1 + (size_t)c->Nv * n;
   double *acc = U2 + (size_t)c->Nv * n;
   XfEpilogue E;
@@ -264,9 +265,9 @@ int xf_destroy(xf_ctx *c) {
 
 size_t xf_num_vars(const xf_ctx *c) { return c ? (size_t)c->Nv : 0; }
 size_t xf_padded_cells(const xf_ctx *c) { return c ? (size_t)c->G.cells : 0; }
-size_t xf_rhs_workspace_bytes(const xf_ctx *c) { return c ? field_bytes(c) * (size_t)(c->N + 5) : 0; }
+size_t xf_rhs_workspace_bytes(const xf_ctx *c) { return c ? field_bytes(c) * (size_t)(c->N + 4) : 0; }
 size_t xf_workspace_bytes(const xf_ctx *c) {
-  return c ? field_bytes(c) * (size_t)(c->N + 5 + 3 * c->Nv) : 0;
+  return c ? field_bytes(c) * (size_t)(c->N + 4 + 3 * c->Nv) : 0;
 }
 
 int xf_fill_ghosts(xf_ctx *c, double *U, void *stream) {

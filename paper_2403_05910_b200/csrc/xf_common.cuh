@@ -54,7 +54,7 @@ struct XfEpilogue {
 };
 
 // launch helpers implemented per translation unit
-// prim: the N + 5 workspace fields p, c, 1/rho, sqrt(rho), Gamma, chi_1..chi_N ([field][padded cells]); NULL = do
+// prim: the N + 4 workspace fields p, c, 1/rho, Gamma, chi_1..chi_N ([field][padded cells]); NULL = do
 // not store them (xf_primitives), p_out / c_out: optional separate copies of p and c for the caller.
 int xf_launch_prim(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *prim, double *p_out,
                    double *c_out, int *status, unsigned long long *itersum, cudaStream_t s);

@@ -44,10 +44,10 @@ template <> struct Axes<0> { static constexpr int nd = 0, t1 = 1, t2 = 2; };
 template <> struct Axes<1> { static constexpr int nd = 1, t1 = 0, t2 = 2; };
 template <> struct Axes<2> { static constexpr int nd = 2, t1 = 1, t2 = 0; };
 
-// Staged cell fields, in this order: the Nv conserved variables, then the N + 5 fields the primitives kernel leaves
-// in the workspace: p, c, 1/rho, sqrt(rho), Gamma, chi_1..chi_N.
-__host__ __device__ constexpr int nstaged(int N) { return 2 * N + 9; }
-__host__ __device__ constexpr int nprimfields(int N) { return N + 5; }
+// Staged cell fields, in this order: the Nv conserved variables, then the N + 4 fields the primitives kernel leaves
+// in the workspace: p, c, 1/rho, Gamma, chi_1..chi_N.
+__host__ __device__ constexpr int nstaged(int N) { return 2 * N + 8; }
+__host__ __device__ constexpr int nprimfields(int N) { return N + 4; }
 
 // Numerical flux at one face.  sm: staged fields, field f of stencil cell m at sm[f*FS + o[m]] (m = 0..5 <-> i-2..i+3;
 // the face lies between m = 2 and m = 3).  emit(v, Fhat_v, vnext) is called once per component, in the order
@@ -57,14 +57,15 @@ template <int DIR, class Emit>
 __device__ __forceinline__ bool face_flux(const int N, const double *sm, const int FS, const int (&o)[6], Emit &emit) {
   constexpr int nd = Axes<DIR>::nd, t1 = Axes<DIR>::t1, t2 = Axes<DIR>::t2;
   const int Nv = N + 4;
-  const int FP = Nv, FC = Nv + 1, FRI = Nv + 2, FSR = Nv + 3, FG = Nv + 4, FCHI = Nv + 5;
+  const int FP = Nv, FC = Nv + 1, FRI = Nv + 2, FG = Nv + 3, FCHI = Nv + 4;
 #define XS(f, m) sm[(f) * FS + o[m]]
 
-  // ---- Roe-type average (reading R5): q~ = (w_a q_a + w_b q_b)/(w_a + w_b), w = sqrt(rho)
-  const double wa = XS(FSR, 2), wb = XS(FSR, 3);
-  const double winv = xf_rcp(wa + wb);
-  const double oa = wa * winv, ob = wb * winv;
-  const double oma = oa * XS(FRI, 2), omb = ob * XS(FRI, 3);  // weights acting on conserved quantities
+  // ---- Roe-type average (reading R5): q~ = (w_a q_a + w_b q_b)/(w_a + w_b), w = sqrt(rho); with
+  //      r = w_b/w_a = sqrt(rho_b/rho_a) the weights are 1/(1+r) and r/(1+r)
+  const double ria = XS(FRI, 2), rib = XS(FRI, 3);
+  const double r = sqrt(XS(0, 3) * ria);
+  const double oa = xf_rcp(1.0 + r), ob = r * oa;
+  const double oma = oa * ria, omb = ob * rib;                // weights acting on conserved quantities
   double ut[3];
 #pragma unroll
   for (int q = 0; q < 3; ++q) ut[q] = fma(oma, XS(1 + q, 2), omb * XS(1 + q, 3));

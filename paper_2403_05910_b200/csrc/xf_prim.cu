@@ -123,15 +123,14 @@ prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *_
     T[idx] = Tn;
     if (p_out) p_out[idx] = pr;
     if (c_out) c_out[idx] = cs;
-    if (prim) {  // what the sweeps stage per cell: p, c, 1/rho, sqrt(rho), Gamma, chi_s
+    if (prim) {  // what the sweeps stage per cell: p, c, 1/rho, Gamma, chi_s
       prim[idx] = pr;
       prim[G.cells + idx] = cs;
       prim[2 * G.cells + idx] = xf_rcp(S.rho);
-      prim[3 * G.cells + idx] = sqrt(S.rho);
-      prim[4 * G.cells + idx] = Gam;
+      prim[3 * G.cells + idx] = Gam;
 #pragma unroll
       for (int s = 0; s < CellState<N_T>::NS; ++s)
-        if (s < N) prim[(5 + s) * G.cells + idx] = th.Rs[s] * fma(-Gam, esR[s], Tn);  // chi_s = R_s T - Gamma e_s
+        if (s < N) prim[(4 + s) * G.cells + idx] = th.Rs[s] * fma(-Gam, esR[s], Tn);  // chi_s = R_s T - Gamma e_s
     }
     int flag = 0;
     if (!(S.rho > 0.0) || !(Tn > 0.0) || !(pr > 0.0)) flag |= XF_FLAG_NONPHYSICAL;

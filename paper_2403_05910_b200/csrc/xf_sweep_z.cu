@@ -5,15 +5,17 @@ int xf_launch_sweep_z(const XfGrid &G, int N, const double *U, const double *pri
                       cudaStream_t s) {
   using namespace xf;
   constexpr int DIR = 2, OD = DIR == 1 ? 2 : 1;
-  const int groups = (G.n[0] + YZ_LI - 1) / YZ_LI;
-  // one warp marches a whole column unless it is very long; each split costs one extra face row
+  const int strips = (G.n[0] + 31) / 32;
+  // one block marches a whole column unless the grid alone cannot fill 148 SMs x 2 blocks a few times over;
+  // each split costs one extra face row
   const int n = G.n[DIR];
-  const int max_len = YZ_MAXCH * YZ_LJ - 1;
-  const int nseg = (n + max_len - 1) / max_len;
+  int nseg = 1;
+  while ((long long)strips * G.n[OD] * nseg < 1184 && n / (nseg * 2) >= 4 * YZ_W) nseg *= 2;
   const int seg_len = (n + nseg - 1) / nseg;
-  const dim3 grid(groups, G.n[OD], nseg);
-  const size_t smem = sizeof(double) * warp_smem_doubles(N, YZ_LI, YZ_LJ);
-#define CALL(NT) sweep_kernel<NT, DIR, YZ_LI, YZ_LJ><<<grid, 32, smem, s>>>(G, N, U, prim, E, status, seg_len)
+  nseg = (n + seg_len - 1) / seg_len;
+  const dim3 grid(strips, G.n[OD], nseg), block(32, YZ_W);
+  const size_t smem = sizeof(double) * yz_smem_doubles(N, YZ_W);
+#define CALL(NT) sweep_yz_kernel<NT, DIR, YZ_W><<<grid, block, smem, s>>>(G, N, U, prim, E, status, seg_len)
   XF_DISPATCH_SWEEP_N(N, CALL)
 #undef CALL
   return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
@@ -22,9 +24,9 @@ int xf_launch_sweep_z(const XfGrid &G, int N, const double *U, const double *pri
 int xf_sweep_z_init() {
   using namespace xf;
   cudaError_t e = cudaSuccess;
-#define CALL(NT)                                                                                               \
-  e = cudaFuncSetAttribute(sweep_kernel<NT, 2, YZ_LI, YZ_LJ>, cudaFuncAttributeMaxDynamicSharedMemorySize,     \
-                           (int)(sizeof(double) * warp_smem_doubles(NT > 0 ? NT : XF_MAXN, YZ_LI, YZ_LJ)));   \
+#define CALL(NT)                                                                                          \
+  e = cudaFuncSetAttribute(sweep_yz_kernel<NT, 2, YZ_W>, cudaFuncAttributeMaxDynamicSharedMemorySize,    \
+                           (int)(sizeof(double) * yz_smem_doubles(NT > 0 ? NT : XF_MAXN, YZ_W)));         \
   if (e != cudaSuccess) return XF_ECUDA;
   CALL(0) CALL(1) CALL(2) CALL(3) CALL(4) CALL(10)
 #undef CALL

@@ -19,7 +19,7 @@
 namespace xf {
 
 constexpr int X_LI = 1, X_LJ = 32, X_NCH = 16;   // x sweep: segment = X_NCH chunks = 32*X_NCH faces, 32*X_NCH - 1 cells
-constexpr int YZ_LI = 4, YZ_LJ = 8, YZ_MAXCH = 64;
+constexpr int YZ_W = 4;                           // y/z sweeps: warps per block = face rows per chunk
 
 __host__ __device__ constexpr int ring_rows(int LJ) { return 2 * LJ + 5; }
 __host__ __device__ inline size_t warp_smem_doubles(int N, int LI, int LJ) {
@@ -59,21 +59,27 @@ struct CellWriter {
     double prev = __shfl_up_sync(0xffffffffu, F, LI);
     if (first_row) prev = carry_rd[v * LI + li];
     if (last_row) carry_wr[v * LI + li] = F;
-    const double a = nacc, un = nun;
-    if (vnext >= 0) preload(vnext);
     if (write_ok) {
       const double div = (F - prev) * ninv;
       const long long idx = v * cells + gi;
       if (E.mode == 0) {
         E.out[idx] = div;
       } else if (E.mode == 1) {
-        E.out[idx] = a + div;
+        E.out[idx] = nacc + div;
       } else {
-        const double L = need_acc ? a + div : div;
+        const double L = need_acc ? nacc + div : div;
         const double us = sm_us[v * FS];
-        E.out[idx] = need_un ? fma(E.alpha, un, E.beta * fma(dt, L, us)) : E.beta * fma(dt, L, us);
+        E.out[idx] = need_un ? fma(E.alpha, nun, E.beta * fma(dt, L, us)) : E.beta * fma(dt, L, us);
       }
     }
+    if (vnext >= 0) preload(vnext);   // after the use: no register copy, the load flies during the next field
+  }
+  // pull the acc / Un operands of cell g (this lane's cell of a later chunk) into L2 ahead of time
+  __device__ __forceinline__ void prefetch_l2(long long g, int Nv) const {
+    if (need_acc)
+      for (int v = 0; v < Nv; ++v) asm volatile("prefetch.global.L2 [%0];" ::"l"(E.acc + v * cells + g));
+    if (need_un)
+      for (int v = 0; v < Nv; ++v) asm volatile("prefetch.global.L2 [%0];" ::"l"(E.Un + v * cells + g));
   }
 };
 
@@ -198,6 +204,11 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
     }
     W.write_ok = ok;
     W.gi = gi;
+    if (W.need_acc || W.need_un) {                          // operands of this lane's cell in the NEXT chunk -> L2
+      const long long gnext = gi + (long long)LJ * sst;
+      if (fc == f_begin && ok) W.prefetch_l2(gi, Nv);
+      if (lane_ok && f + LJ <= f_end && gnext < G.cells) W.prefetch_l2(gnext, Nv);
+    }
     W.sm_us = sm + o[2];
     W.carry_rd = carry + par * Nv * LI;
     W.carry_wr = carry + (par ^ 1) * Nv * LI;
@@ -208,6 +219,144 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
     rb += LJ;
     rb -= rb >= RR ? RR : 0;
     par ^= 1;
+  }
+  cp_async_wait<0>();
+  if (bad) atomicOr(status, XF_FLAG_NONPHYSICAL);
+}
+
+
+// ---------------------------------------------------------------------------------------------------------------
+// y / z sweeps: block-cooperative, every global access a full 256-byte row.
+// Block = 32 lanes (consecutive i) x W warps (consecutive faces along the sweep direction).  The stencil rows live in
+// a shared ring of 2 W + 5 rows: while the W face rows of a chunk are computed, the W new rows of the next chunk
+// land through cp.async (warp w fetches one row: 32 consecutive doubles per field).  Face fluxes go to a small
+// shared buffer (row w + 1; row 0 is the last face of the previous chunk); after one barrier every warp updates its
+// row of cells with coalesced loads of the residual / U^n operands (all Nv in flight at once) and coalesced stores.
+// Two barriers per chunk; two blocks per SM overlap one block's update phase with the other's arithmetic.
+// ---------------------------------------------------------------------------------------------------------------
+__host__ __device__ inline size_t yz_smem_doubles(int N, int W) {
+  return (size_t)nstaged(N) * ring_rows(W) * 32 + (size_t)(N + 4) * (W + 1) * 32;
+}
+
+struct FluxStore {
+  double *dst;   // fb + row * 32 + lane
+  int stride;    // doubles between components
+  __device__ __forceinline__ void operator()(int v, double F, int) { dst[v * stride] = F; }
+};
+
+template <int N_T, int DIR, int W>
+__global__ void __launch_bounds__(32 * W, (W <= 4 ? 2 : 1))
+sweep_yz_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const double *__restrict__ prim,
+                const XfEpilogue E, int *__restrict__ status, const int seg_len) {
+  const int N = N_T > 0 ? N_T : Nrt;
+  const int Nv = N + 4, NST = nstaged(N);
+  constexpr int NVS = N_T > 0 ? N_T + 4 : XF_MAXNV;        // static bound of Nv for register arrays
+  constexpr int RR = ring_rows(W);
+  constexpr int FS = RR * 32;                               // ring doubles per field
+  constexpr int FBS = (W + 1) * 32;                         // flux-buffer doubles per component
+  extern __shared__ double smem[];
+  double *sm = smem;
+  double *fb = smem + (size_t)NST * FS;
+
+  const int lane = threadIdx.x, w = threadIdx.y;
+  constexpr int OD = DIR == 1 ? 2 : 1;                      // the other transverse direction
+  const int i = G.g[0] + blockIdx.x * 32 + lane;
+  const int imax = G.g[0] + G.n[0] - 1;
+  const bool lane_ok = i <= imax;
+  const long long colbase = (long long)(blockIdx.y + G.g[OD]) * G.st[OD] + (lane_ok ? i : imax);  // idle lanes: valid data
+  const long long sst = G.st[DIR];
+  const int f_begin = blockIdx.z * seg_len;                 // faces f_begin .. f_end, cells f_begin .. f_end - 1
+  const int f_end = f_begin + seg_len < G.n[DIR] ? f_begin + seg_len : G.n[DIR];
+  const int rmax = G.np[DIR] - 1;
+
+  auto stage_row = [&](int slot, int r) {                   // stencil row r (= padded row r) -> ring slot
+    const long long gi = colbase + (long long)(r < rmax ? r : rmax) * sst;
+    double *dst = sm + slot * 32 + lane;
+    if (N_T > 0) {
+#pragma unroll
+      for (int f = 0; f < nstaged(N_T > 0 ? N_T : 1); ++f)
+        cp_async8(dst + f * FS, (f < Nv ? U + (size_t)f * G.cells : prim + (size_t)(f - Nv) * G.cells) + gi);
+    } else {
+      for (int f = 0; f < NST; ++f)
+        cp_async8(dst + f * FS, (f < Nv ? U + (size_t)f * G.cells : prim + (size_t)(f - Nv) * G.cells) + gi);
+    }
+  };
+
+  // ---- prologue: rows f_begin .. f_begin + W + 4 into ring slots 0 .. W + 4
+  for (int r = w; r < W + 5; r += W) stage_row(r, f_begin + r);
+  cp_async_commit();
+
+  const double dt = E.mode == 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
+  const double ninv = -G.inv_d[DIR];
+  const bool need_acc = E.mode == 1 || (E.mode == 2 && E.has_acc);
+  const bool need_un = E.mode == 2 && E.alpha != 0.0;
+
+  int rb = 0;       // ring slot of stencil row fc
+  bool bad = false;
+  for (int fc = f_begin; fc <= f_end; fc += W) {
+    cp_async_wait<0>();
+    __syncthreads();      // [A] this chunk's rows have landed; every warp is done with the previous chunk
+    if (fc + W <= f_end) {                                  // the W new rows of the next chunk: row fc + W + 5 + w
+      int slot = rb + W + 5 + w;
+      slot -= slot >= RR ? RR : 0;
+      stage_row(slot, fc + W + 5 + w);
+    }
+    cp_async_commit();
+
+    const int f = fc + w;
+    int o[6];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) {
+      int s = rb + w + m;
+      s -= s >= RR ? RR : 0;
+      o[m] = s * 32 + lane;
+    }
+    if (f <= f_end) {                                       // warp-uniform
+      FluxStore st{fb + (w + 1) * 32 + lane, FBS};
+      const bool c2ok = face_flux<DIR>(N, sm, FS, o, st);
+      bad = bad || (!c2ok && lane_ok);
+    }
+    __syncthreads();      // [B] the chunk's fluxes are in fb
+
+    // ---- cell f - 1 (between faces f - 1 and f; staged at stencil row f + 2): Eq. 13 and the stage combination
+    if (f > f_begin && f <= f_end) {                        // warp-uniform
+      const long long gi = colbase + (long long)(f + 2) * sst;
+      double a[NVS], un[NVS];
+      if (need_acc) {
+#pragma unroll
+        for (int v = 0; v < NVS; ++v)
+          if (v < Nv) a[v] = E.acc[v * G.cells + gi];
+      }
+      if (need_un) {
+#pragma unroll
+        for (int v = 0; v < NVS; ++v)
+          if (v < Nv) un[v] = E.Un[v * G.cells + gi];
+      }
+      if (lane_ok) {
+#pragma unroll
+        for (int v = 0; v < NVS; ++v) {
+          if (v < Nv) {
+            const double div = (fb[v * FBS + (w + 1) * 32 + lane] - fb[v * FBS + w * 32 + lane]) * ninv;
+            const long long idx = v * G.cells + gi;
+            if (E.mode == 0) {
+              E.out[idx] = div;
+            } else if (E.mode == 1) {
+              E.out[idx] = a[v] + div;
+            } else {
+              const double L = need_acc ? a[v] + div : div;
+              const double us = sm[v * FS + o[2]];
+              E.out[idx] = need_un ? fma(E.alpha, un[v], E.beta * fma(dt, L, us)) : E.beta * fma(dt, L, us);
+            }
+          }
+        }
+      }
+    }
+    if (w == 0) {                                           // carry the chunk's last face to row 0 (only warp 0 reads row 0)
+      __syncwarp();
+      for (int v = 0; v < Nv; ++v) fb[v * FBS + lane] = fb[v * FBS + W * 32 + lane];
+    }
+    rb += W;
+    rb -= rb >= RR ? RR : 0;
   }
   cp_async_wait<0>();
   if (bad) atomicOr(status, XF_FLAG_NONPHYSICAL);
