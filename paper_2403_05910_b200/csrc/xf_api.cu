@@ -100,7 +100,7 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
   const int nact = count_active(c->G);
   int done = 0;
   for (int dd = 0; dd < 3; ++dd) {
-    const int d = getenv("XF_REV") ? 2 - dd : dd;
+    const int d = dd;
     if (c->G.n[d] == 1) continue;
     XfEpilogue E;
     if (done == nact - 1) {

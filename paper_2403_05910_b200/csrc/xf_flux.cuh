@@ -21,7 +21,15 @@ namespace xf {
 //   result = v2 + (D2 + 2 D3)/6 + [ (2/3) P0 (d0 - d1) + P2 (d1 - d2) ] / [ 2 P0 + 12 P1 + 6 P2 ],
 // with P0 = (s1 s2)^2, P1 = (s0 s2)^2, P2 = (s0 s1)^2, s_k = 4 (eps + beta_k): the Jiang-Shu weights
 // d_k/(eps+beta_k)^2 brought to a common denominator, so one reciprocal instead of four divisions.
-__device__ __forceinline__ double weno5(double v0, double v1, double v2, double v3, double v4) {
+#ifndef XF_SPECIES_UNROLL
+#define XF_SPECIES_UNROLL 1
+#endif
+#define XF_PRAGMA(x) _Pragma(#x)
+#define XF_UNROLL(n) XF_PRAGMA(unroll n)
+
+// the nonlinear part of one reconstruction as a fraction num/den and the linear part `base`
+__device__ __forceinline__ void weno5_parts(double v0, double v1, double v2, double v3, double v4, double &num,
+                                            double &den, double &base) {
   const double D1 = v1 - v0, D2 = v2 - v1, D3 = v3 - v2, D4 = v4 - v3;
   const double d0 = D2 - D1, d1 = D3 - D2, d2 = D4 - D3;
   const double e0 = fma(3.0, D2, -D1);   // v0 - 4 v1 + 3 v2
@@ -33,10 +41,20 @@ __device__ __forceinline__ double weno5(double v0, double v1, double v2, double 
   const double s2 = fma(e2, e2, fma(k133 * d2, d2, eps4));
   const double p12 = s1 * s2, p02 = s0 * s2, p01 = s0 * s1;
   const double P0 = p12 * p12, P1 = p02 * p02, P2 = p01 * p01;
-  const double num = fma(P0 * (d0 - d1), 2.0 / 3.0, P2 * (d1 - d2));
-  const double den = fma(2.0, P0, fma(12.0, P1, 6.0 * P2));
-  const double base = fma(fma(2.0, D3, D2), 1.0 / 6.0, v2);
+  num = fma(P0 * (d0 - d1), 2.0 / 3.0, P2 * (d1 - d2));
+  den = fma(2.0, P0, fma(12.0, P1, 6.0 * P2));
+  base = fma(fma(2.0, D3, D2), 1.0 / 6.0, v2);
+}
+
+__device__ __forceinline__ double weno5(double v0, double v1, double v2, double v3, double v4) {
+  double num, den, base;
+  weno5_parts(v0, v1, v2, v3, v4, num, den, base);
   return fma(num, xf_rcp(den), base);
+}
+
+// g = WENO5(f+ at i-2..i+2) + WENO5(f- at i+3..i-1)  (Eq. 15)
+__device__ __forceinline__ double weno5_pair(const double (&fp)[6], const double (&fm)[6]) {
+  return weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + weno5(fm[5], fm[4], fm[3], fm[2], fm[1]);
 }
 
 template <int DIR> struct Axes;
@@ -53,12 +71,18 @@ __host__ __device__ constexpr int nprimfields(int N) { return N + 4; }
 // the face lies between m = 2 and m = 3).  emit(v, Fhat_v, vnext) is called once per component, in the order
 // 0, 1+nd, 1+t1, 1+t2, 5, ..., Nv-1, 4 (vnext = the component that follows, -1 after the last).
 // Returns false if the Roe-averaged c~^2 is not positive.
+// The fields needed only at the two cells next to the face (Gamma, chi_1..chi_N) are read through a second
+// accessor: field g (0 = Gamma, 1 + s = chi_s) of the cell below / above the face at ss[g*SS + s2] / ss[g*SS + s3],
+// so a sweep may keep them in a shallower ring than the six-deep stencil fields.
 template <int DIR, class Emit>
-__device__ __forceinline__ bool face_flux(const int N, const double *sm, const int FS, const int (&o)[6], Emit &emit) {
+__device__ __forceinline__ bool face_flux(const int N, const double *sm, const int FS, const int (&o)[6],
+                                          const double *ss, const int SS, const int s2, const int s3, Emit &emit) {
   constexpr int nd = Axes<DIR>::nd, t1 = Axes<DIR>::t1, t2 = Axes<DIR>::t2;
   const int Nv = N + 4;
-  const int FP = Nv, FC = Nv + 1, FRI = Nv + 2, FG = Nv + 3, FCHI = Nv + 4;
+  const int FP = Nv, FC = Nv + 1, FRI = Nv + 2;
 #define XS(f, m) sm[(f) * FS + o[m]]
+#define XA(g) ss[(g) * SS + s2]
+#define XB(g) ss[(g) * SS + s3]
 
   // ---- Roe-type average (reading R5): q~ = (w_a q_a + w_b q_b)/(w_a + w_b), w = sqrt(rho); with
   //      r = w_b/w_a = sqrt(rho_b/rho_a) the weights are 1/(1+r) and r/(1+r)
@@ -70,9 +94,9 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const i
 #pragma unroll
   for (int q = 0; q < 3; ++q) ut[q] = fma(oma, XS(1 + q, 2), omb * XS(1 + q, 3));
   const double Ht = fma(oma, XS(4, 2) + XS(FP, 2), omb * (XS(4, 3) + XS(FP, 3)));
-  const double Gt = fma(oa, XS(FG, 2), ob * XS(FG, 3));
+  const double Gt = fma(oa, XA(0), ob * XB(0));
   const double kt = 0.5 * fma(ut[0], ut[0], fma(ut[1], ut[1], ut[2] * ut[2]));
-  const double chiN = fma(oa, XS(FCHI + N - 1, 2), ob * XS(FCHI + N - 1, 3));
+  const double chiN = fma(oa, XA(N), ob * XB(N));
 
   // ---- the dense functional pi.U_m for the six stencil cells; species part first
   double rho[6], piU[6];
@@ -84,7 +108,7 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const i
   double c2acc = 0.0;
 #pragma unroll 3
   for (int i = 0; i < N - 1; ++i) {
-    const double zeta = fma(oa, XS(FCHI + i, 2), ob * XS(FCHI + i, 3)) - chiN;
+    const double zeta = fma(oa, XA(1 + i), ob * XB(1 + i)) - chiN;
     double y[6];
 #pragma unroll
     for (int m = 0; m < 6; ++m) y[m] = XS(5 + i, m);
@@ -128,7 +152,7 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const i
       fp[m] = fma(0.5 * (ud[m] + lam_m), a, pt);
       fm[m] = fma(0.5 * (ud[m] - lam_m), a, pt);
     }
-    g0 = weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + weno5(fm[5], fm[4], fm[3], fm[2], fm[1]);
+    g0 = weno5_pair(fp, fm);
 #pragma unroll
     for (int m = 0; m < 6; ++m) {
       const double a = h * fma(ct, nuU[m], piU[m]);
@@ -136,7 +160,7 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const i
       fp[m] = fma(0.5 * (ud[m] + lam_p), a, pt);
       fm[m] = fma(0.5 * (ud[m] - lam_p), a, pt);
     }
-    gL = weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + weno5(fm[5], fm[4], fm[3], fm[2], fm[1]);
+    gL = weno5_pair(fp, fm);
   }
   double ap[6], am[6];  // (u_m +- Lambda_u)/2 for all fields that travel with u
 #pragma unroll
@@ -153,7 +177,7 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const i
       fp[m] = fma(ap[m], a, pt);
       fm[m] = fma(am[m], a, pt);
     }
-    g1 = weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + weno5(fm[5], fm[4], fm[3], fm[2], fm[1]);
+    g1 = weno5_pair(fp, fm);
   }
 
   // ---- back-projection Fhat = R g (Eq. 15), structured
@@ -176,20 +200,22 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const i
       fp[m] = ap[m] * a;                                                                               \
       fm[m] = am[m] * a;                                                                               \
     }                                                                                                  \
-    const double g = weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + weno5(fm[5], fm[4], fm[3], fm[2], fm[1]); \
+    const double g = weno5_pair(fp, fm);                                                               \
     F4 = fma((DEXPR), g, F4);                                                                          \
     emit(VIDX, fma(C, s, g), VNEXT);                                                                   \
   }
   XF_LINEAR_FIELD(1 + t1, C, 1 + t2)
   XF_LINEAR_FIELD(1 + t2, C, N > 1 ? 5 : 4)
-#pragma unroll 1
+XF_UNROLL(XF_SPECIES_UNROLL)
   for (int i = 0; i < N - 1; ++i) {
-    const double zeta = fma(oa, XS(FCHI + i, 2), ob * XS(FCHI + i, 3)) - chiN;
+    const double zeta = fma(oa, XA(1 + i), ob * XB(1 + i)) - chiN;
     XF_LINEAR_FIELD(5 + i, -zeta * invG, i + 2 < N ? 6 + i : 4)
   }
 #undef XF_LINEAR_FIELD
   emit(4, F4, -1);
 #undef XS
+#undef XA
+#undef XB
   return c2 > 0.0;
 }
 

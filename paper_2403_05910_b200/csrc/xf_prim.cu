@@ -88,52 +88,90 @@ __device__ __forceinline__ double newton_T(const XfThermo &th, int N, const Cell
   return T;
 }
 
+// One evaluation site for the species polynomials: the loop body evaluates sum Y_s h_s, sum Y_s cp_s and e_s/R_s at
+// the current T; a Newton update follows unless the previous update already converged, in which case the values
+// just computed ARE the final ones (C_v, e_s at the converged T, as the problem statement asks: p, Gamma, c, chi_s
+// follow from the final T).  One code copy instead of two keeps the kernel at 128 registers = 16 warps per SM.
 template <int N_T>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(128, 4)
 prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *__restrict__ U, double *__restrict__ T,
             double *__restrict__ prim, double *__restrict__ p_out, double *__restrict__ c_out,
             int *__restrict__ status, unsigned long long *__restrict__ itersum) {
+  constexpr int NS = CellState<N_T>::NS;
   const int N = N_T > 0 ? N_T : th.N;
   const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   int it = 0;
   if (idx < G.cells) {
-    CellState<N_T> S;
-    load_cell<N_T>(G, N, U, idx, S);
-    bool conv;
-    const double Tn = newton_T<N_T>(th, N, S, T[idx], it, conv);
-    // everything that follows from T
-    const double Tc = fmin(fmax(Tn, th.Tlo), th.Thi);
-    double Rbar = 0.0, cpm = 0.0;
-    double esR[CellState<N_T>::NS];
+    const double rho = U[idx];
+    const double rinv = xf_rcp(rho);
+    double k2 = 0.0;
 #pragma unroll
-    for (int s = 0; s < CellState<N_T>::NS; ++s) {
-      if (s < N) {
-        double cpR, hR;
-        species_cp_h(th, s, Tn, Tc, cpR, hR);
-        const double yr = S.Y[s] * th.Rs[s];
-        Rbar += yr;
-        cpm = fma(yr, cpR, cpm);
-        esR[s] = hR - Tn;  // e_s / R_s
+    for (int q = 0; q < 3; ++q) {
+      const double v = U[(1 + q) * G.cells + idx] * rinv;
+      k2 = fma(v, v, k2);
+    }
+    const double e = fma(U[4 * G.cells + idx], rinv, -0.5 * k2);
+    double yr[NS];  // Y_s R_s
+    double sum = 0.0, Rbar = 0.0;
+#pragma unroll
+    for (int i = 0; i < NS - 1; ++i) {
+      if (i < N - 1) {
+        const double Y = U[(5 + i) * G.cells + idx] * rinv;
+        sum += Y;
+        yr[i] = Y * th.Rs[i];
+        Rbar += yr[i];
       }
     }
-    const double Cv = cpm - Rbar;
-    const double pr = S.rho * Rbar * Tn;  // Eq. 7
-    const double Gam = Rbar / Cv;
-    const double cs = sqrt((1.0 + Gam) * pr * S.rinv);
-    T[idx] = Tn;
+#pragma unroll
+    for (int i = 0; i < NS; ++i)
+      if (i == N - 1) {  // closure: no clipping, no renormalisation (reading R12)
+        yr[i] = (1.0 - sum) * th.Rs[i];
+        Rbar += yr[i];
+      }
+    double Tk = T[idx];
+    double esR[NS], cpm;
+    bool fin = false, conv = false;
+#pragma unroll 1
+    for (;;) {
+      const double Tc = fmin(fmax(Tk, th.Tlo), th.Thi);
+      double hm = 0.0;
+      cpm = 0.0;
+#pragma unroll
+      for (int s = 0; s < NS; ++s) {
+        if (s < N) {
+          double cpR, hR;
+          species_cp_h(th, s, Tk, Tc, cpR, hR);
+          hm = fma(yr[s], hR, hm);
+          cpm = fma(yr[s], cpR, cpm);
+          esR[s] = hR - Tk;  // e_s / R_s
+        }
+      }
+      if (fin) break;
+      // Eq. 21: T <- T + (e - e(T)) / C_v(T)
+      const double Tn = fma(e - fma(-Rbar, Tk, hm), xf_rcp(cpm - Rbar), Tk);
+      ++it;
+      conv = fabs(Tn - Tk) <= th.rtol * fabs(Tn);
+      fin = conv || it >= th.maxit || !(Tn == Tn);
+      Tk = Tn;
+    }
+    const double iCv = xf_rcp(cpm - Rbar);
+    const double pr = rho * Rbar * Tk;  // Eq. 7
+    const double Gam = Rbar * iCv;
+    const double cs = sqrt((1.0 + Gam) * pr * rinv);
+    T[idx] = Tk;
     if (p_out) p_out[idx] = pr;
     if (c_out) c_out[idx] = cs;
     if (prim) {  // what the sweeps stage per cell: p, c, 1/rho, Gamma, chi_s
       prim[idx] = pr;
       prim[G.cells + idx] = cs;
-      prim[2 * G.cells + idx] = xf_rcp(S.rho);
+      prim[2 * G.cells + idx] = rinv;
       prim[3 * G.cells + idx] = Gam;
 #pragma unroll
-      for (int s = 0; s < CellState<N_T>::NS; ++s)
-        if (s < N) prim[(4 + s) * G.cells + idx] = th.Rs[s] * fma(-Gam, esR[s], Tn);  // chi_s = R_s T - Gamma e_s
+      for (int s = 0; s < NS; ++s)
+        if (s < N) prim[(4 + s) * G.cells + idx] = th.Rs[s] * fma(-Gam, esR[s], Tk);  // chi_s = R_s T - Gamma e_s
     }
     int flag = 0;
-    if (!(S.rho > 0.0) || !(Tn > 0.0) || !(pr > 0.0)) flag |= XF_FLAG_NONPHYSICAL;
+    if (!(rho > 0.0) || !(Tk > 0.0) || !(pr > 0.0)) flag |= XF_FLAG_NONPHYSICAL;
     if (!conv) flag |= XF_FLAG_NOCONV;
     if (flag) atomicOr(status, flag);
   }
@@ -217,7 +255,7 @@ wavespeed_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const doub
 
 int xf_launch_prim(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *prim, double *p,
                    double *c, int *status, unsigned long long *itersum, cudaStream_t s) {
-  const int threads = 256;
+  const int threads = 128;
   const unsigned blocks = (unsigned)((G.cells + threads - 1) / threads);
 #define CALL(NT) prim_kernel<NT><<<blocks, threads, 0, s>>>(G, Th, U, T, prim, p, c, status, itersum)
   XF_DISPATCH_N(Th.N, CALL)

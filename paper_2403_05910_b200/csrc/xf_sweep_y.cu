@@ -1,10 +1,12 @@
 // xf_sweep_y.cu -- instantiations and launcher of the y-direction sweep (see xf_sweeps.cuh).
 #include "xf_sweeps.cuh"
 
-int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
-                      cudaStream_t s) {
+namespace {
+constexpr int DIR = 1, OD = DIR == 1 ? 2 : 1;
+
+template <int NT>
+int launch(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status, cudaStream_t s) {
   using namespace xf;
-  constexpr int DIR = 1, OD = DIR == 1 ? 2 : 1;
   const int strips = (G.n[0] + 31) / 32;
   // one block marches a whole column unless the grid alone cannot fill 148 SMs x 2 blocks a few times over;
   // each split costs one extra face row
@@ -13,20 +15,27 @@ int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *pri
   while ((long long)strips * G.n[OD] * nseg < 1184 && n / (nseg * 2) >= 4 * YZ_W) nseg *= 2;
   const int seg_len = (n + nseg - 1) / nseg;
   nseg = (n + seg_len - 1) / seg_len;
-  const dim3 grid(strips, G.n[OD], nseg), block(32, YZ_W);
+  const dim3 grid(strips, G.n[OD], nseg), block(32, 2 * YZ_W);
   const size_t smem = sizeof(double) * yz_smem_doubles(N, YZ_W);
-#define CALL(NT) sweep_yz_kernel<NT, DIR, YZ_W><<<grid, block, smem, s>>>(G, N, U, prim, E, status, seg_len)
+  sweep_yz_ws_kernel<NT, DIR, YZ_W><<<grid, block, smem, s>>>(G, N, U, prim, E, status, seg_len);
+  return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
+}
+}  // namespace
+
+int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
+                      cudaStream_t s) {
+#define CALL(NT) return launch<NT>(G, N, U, prim, E, status, s)
   XF_DISPATCH_SWEEP_N(N, CALL)
 #undef CALL
-  return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
+  return XF_EINVAL;
 }
 
 int xf_sweep_y_init() {
   using namespace xf;
   cudaError_t e = cudaSuccess;
-#define CALL(NT)                                                                                          \
-  e = cudaFuncSetAttribute(sweep_yz_kernel<NT, 1, YZ_W>, cudaFuncAttributeMaxDynamicSharedMemorySize,    \
-                           (int)(sizeof(double) * yz_smem_doubles(NT > 0 ? NT : XF_MAXN, YZ_W)));         \
+#define CALL(NT)                                                                                             \
+  e = cudaFuncSetAttribute(sweep_yz_ws_kernel<NT, DIR, YZ_W>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
+                           (int)(sizeof(double) * yz_smem_doubles(NT > 0 ? NT : XF_MAXN, YZ_W)));            \
   if (e != cudaSuccess) return XF_ECUDA;
   CALL(0) CALL(1) CALL(2) CALL(3) CALL(4) CALL(10)
 #undef CALL

@@ -19,11 +19,12 @@
 namespace xf {
 
 constexpr int X_LI = 1, X_LJ = 32, X_NCH = 16;   // x sweep: segment = X_NCH chunks = 32*X_NCH faces, 32*X_NCH - 1 cells
+constexpr int X_RR = X_LJ + 5, X_MINB = 12;       // ring of exactly one chunk, 12 warps per SM (measured best, profiles/)
 constexpr int YZ_W = 4;                           // y/z sweeps: warps per block = face rows per chunk
 
 __host__ __device__ constexpr int ring_rows(int LJ) { return 2 * LJ + 5; }
-__host__ __device__ inline size_t warp_smem_doubles(int N, int LI, int LJ) {
-  return (size_t)nstaged(N) * ring_rows(LJ) * LI + 2 * (size_t)(N + 4) * LI;
+__host__ __device__ inline size_t warp_smem_doubles(int N, int LI, int RR) {
+  return (size_t)nstaged(N) * RR * LI + 2 * (size_t)(N + 4) * LI;
 }
 
 __device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc) {
@@ -85,14 +86,15 @@ struct CellWriter {
 
 // One warp = one segment of one pencil group.  DIR = 0: blockIdx.x enumerates (k-plane, segment of the flat pencil).
 // DIR = 1, 2: blockIdx = (group of LI pencils along i, index along the other transverse direction, segment).
-template <int N_T, int DIR, int LI, int LJ>
-__global__ void __launch_bounds__(32, 12)
+template <int N_T, int DIR, int LI, int LJ, int RR, int MINB>
+__global__ void __launch_bounds__(32, MINB)
 sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const double *__restrict__ prim,
              const XfEpilogue E, int *__restrict__ status, const int seg_param) {
   static_assert(LI * LJ == 32, "one lane per face");
   const int N = N_T > 0 ? N_T : Nrt;
   const int Nv = N + 4, NST = nstaged(N);
-  constexpr int RR = ring_rows(LJ);
+  static_assert(RR >= LJ + 5 && RR <= 2 * LJ + 5, "ring: one chunk plus 0..LJ rows of prefetch");
+  constexpr int PF = RR - (LJ + 5);                         // rows of the next chunk that land during the arithmetic
   constexpr int FS = RR * LI;
   extern __shared__ double smem[];
   double *sm = smem;
@@ -173,8 +175,8 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
   int par = 0;
   bool bad = false;
   for (int fc = f_begin; fc <= f_end; fc += LJ) {
-    // ---- prefetch the LJ new rows of the next chunk: rows fc + LJ + 5 + lj
-    if (fc + LJ <= f_end) {
+    // ---- prefetch the first PF new rows of the next chunk (rows fc + LJ + 5 + lj) into the free part of the ring
+    if (PF > 0 && lj < PF && fc + LJ <= f_end) {
       int slot = rb + LJ + 5 + lj;
       slot -= slot >= RR ? RR : 0;
       stage(slot * LI + li, row_addr(fc + LJ + 5 + lj, li));
@@ -213,9 +215,18 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
     W.carry_rd = carry + par * Nv * LI;
     W.carry_wr = carry + (par ^ 1) * Nv * LI;
     W.preload(0);
-    const bool c2ok = face_flux<DIR>(N, sm, FS, o, W);
+    const bool c2ok = face_flux<DIR>(N, sm, FS, o, sm + (Nv + 3) * FS, FS, o[2], o[3], W);
     bad = bad || (!c2ok && lane_ok && f <= f_end);
     __syncwarp();         // all lanes are done with the rows the next iteration's prefetch overwrites
+    if (PF < LJ) {        // the remaining LJ - PF rows of the next chunk go where this chunk's first rows were
+      if (lj >= PF && fc + LJ <= f_end) {
+        int slot = rb + LJ + 5 + lj;
+        slot -= slot >= RR ? RR : 0;
+        slot -= slot >= RR ? RR : 0;
+        stage(slot * LI + li, row_addr(fc + LJ + 5 + lj, li));
+      }
+      cp_async_commit();
+    }
     rb += LJ;
     rb -= rb >= RR ? RR : 0;
     par ^= 1;
@@ -227,38 +238,66 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
 
 // ---------------------------------------------------------------------------------------------------------------
 // y / z sweeps: block-cooperative, every global access a full 256-byte row.
-// Block = 32 lanes (consecutive i) x W warps (consecutive faces along the sweep direction).  The stencil rows live in
-// a shared ring of 2 W + 5 rows: while the W face rows of a chunk are computed, the W new rows of the next chunk
-// land through cp.async (warp w fetches one row: 32 consecutive doubles per field).  Face fluxes go to a small
-// shared buffer (row w + 1; row 0 is the last face of the previous chunk); after one barrier every warp updates its
-// row of cells with coalesced loads of the residual / U^n operands (all Nv in flight at once) and coalesced stores.
-// Two barriers per chunk; two blocks per SM overlap one block's update phase with the other's arithmetic.
+// Block = 32 lanes (consecutive i) x W face rows along the sweep direction.  The stencil rows live in a shared ring
+// of 2 W + 5 rows: while the W face rows of a chunk are computed, the W new rows of the next chunk land through
+// cp.async (one row per warp: 32 consecutive doubles per field).  Face fluxes go to a small shared buffer (row w + 1;
+// row 0 is the last face of the previous chunk) and are differenced from there.
 // ---------------------------------------------------------------------------------------------------------------
 __host__ __device__ inline size_t yz_smem_doubles(int N, int W) {
   return (size_t)nstaged(N) * ring_rows(W) * 32 + (size_t)(N + 4) * (W + 1) * 32;
 }
 
-struct FluxStore {
+// ---------------------------------------------------------------------------------------------------------------
+// Warp-specialised.  Measured on config 4 (profiles/): with every warp doing staging, arithmetic and the cell
+// update in turn, a quarter of the warp time sits in the update
+// (global operands, stores) and in issuing copies, and while one of the SM's two blocks is there the fp64 pipe is
+// fed by a single warp per scheduler.  Here a block is two warp groups:
+//   * W COMPUTE warps (warp w = face row fc + w) run xf::face_flux back to back and nothing else;
+//   * W SERVICE warps keep the ring one chunk ahead (cp.async) and, concurrently with the next chunk's arithmetic,
+//     difference the fluxes of the chunk just finished and write the cells (Eq. 13, Eq. 16).
+// setmaxnreg moves registers from the service group (72) to the compute group (184): two blocks per SM.
+// Named barriers (ids alternate with the chunk parity): RING_FULL  service -> compute  rows of chunk c landed
+//                                                        FLUX_READY compute -> service  fluxes of chunk c in fb
+//                                                        FB_EMPTY   service -> compute  fb of chunk c - 1 consumed
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void named_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ void named_arrive(int id, int nthreads) {
+  asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+constexpr int BAR_RING_FULL = 1, BAR_FLUX_READY = 3, BAR_FB_EMPTY = 5;   // + chunk parity
+constexpr int WS_REGS_COMPUTE = 184, WS_REGS_SERVICE = 72;
+
+struct FluxStoreWS {
   double *dst;   // fb + row * 32 + lane
   int stride;    // doubles between components
-  __device__ __forceinline__ void operator()(int v, double F, int) { dst[v * stride] = F; }
+  int wait_id;   // named barrier to pass before the first component is written (-1: none)
+  int nthreads;
+  __device__ __forceinline__ void operator()(int v, double F, int) {
+    if (v == 0 && wait_id >= 0) named_sync(wait_id, nthreads);
+    dst[v * stride] = F;
+  }
 };
 
 template <int N_T, int DIR, int W>
-__global__ void __launch_bounds__(32 * W, (W <= 4 ? 2 : 1))
-sweep_yz_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const double *__restrict__ prim,
-                const XfEpilogue E, int *__restrict__ status, const int seg_len) {
+__global__ void __launch_bounds__(64 * W, 2)
+sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const double *__restrict__ prim,
+                   const XfEpilogue E, int *__restrict__ status, const int seg_len) {
   const int N = N_T > 0 ? N_T : Nrt;
   const int Nv = N + 4, NST = nstaged(N);
   constexpr int NVS = N_T > 0 ? N_T + 4 : XF_MAXNV;        // static bound of Nv for register arrays
   constexpr int RR = ring_rows(W);
   constexpr int FS = RR * 32;                               // ring doubles per field
   constexpr int FBS = (W + 1) * 32;                         // flux-buffer doubles per component
+  constexpr int NT = 64 * W;                                // threads that take part in every named barrier
   extern __shared__ double smem[];
   double *sm = smem;
   double *fb = smem + (size_t)NST * FS;
 
-  const int lane = threadIdx.x, w = threadIdx.y;
+  const int lane = threadIdx.x;
+  const bool service = threadIdx.y >= W;
+  const int w = service ? threadIdx.y - W : threadIdx.y;    // face row within the chunk / ring row staged
   constexpr int OD = DIR == 1 ? 2 : 1;                      // the other transverse direction
   const int i = G.g[0] + blockIdx.x * 32 + lane;
   const int imax = G.g[0] + G.n[0] - 1;
@@ -267,18 +306,104 @@ sweep_yz_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, con
   const long long sst = G.st[DIR];
   const int f_begin = blockIdx.z * seg_len;                 // faces f_begin .. f_end, cells f_begin .. f_end - 1
   const int f_end = f_begin + seg_len < G.n[DIR] ? f_begin + seg_len : G.n[DIR];
-  const int rmax = G.np[DIR] - 1;
 
+  if (!service) {
+    // =========================================================== compute warps
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(WS_REGS_COMPUTE));
+    int rb = 0, par = 0;
+    bool bad = false, first = true;
+    for (int fc = f_begin; fc <= f_end; fc += W) {
+      named_sync(BAR_RING_FULL + par, NT);                  // rows fc .. fc + W + 4 are in the ring
+      const int f = fc + w;
+      int o[6];
+#pragma unroll
+      for (int m = 0; m < 6; ++m) {
+        int sl = rb + w + m;
+        sl -= sl >= RR ? RR : 0;
+        o[m] = sl * 32 + lane;
+      }
+      if (f <= f_end) {                                     // warp-uniform
+        FluxStoreWS st{fb + (w + 1) * 32 + lane, FBS, first ? -1 : BAR_FB_EMPTY + par, NT};
+        const bool c2ok = face_flux<DIR>(N, sm, FS, o, sm + (Nv + 3) * FS, FS, o[2], o[3], st);
+        bad = bad || (!c2ok && lane_ok);
+      } else if (!first) {
+        named_sync(BAR_FB_EMPTY + par, NT);                 // keep the barrier counts whole
+      }
+      named_arrive(BAR_FLUX_READY + par, NT);
+      rb += W;
+      rb -= rb >= RR ? RR : 0;
+      par ^= 1;
+      first = false;
+    }
+    if (bad) atomicOr(status, XF_FLAG_NONPHYSICAL);
+    return;
+  }
+
+  // ============================================================= service warps
+  asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(WS_REGS_SERVICE));
+  const int rmax = G.np[DIR] - 1;
   auto stage_row = [&](int slot, int r) {                   // stencil row r (= padded row r) -> ring slot
     const long long gi = colbase + (long long)(r < rmax ? r : rmax) * sst;
     double *dst = sm + slot * 32 + lane;
-    if (N_T > 0) {
+#pragma unroll 4
+    for (int f = 0; f < NST; ++f)
+      cp_async8(dst + f * FS, (f < Nv ? U + (size_t)f * G.cells : prim + (size_t)(f - Nv) * G.cells) + gi);
+  };
+  const double dt = E.mode == 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
+  const double ninv = -G.inv_d[DIR];
+  const bool need_acc = E.mode == 1 || (E.mode == 2 && E.has_acc);
+  const bool need_un = E.mode == 2 && E.alpha != 0.0;
+
+  // cell row of face f (cell f - 1, staged at stencil row f + 2): Eq. 13 and the stage combination
+  double d[NVS];
+  auto read_fluxes = [&]() {                                // part 1: everything the update needs from fb
 #pragma unroll
-      for (int f = 0; f < nstaged(N_T > 0 ? N_T : 1); ++f)
-        cp_async8(dst + f * FS, (f < Nv ? U + (size_t)f * G.cells : prim + (size_t)(f - Nv) * G.cells) + gi);
-    } else {
-      for (int f = 0; f < NST; ++f)
-        cp_async8(dst + f * FS, (f < Nv ? U + (size_t)f * G.cells : prim + (size_t)(f - Nv) * G.cells) + gi);
+    for (int v = 0; v < NVS; ++v)
+      if (v < Nv) d[v] = (fb[v * FBS + (w + 1) * 32 + lane] - fb[v * FBS + w * 32 + lane]) * ninv;
+    if (w == 0) {                                           // carry the chunk's last face to row 0 (only warp 0 reads row 0)
+      for (int v = 0; v < Nv; ++v) fb[v * FBS + lane] = fb[v * FBS + W * 32 + lane];
+    }
+  };
+  auto prefetch_operands = [&](int f) {                     // the update's global operands of cell row f -> L2
+    if (!(f > f_begin && f <= f_end) || (lane & 15) != 0) return;
+    const long long gi = colbase + (long long)(f + 2) * sst;
+    for (int v = 0; v < Nv; ++v) {
+      if (need_acc) asm volatile("prefetch.global.L2 [%0];" ::"l"(E.acc + v * G.cells + gi));
+      if (need_un) asm volatile("prefetch.global.L2 [%0];" ::"l"(E.Un + v * G.cells + gi));
+    }
+  };
+  auto write_cells = [&](int f) {                           // part 2: global operands, Eq. 16, stores
+    if (!(f > f_begin && f <= f_end) || !lane_ok) return;
+    const long long gi = colbase + (long long)(f + 2) * sst;
+    constexpr int VB = 4;                                   // fields per batch: all loads of a batch fly together
+#pragma unroll
+    for (int v0 = 0; v0 < NVS; v0 += VB) {
+      double a[VB], un[VB], us[VB];
+#pragma unroll
+      for (int q = 0; q < VB; ++q) {
+        const int v = v0 + q;
+        if (v < Nv && v < NVS) {
+          const long long idx = v * G.cells + gi;
+          a[q] = need_acc ? E.acc[idx] : 0.0;
+          un[q] = need_un ? E.Un[idx] : 0.0;
+          us[q] = E.mode == 2 ? U[idx] : 0.0;
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < VB; ++q) {
+        const int v = v0 + q;
+        if (v < Nv && v < NVS) {
+          const long long idx = v * G.cells + gi;
+          if (E.mode == 0) {
+            E.out[idx] = d[v];
+          } else if (E.mode == 1) {
+            E.out[idx] = a[q] + d[v];
+          } else {
+            const double L = need_acc ? a[q] + d[v] : d[v];
+            E.out[idx] = need_un ? fma(E.alpha, un[q], E.beta * fma(dt, L, us[q])) : E.beta * fma(dt, L, us[q]);
+          }
+        }
+      }
     }
   };
 
@@ -286,80 +411,34 @@ sweep_yz_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, con
   for (int r = w; r < W + 5; r += W) stage_row(r, f_begin + r);
   cp_async_commit();
 
-  const double dt = E.mode == 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
-  const double ninv = -G.inv_d[DIR];
-  const bool need_acc = E.mode == 1 || (E.mode == 2 && E.has_acc);
-  const bool need_un = E.mode == 2 && E.alpha != 0.0;
-
-  int rb = 0;       // ring slot of stencil row fc
-  bool bad = false;
+  int rb = 0, par = 0;
+  bool first = true;
+  int fprev = 0;
   for (int fc = f_begin; fc <= f_end; fc += W) {
     cp_async_wait<0>();
-    __syncthreads();      // [A] this chunk's rows have landed; every warp is done with the previous chunk
+    named_arrive(BAR_RING_FULL + par, NT);                  // this chunk's rows have landed
+    if (!first) {
+      named_sync(BAR_FLUX_READY + (par ^ 1), NT);           // the previous chunk's fluxes are in fb, its ring rows are dead
+      read_fluxes();
+      named_arrive(BAR_FB_EMPTY + par, NT);
+    }
     if (fc + W <= f_end) {                                  // the W new rows of the next chunk: row fc + W + 5 + w
       int slot = rb + W + 5 + w;
       slot -= slot >= RR ? RR : 0;
       stage_row(slot, fc + W + 5 + w);
     }
     cp_async_commit();
-
-    const int f = fc + w;
-    int o[6];
-#pragma unroll
-    for (int m = 0; m < 6; ++m) {
-      int s = rb + w + m;
-      s -= s >= RR ? RR : 0;
-      o[m] = s * 32 + lane;
-    }
-    if (f <= f_end) {                                       // warp-uniform
-      FluxStore st{fb + (w + 1) * 32 + lane, FBS};
-      const bool c2ok = face_flux<DIR>(N, sm, FS, o, st);
-      bad = bad || (!c2ok && lane_ok);
-    }
-    __syncthreads();      // [B] the chunk's fluxes are in fb
-
-    // ---- cell f - 1 (between faces f - 1 and f; staged at stencil row f + 2): Eq. 13 and the stage combination
-    if (f > f_begin && f <= f_end) {                        // warp-uniform
-      const long long gi = colbase + (long long)(f + 2) * sst;
-      double a[NVS], un[NVS];
-      if (need_acc) {
-#pragma unroll
-        for (int v = 0; v < NVS; ++v)
-          if (v < Nv) a[v] = E.acc[v * G.cells + gi];
-      }
-      if (need_un) {
-#pragma unroll
-        for (int v = 0; v < NVS; ++v)
-          if (v < Nv) un[v] = E.Un[v * G.cells + gi];
-      }
-      if (lane_ok) {
-#pragma unroll
-        for (int v = 0; v < NVS; ++v) {
-          if (v < Nv) {
-            const double div = (fb[v * FBS + (w + 1) * 32 + lane] - fb[v * FBS + w * 32 + lane]) * ninv;
-            const long long idx = v * G.cells + gi;
-            if (E.mode == 0) {
-              E.out[idx] = div;
-            } else if (E.mode == 1) {
-              E.out[idx] = a[v] + div;
-            } else {
-              const double L = need_acc ? a[v] + div : div;
-              const double us = sm[v * FS + o[2]];
-              E.out[idx] = need_un ? fma(E.alpha, un[v], E.beta * fma(dt, L, us)) : E.beta * fma(dt, L, us);
-            }
-          }
-        }
-      }
-    }
-    if (w == 0) {                                           // carry the chunk's last face to row 0 (only warp 0 reads row 0)
-      __syncwarp();
-      for (int v = 0; v < Nv; ++v) fb[v * FBS + lane] = fb[v * FBS + W * 32 + lane];
-    }
+    prefetch_operands(fc + w);                              // read one chunk later
+    if (!first) write_cells(fprev);
+    fprev = fc + w;
     rb += W;
     rb -= rb >= RR ? RR : 0;
+    par ^= 1;
+    first = false;
   }
-  cp_async_wait<0>();
-  if (bad) atomicOr(status, XF_FLAG_NONPHYSICAL);
+  named_sync(BAR_FLUX_READY + (par ^ 1), NT);               // the last chunk
+  read_fluxes();
+  write_cells(fprev);
 }
 
 }  // namespace xf
