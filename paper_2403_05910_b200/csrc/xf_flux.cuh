@@ -74,26 +74,31 @@ __host__ __device__ constexpr int nprimfields(int N) { return N + 4; }
 // The fields needed only at the two cells next to the face (Gamma, chi_1..chi_N) are read through a second
 // accessor: field g (0 = Gamma, 1 + s = chi_s) of the cell below / above the face at ss[g*SS + s2] / ss[g*SS + s3],
 // so a sweep may keep them in a shallower ring than the six-deep stencil fields.
+// p, c, 1/rho (six-deep like U) are read through their own base pointer sp (field g at sp[g*FS + o[m]]) so that a
+// sweep may place them in a separately aligned box of the same ring row.
 template <int DIR, class Emit>
-__device__ __forceinline__ bool face_flux(const int N, const double *sm, const int FS, const int (&o)[6],
-                                          const double *ss, const int SS, const int s2, const int s3, Emit &emit) {
+__device__ __forceinline__ bool face_flux(const int N, const double *sm, const double *sp, const int FS,
+                                          const int (&o)[6], const double *ss, const int SS, const int s2,
+                                          const int s3, Emit &emit) {
   constexpr int nd = Axes<DIR>::nd, t1 = Axes<DIR>::t1, t2 = Axes<DIR>::t2;
-  const int Nv = N + 4;
-  const int FP = Nv, FC = Nv + 1, FRI = Nv + 2;
+  
 #define XS(f, m) sm[(f) * FS + o[m]]
+#define XP(m) sp[o[m]]
+#define XC(m) sp[FS + o[m]]
+#define XRI(m) sp[2 * FS + o[m]]
 #define XA(g) ss[(g) * SS + s2]
 #define XB(g) ss[(g) * SS + s3]
 
   // ---- Roe-type average (reading R5): q~ = (w_a q_a + w_b q_b)/(w_a + w_b), w = sqrt(rho); with
   //      r = w_b/w_a = sqrt(rho_b/rho_a) the weights are 1/(1+r) and r/(1+r)
-  const double ria = XS(FRI, 2), rib = XS(FRI, 3);
+  const double ria = XRI(2), rib = XRI(3);
   const double r = sqrt(XS(0, 3) * ria);
   const double oa = xf_rcp(1.0 + r), ob = r * oa;
   const double oma = oa * ria, omb = ob * rib;                // weights acting on conserved quantities
   double ut[3];
 #pragma unroll
   for (int q = 0; q < 3; ++q) ut[q] = fma(oma, XS(1 + q, 2), omb * XS(1 + q, 3));
-  const double Ht = fma(oma, XS(4, 2) + XS(FP, 2), omb * (XS(4, 3) + XS(FP, 3)));
+  const double Ht = fma(oma, XS(4, 2) + XP(2), omb * (XS(4, 3) + XP(3)));
   const double Gt = fma(oa, XA(0), ob * XB(0));
   const double kt = 0.5 * fma(ut[0], ut[0], fma(ut[1], ut[1], ut[2] * ut[2]));
   const double chiN = fma(oa, XA(N), ob * XB(N));
@@ -131,12 +136,12 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const i
     const double mdot = fma(ut[nd], mn, fma(ut[t1], XS(1 + t1, m), ut[t2] * XS(1 + t2, m)));
     piU[m] += fma(Prho, rho[m], Gt * (XS(4, m) - mdot));
     nuU[m] = fma(-ut[nd], rho[m], mn);
-    ud[m] = mn * XS(FRI, m);
-    const double cm = XS(FC, m);
+    ud[m] = mn * XRI(m);
+    const double cm = XC(m);
     lam_m = fmax(lam_m, fabs(ud[m] - cm));
     lam_0 = fmax(lam_0, fabs(ud[m]));
     lam_p = fmax(lam_p, fabs(ud[m] + cm));
-    const double ph = 0.5 * XS(FP, m) * h;             // p_m / (4 c~^2)
+    const double ph = 0.5 * XP(m) * h;             // p_m / (4 c~^2)
     qp[m] = Gt * (ud[m] - ut[nd]) * ph;                // pressure terms of L F_m
     rp[m] = ct * ph;
   }
@@ -215,6 +220,9 @@ XF_UNROLL(XF_SPECIES_UNROLL)
   emit(4, F4, -1);
 #undef XS
 #undef XA
+#undef XP
+#undef XC
+#undef XRI
 #undef XB
   return c2 > 0.0;
 }

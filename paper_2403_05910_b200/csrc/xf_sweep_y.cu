@@ -1,4 +1,6 @@
 // xf_sweep_y.cu -- instantiations and launcher of the y-direction sweep (see xf_sweeps.cuh).
+#include <stdlib.h>
+
 #include "xf_sweeps.cuh"
 
 namespace {
@@ -17,7 +19,13 @@ int launch(const XfGrid &G, int N, const double *U, const double *prim, const Xf
   nseg = (n + seg_len - 1) / seg_len;
   const dim3 grid(strips, G.n[OD], nseg), block(32, 2 * YZ_W);
   const size_t smem = sizeof(double) * yz_smem_doubles(N, YZ_W);
-  sweep_yz_ws_kernel<NT, DIR, YZ_W><<<grid, block, smem, s>>>(G, N, U, prim, E, status, seg_len);
+  CUtensorMap tmU, tmP, tmS;   // U [N + 4]; p, c, 1/rho [3]; Gamma, chi_s [N + 1]
+  static const bool no_tma = getenv("XF_NO_TMA") != nullptr;
+  if (!no_tma && G.g[0] == XF_NG && xf_row_tensor_map(&tmU, G, U, N + 4) && xf_row_tensor_map(&tmP, G, prim, 3) &&
+      xf_row_tensor_map(&tmS, G, prim + 3 * G.cells, N + 1))
+    sweep_yz_ws_kernel<NT, DIR, YZ_W, true><<<grid, block, smem, s>>>(G, N, U, prim, E, status, seg_len, tmU, tmP, tmS);
+  else
+    sweep_yz_ws_kernel<NT, DIR, YZ_W, false><<<grid, block, smem, s>>>(G, N, U, prim, E, status, seg_len, tmU, tmP, tmS);
   return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
 }
 }  // namespace
@@ -34,7 +42,10 @@ int xf_sweep_y_init() {
   using namespace xf;
   cudaError_t e = cudaSuccess;
 #define CALL(NT)                                                                                             \
-  e = cudaFuncSetAttribute(sweep_yz_ws_kernel<NT, DIR, YZ_W>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
+  e = cudaFuncSetAttribute(sweep_yz_ws_kernel<NT, DIR, YZ_W, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
+                           (int)(sizeof(double) * yz_smem_doubles(NT > 0 ? NT : XF_MAXN, YZ_W)));            \
+  if (e != cudaSuccess) return XF_ECUDA;                                                                     \
+  e = cudaFuncSetAttribute(sweep_yz_ws_kernel<NT, DIR, YZ_W, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
                            (int)(sizeof(double) * yz_smem_doubles(NT > 0 ? NT : XF_MAXN, YZ_W)));            \
   if (e != cudaSuccess) return XF_ECUDA;
   CALL(0) CALL(1) CALL(2) CALL(3) CALL(4) CALL(10)

@@ -14,6 +14,8 @@
 // stencil is rows f .. f+5; the lane that owns face f updates cell f-1 from its own flux and that of face f-1
 // (the lane LI below it, or the carry left in shared memory by the previous chunk).
 #pragma once
+#include <cuda.h>
+
 #include "xf_flux.cuh"
 
 namespace xf {
@@ -215,7 +217,7 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
     W.carry_rd = carry + par * Nv * LI;
     W.carry_wr = carry + (par ^ 1) * Nv * LI;
     W.preload(0);
-    const bool c2ok = face_flux<DIR>(N, sm, FS, o, sm + (Nv + 3) * FS, FS, o[2], o[3], W);
+    const bool c2ok = face_flux<DIR>(N, sm, sm + Nv * FS, FS, o, sm + (Nv + 3) * FS, FS, o[2], o[3], W);
     bad = bad || (!c2ok && lane_ok && f <= f_end);
     __syncwarp();         // all lanes are done with the rows the next iteration's prefetch overwrites
     if (PF < LJ) {        // the remaining LJ - PF rows of the next chunk go where this chunk's first rows were
@@ -243,8 +245,19 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
 // cp.async (one row per warp: 32 consecutive doubles per field).  Face fluxes go to a small shared buffer (row w + 1;
 // row 0 is the last face of the previous chunk) and are differenced from there.
 // ---------------------------------------------------------------------------------------------------------------
-__host__ __device__ inline size_t yz_smem_doubles(int N, int W) {
-  return (size_t)nstaged(N) * ring_rows(W) * 32 + (size_t)(N + 4) * (W + 1) * 32;
+// TMA layout (doubles).  A box must start 16-byte aligned in global memory and 128-byte aligned in shared memory
+// (measured: anything else raises "illegal instruction" / "misaligned address"), and the interior starts at the odd
+// index 3, so a row is fetched as 34 doubles from i0 - 1: lane l reads element l + 1.  One ring row = the U box
+// [Nv][34] and the p, c, 1/rho box [3][34], each padded to 128 bytes; Gamma and chi_s (needed only at the two cells
+// next to a face) live in a second, shallower ring of [N + 1][34] boxes.
+constexpr int TMA_RW = 34;
+__host__ __device__ constexpr int tma_box_doubles(int nf) { return (nf * TMA_RW * 8 + 127) / 128 * 16; }
+__host__ __device__ constexpr int tma_deep_slot(int N) { return tma_box_doubles(N + 4) + tma_box_doubles(3); }
+__host__ __device__ constexpr int tma_shallow_slot(int N) { return tma_box_doubles(N + 1); }
+__host__ __device__ inline size_t yz_smem_doubles(int N, int W) {   // ring(s), flux buffer, two mbarriers
+  const size_t plain = (size_t)nstaged(N) * ring_rows(W) * 32;
+  const size_t tma = (size_t)ring_rows(W) * tma_deep_slot(N) + (size_t)(2 * W + 1) * tma_shallow_slot(N);
+  return (plain > tma ? plain : tma) + (size_t)(N + 4) * (W + 1) * 32 + 2;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -266,6 +279,32 @@ __device__ __forceinline__ void named_sync(int id, int nthreads) {
 __device__ __forceinline__ void named_arrive(int id, int nthreads) {
   asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
+// mbarrier / TMA (cp.async.bulk.tensor) primitives of the ring's producer side
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "XF_MBAR_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra XF_MBAR_DONE;\n"
+      "bra XF_MBAR_WAIT;\n"
+      "XF_MBAR_DONE:\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// one box {32 cells along i} x {nf fields} of row (c1, c2) -> dst, completion counted in bytes on `bar`
+__device__ __forceinline__ void tma_load_row(unsigned dst, const void *tmap, int c0, int c1, int c2, unsigned bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(dst),
+      "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(0), "r"(bar)
+      : "memory");
+}
+
 constexpr int BAR_RING_FULL = 1, BAR_FLUX_READY = 3, BAR_FB_EMPTY = 5;   // + chunk parity
 constexpr int WS_REGS_COMPUTE = 184, WS_REGS_SERVICE = 72;
 
@@ -280,20 +319,37 @@ struct FluxStoreWS {
   }
 };
 
-template <int N_T, int DIR, int W>
+template <int N_T, int DIR, int W, bool TMA>
 __global__ void __launch_bounds__(64 * W, 2)
 sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const double *__restrict__ prim,
-                   const XfEpilogue E, int *__restrict__ status, const int seg_len) {
+                   const XfEpilogue E, int *__restrict__ status, const int seg_len,
+                   const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmP,
+                   const __grid_constant__ CUtensorMap tmS) {
   const int N = N_T > 0 ? N_T : Nrt;
   const int Nv = N + 4, NST = nstaged(N);
   constexpr int NVS = N_T > 0 ? N_T + 4 : XF_MAXNV;        // static bound of Nv for register arrays
   constexpr int RR = ring_rows(W);
-  constexpr int FS = RR * 32;                               // ring doubles per field
+  // ring layout: TMA -> sm[slot][box][field][34] (see above), cp.async -> sm[field][slot][32]
+  constexpr int RS = 2 * W + 1;                             // rows of the shallow ring (TMA only)
+  const int FS = TMA ? TMA_RW : RR * 32;                    // doubles between fields
+  const int SLOT = TMA ? tma_deep_slot(N) : 32;             // doubles between ring rows
+  const int SSLOT = TMA ? tma_shallow_slot(N) : 32;
   constexpr int FBS = (W + 1) * 32;                         // flux-buffer doubles per component
   constexpr int NT = 64 * W;                                // threads that take part in every named barrier
-  extern __shared__ double smem[];
-  double *sm = smem;
-  double *fb = smem + (size_t)NST * FS;
+  extern __shared__ __align__(128) double smem[];
+  double *sm = smem;                                                            // U fields
+  double *smp = TMA ? smem + tma_box_doubles(Nv) : smem + (size_t)Nv * FS;      // p, c, 1/rho
+  double *sms = TMA ? smem + (size_t)RR * SLOT : smem + (size_t)(Nv + 3) * FS;  // Gamma, chi_s
+  double *fb = TMA ? sms + (size_t)RS * SSLOT : smem + (size_t)NST * RR * 32;
+  const unsigned full_bar = (unsigned)__cvta_generic_to_shared(fb + (size_t)Nv * FBS);   // two mbarriers (TMA only)
+  if (TMA) {
+    if (threadIdx.x == 0 && threadIdx.y == 0) {
+      mbar_init(full_bar, W);                               // one arrival (with its byte count) per service warp
+      mbar_init(full_bar + 8, W);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+  }
 
   const int lane = threadIdx.x;
   const bool service = threadIdx.y >= W;
@@ -310,21 +366,32 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
   if (!service) {
     // =========================================================== compute warps
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(WS_REGS_COMPUTE));
-    int rb = 0, par = 0;
+    int rb = 0, rs = 0, par = 0;
+    unsigned phase = 0;
     bool bad = false, first = true;
     for (int fc = f_begin; fc <= f_end; fc += W) {
-      named_sync(BAR_RING_FULL + par, NT);                  // rows fc .. fc + W + 4 are in the ring
+      if (TMA) mbar_wait(full_bar + 8 * par, phase);        // rows fc .. fc + W + 4 are in the ring
+      else named_sync(BAR_RING_FULL + par, NT);
       const int f = fc + w;
       int o[6];
 #pragma unroll
       for (int m = 0; m < 6; ++m) {
         int sl = rb + w + m;
         sl -= sl >= RR ? RR : 0;
-        o[m] = sl * 32 + lane;
+        o[m] = sl * SLOT + lane + (TMA ? 1 : 0);
+      }
+      int s2 = o[2], s3 = o[3];
+      if (TMA) {                                            // shallow ring: slot of stencil row r is (r - f_begin - 2) mod RS
+        int q2 = rs + w;
+        q2 -= q2 >= RS ? RS : 0;
+        int q3 = q2 + 1;
+        q3 -= q3 >= RS ? RS : 0;
+        s2 = q2 * SSLOT + lane + 1;
+        s3 = q3 * SSLOT + lane + 1;
       }
       if (f <= f_end) {                                     // warp-uniform
         FluxStoreWS st{fb + (w + 1) * 32 + lane, FBS, first ? -1 : BAR_FB_EMPTY + par, NT};
-        const bool c2ok = face_flux<DIR>(N, sm, FS, o, sm + (Nv + 3) * FS, FS, o[2], o[3], st);
+        const bool c2ok = face_flux<DIR>(N, sm, smp, FS, o, sms, FS, s2, s3, st);
         bad = bad || (!c2ok && lane_ok);
       } else if (!first) {
         named_sync(BAR_FB_EMPTY + par, NT);                 // keep the barrier counts whole
@@ -332,6 +399,9 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
       named_arrive(BAR_FLUX_READY + par, NT);
       rb += W;
       rb -= rb >= RR ? RR : 0;
+      rs += W;
+      rs -= rs >= RS ? RS : 0;
+      phase ^= par;                                         // each mbarrier is used every other chunk
       par ^= 1;
       first = false;
     }
@@ -342,12 +412,31 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
   // ============================================================= service warps
   asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(WS_REGS_SERVICE));
   const int rmax = G.np[DIR] - 1;
-  auto stage_row = [&](int slot, int r) {                   // stencil row r (= padded row r) -> ring slot
-    const long long gi = colbase + (long long)(r < rmax ? r : rmax) * sst;
-    double *dst = sm + slot * 32 + lane;
+  const unsigned deep_bytes = (unsigned)(Nv + 3) * TMA_RW * sizeof(double);
+  const unsigned shallow_bytes = (unsigned)(N + 1) * TMA_RW * sizeof(double);
+  const int c0 = G.g[0] + blockIdx.x * 32 - 1, co = blockIdx.y + G.g[OD];      // TMA box origin (c0 is even)
+  auto stage_row = [&](int slot, int r, unsigned bar) {     // stencil row r (= padded row r) -> ring slot
+    const int rc = r < rmax ? r : rmax;
+    if (TMA) {                                              // boxes U [Nv][34] and p, c, 1/rho [3][34]
+      if (lane == 0) {
+        const unsigned dst = (unsigned)__cvta_generic_to_shared(sm + (size_t)slot * SLOT);
+        tma_load_row(dst, &tmU, c0, DIR == 1 ? rc : co, DIR == 1 ? co : rc, bar);
+        tma_load_row(dst + (unsigned)(tma_box_doubles(Nv) * sizeof(double)), &tmP, c0, DIR == 1 ? rc : co,
+                     DIR == 1 ? co : rc, bar);
+      }
+    } else {
+      const long long gi = colbase + (long long)rc * sst;
+      double *dst = sm + slot * 32 + lane;
 #pragma unroll 4
-    for (int f = 0; f < NST; ++f)
-      cp_async8(dst + f * FS, (f < Nv ? U + (size_t)f * G.cells : prim + (size_t)(f - Nv) * G.cells) + gi);
+      for (int f = 0; f < NST; ++f)
+        cp_async8(dst + f * FS, (f < Nv ? U + (size_t)f * G.cells : prim + (size_t)(f - Nv) * G.cells) + gi);
+    }
+  };
+  auto stage_shallow = [&](int slot, int r, unsigned bar) { // TMA only: box Gamma, chi_s [N + 1][34] of stencil row r
+    const int rc = r < rmax ? r : rmax;
+    if (lane == 0)
+      tma_load_row((unsigned)__cvta_generic_to_shared(sms + (size_t)slot * SSLOT), &tmS, c0, DIR == 1 ? rc : co,
+                   DIR == 1 ? co : rc, bar);
   };
   const double dt = E.mode == 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
   const double ninv = -G.inv_d[DIR];
@@ -408,15 +497,22 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
   };
 
   // ---- prologue: rows f_begin .. f_begin + W + 4 into ring slots 0 .. W + 4
-  for (int r = w; r < W + 5; r += W) stage_row(r, f_begin + r);
+  if (TMA) {                                                // shallow rows f_begin + 2 .. f_begin + W + 2 into slots 0 .. W
+    if (lane == 0)
+      mbar_expect_tx(full_bar, deep_bytes * (unsigned)((W + 5 - w + W - 1) / W) + shallow_bytes * (w == 0 ? 2u : 1u));
+    for (int r = w; r < W + 1; r += W) stage_shallow(r, f_begin + 2 + r, full_bar);
+  }
+  for (int r = w; r < W + 5; r += W) stage_row(r, f_begin + r, full_bar);
   cp_async_commit();
 
-  int rb = 0, par = 0;
+  int rb = 0, rs = 0, par = 0;
   bool first = true;
   int fprev = 0;
   for (int fc = f_begin; fc <= f_end; fc += W) {
-    cp_async_wait<0>();
-    named_arrive(BAR_RING_FULL + par, NT);                  // this chunk's rows have landed
+    if (!TMA) {
+      cp_async_wait<0>();
+      named_arrive(BAR_RING_FULL + par, NT);                // this chunk's rows have landed
+    }
     if (!first) {
       named_sync(BAR_FLUX_READY + (par ^ 1), NT);           // the previous chunk's fluxes are in fb, its ring rows are dead
       read_fluxes();
@@ -425,7 +521,14 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
     if (fc + W <= f_end) {                                  // the W new rows of the next chunk: row fc + W + 5 + w
       int slot = rb + W + 5 + w;
       slot -= slot >= RR ? RR : 0;
-      stage_row(slot, fc + W + 5 + w);
+      const unsigned bar = full_bar + 8 * (par ^ 1);
+      if (TMA && lane == 0) mbar_expect_tx(bar, deep_bytes + shallow_bytes);
+      stage_row(slot, fc + W + 5 + w, bar);
+      if (TMA) {                                            // shallow row fc + W + 3 + w
+        int q = rs + W + 1 + w;
+        q -= q >= RS ? RS : 0;
+        stage_shallow(q, fc + W + 3 + w, bar);
+      }
     }
     cp_async_commit();
     prefetch_operands(fc + w);                              // read one chunk later
@@ -433,6 +536,8 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
     fprev = fc + w;
     rb += W;
     rb -= rb >= RR ? RR : 0;
+    rs += W;
+    rs -= rs >= RS ? RS : 0;
     par ^= 1;
     first = false;
   }
@@ -442,6 +547,31 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
 }
 
 }  // namespace xf
+
+// Host side of the TMA path: a rank-4 tensor map {i, j, k, field} over `nf` consecutive fields of the padded box, with
+// one box = 34 cells along i (from an even index) of every field.  Returns false where TMA cannot describe the array (odd padded extents
+// make the strides no multiple of 16 bytes, or an unaligned base): the launcher then takes the cp.async kernel.
+inline bool xf_row_tensor_map(CUtensorMap *tm, const XfGrid &G, const double *base, int nf) {
+  typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                               const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                               CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static EncodeFn encode = [] {
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      fn = nullptr;
+    return reinterpret_cast<EncodeFn>(fn);
+  }();
+  if (!encode || (G.np[0] & 1) || (G.cells & 1) || (reinterpret_cast<uintptr_t>(base) & 15)) return false;
+  const cuuint64_t dims[4] = {(cuuint64_t)G.np[0], (cuuint64_t)G.np[1], (cuuint64_t)G.np[2], (cuuint64_t)nf};
+  const cuuint64_t strides[3] = {(cuuint64_t)G.st[1] * 8, (cuuint64_t)G.st[2] * 8, (cuuint64_t)G.cells * 8};
+  const cuuint32_t box[4] = {xf::TMA_RW, 1, 1, (cuuint32_t)nf};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  return encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double *>(base), dims, strides, box, estr,
+                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 
 #define XF_DISPATCH_SWEEP_N(N, CALL) \
   switch (N) {                       \
