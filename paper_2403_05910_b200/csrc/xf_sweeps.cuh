@@ -213,6 +213,8 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
       if (fc == f_begin && ok) W.prefetch_l2(gi, Nv);
       if (lane_ok && f + LJ <= f_end && gnext < G.cells) W.prefetch_l2(gnext, Nv);
     }
+#pragma unroll
+    for (int m = 0; m < 6; ++m) asm volatile("" : "+r"(o[m]));   // keep the six ring offsets in registers (see the y/z kernel)
     W.sm_us = sm + o[2];
     W.carry_rd = carry + par * Nv * LI;
     W.carry_wr = carry + (par ^ 1) * Nv * LI;
@@ -389,6 +391,11 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
         s2 = q2 * SSLOT + lane + 1;
         s3 = q3 * SSLOT + lane + 1;
       }
+      // the ring offsets are made opaque: otherwise the compiler, short of registers, re-derives every one of them
+      // (wrap selects and multiplies, ~40 integer instructions per species field) instead of keeping six registers
+#pragma unroll
+      for (int m = 0; m < 6; ++m) asm volatile("" : "+r"(o[m]));
+      asm volatile("" : "+r"(s2), "+r"(s3));
       if (f <= f_end) {                                     // warp-uniform
         FluxStoreWS st{fb + (w + 1) * 32 + lane, FBS, first ? -1 : BAR_FB_EMPTY + par, NT};
         const bool c2ok = face_flux<DIR>(N, sm, smp, FS, o, sms, FS, s2, s3, st);
