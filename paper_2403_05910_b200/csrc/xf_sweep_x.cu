@@ -1,4 +1,6 @@
 // xf_sweep_x.cu -- instantiations and launcher of the x-direction sweep (see xf_sweeps.cuh).
+#include <stdlib.h>
+
 #include "xf_sweeps.cuh"
 
 namespace {
@@ -6,6 +8,18 @@ using namespace xf;
 
 template <int NT>
 int launch(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status, cudaStream_t s) {
+  CUtensorMap tmU, tmP, tmS;   // U [N + 4]; p, c, 1/rho [3]; Gamma, chi_s [N + 1]
+  static const bool no_tma = getenv("XF_NO_TMA") != nullptr;
+  if (!no_tma && xf_span_tensor_map(&tmU, G, U, N + 4) && xf_span_tensor_map(&tmP, G, prim, 3) &&
+      xf_span_tensor_map(&tmS, G, prim + 3 * G.cells, N + 1)) {
+    const long long Lf = (long long)G.n[1] * G.np[0];
+    const int segc = XW_NCH * XW_CH - 1;
+    const int segs = (int)((Lf + segc - 1) / segc);
+    const unsigned blocks = (unsigned)(segs * G.n[2]);
+    const size_t smem = sizeof(double) * xw_smem_doubles(N);
+    sweep_x_ws_kernel<NT><<<blocks, dim3(32, 2 * XW_W), smem, s>>>(G, N, U, E, status, segs, tmU, tmP, tmS);
+    return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
+  }
   const long long L = (long long)G.n[1] * G.np[0];
   const int SEGC = X_NCH * 32 - 1;
   const int segs = (int)((L + SEGC - 1) / SEGC);
@@ -29,6 +43,9 @@ int xf_sweep_x_init() {
 #define CALL(NT)                                                                                                   \
   e = cudaFuncSetAttribute(sweep_kernel<NT, 0, X_LI, X_LJ, X_RR, X_MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
                            (int)(sizeof(double) * warp_smem_doubles(NT > 0 ? NT : XF_MAXN, X_LI, X_RR)));         \
+  if (e != cudaSuccess) return XF_ECUDA;                                                                           \
+  e = cudaFuncSetAttribute(sweep_x_ws_kernel<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize,                     \
+                           (int)(sizeof(double) * xw_smem_doubles(NT > 0 ? NT : XF_MAXN)));                        \
   if (e != cudaSuccess) return XF_ECUDA;
   CALL(0) CALL(1) CALL(2) CALL(3) CALL(4) CALL(10)
 #undef CALL

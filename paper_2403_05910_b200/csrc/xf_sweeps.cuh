@@ -553,29 +553,235 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
   write_cells(fprev);
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// x sweep, warp-specialised with TMA.  The interior rows of one k-plane are contiguous in memory, so a plane is one
+// flat pencil (see the top of this file) and a chunk is XW_W x 32 = 128 consecutive faces.  No ring: the chunk's
+// 133 stencil cells (+ alignment) are fetched as three dense boxes [fields][136] of a rank-2 tensor {cell, field}
+// into one of two stages; the 5-cell overlap between chunks is re-read from L2.  The stencil offsets of a lane are
+// then consecutive (immediate offsets in the loads).  Roles and barriers as in the y/z kernel.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int XW_W = 4;                    // compute warps = service warps per block
+constexpr int XW_CH = XW_W * 32;           // faces per chunk
+constexpr int XW_BOX = XW_CH + 8;          // cells per box: 133 needed, from an even index, 16-byte multiple
+constexpr int XW_NCH = 16;                 // chunks per block
+constexpr int XW_FBW = XW_CH + 2;          // flux-buffer doubles per component: [0] = last face of the previous chunk
+__host__ __device__ constexpr int xw_box_doubles(int nf) { return (nf * XW_BOX * 8 + 127) / 128 * 16; }
+__host__ __device__ constexpr int xw_stage_doubles(int N) {
+  return xw_box_doubles(N + 4) + xw_box_doubles(3) + xw_box_doubles(N + 1);
+}
+__host__ __device__ inline size_t xw_smem_doubles(int N) {
+  return 2 * (size_t)xw_stage_doubles(N) + (size_t)(N + 4) * XW_FBW + 2;
+}
+__device__ __forceinline__ void tma_load_span(unsigned dst, const void *tmap, int c0, unsigned bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
+      "l"(tmap), "r"(c0), "r"(0), "r"(bar)
+      : "memory");
+}
+
+template <int N_T>
+__global__ void __launch_bounds__(64 * XW_W, 2)
+sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const XfEpilogue E,
+                  int *__restrict__ status, const int segs_per_plane, const __grid_constant__ CUtensorMap tmU,
+                  const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmS) {
+  constexpr int W = XW_W, NT = 64 * W, FS = XW_BOX;
+  const int N = N_T > 0 ? N_T : Nrt;
+  const int Nv = N + 4;
+  constexpr int NVS = N_T > 0 ? N_T + 4 : XF_MAXNV;
+  const int STAGE = xw_stage_doubles(N), OFFP = xw_box_doubles(Nv), OFFS = OFFP + xw_box_doubles(3);
+  extern __shared__ __align__(128) double smem[];
+  double *fb = smem + 2 * (size_t)STAGE;                    // face fluxes [Nv][XW_FBW]
+  const unsigned full_bar = (unsigned)__cvta_generic_to_shared(fb + (size_t)Nv * XW_FBW);
+  if (threadIdx.x == 0 && threadIdx.y == 0) {
+    mbar_init(full_bar, 1);
+    mbar_init(full_bar + 8, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  const int lane = threadIdx.x;
+  const bool service = threadIdx.y >= W;
+  const int w = service ? threadIdx.y - W : threadIdx.y;
+  const int plane = blockIdx.x / segs_per_plane, seg = blockIdx.x - plane * segs_per_plane;
+  const int L = G.n[1] * G.np[0];                           // flat cells of the plane's interior rows
+  constexpr int SEGC = XW_NCH * XW_CH - 1;
+  const int f_begin = seg * SEGC;                           // faces f_begin .. f_end, cells f_begin .. f_end - 1
+  const int f_end = f_begin + SEGC < L ? f_begin + SEGC : L;
+  const long long P0 = (long long)(plane + G.g[2]) * G.st[2] + (long long)G.g[1] * G.st[1];  // flat cell 0
+  // chunk c needs flat cells fc - 3 .. fc + 130; its boxes start at the even global index below P0 + fc - 3
+  const long long g0 = P0 + f_begin - 3;
+  const int delta = (int)(g0 & 1);                          // same for every chunk: they are 128 cells apart
+  const int u = 32 * w + lane;                              // face within the chunk (compute) / cell slot (service)
+
+  if (!service) {
+    // =========================================================== compute warps
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(WS_REGS_COMPUTE));
+    int par = 0;
+    unsigned phase = 0;
+    bool bad = false, first = true;
+    for (int fc = f_begin; fc <= f_end; fc += XW_CH) {
+      mbar_wait(full_bar + 8 * par, phase);
+      const double *st = smem + (size_t)par * STAGE;
+      const int f = fc + u;
+      int o[6];
+#pragma unroll
+      for (int m = 0; m < 6; ++m) o[m] = u + delta + m;
+      // every lane of the block passes the same barriers; lanes past f_end compute on staged (valid or zero) data
+      FluxStoreWS fsw{fb + u + 1, XW_FBW, first ? -1 : BAR_FB_EMPTY + par, NT};
+      const bool c2ok = face_flux<0>(N, st, st + OFFP, FS, o, st + OFFS, FS, o[2], o[3], fsw);
+      {
+        const int ia = (f - 1 + G.np[0]) % G.np[0], ib = f % G.np[0];
+        const bool used = f <= f_end && ((ia >= G.g[0] && ia < G.g[0] + G.n[0]) || (ib >= G.g[0] && ib < G.g[0] + G.n[0]));
+        bad = bad || (!c2ok && used);
+      }
+      named_arrive(BAR_FLUX_READY + par, NT);
+      phase ^= par;
+      par ^= 1;
+      first = false;
+    }
+    if (bad) atomicOr(status, XF_FLAG_NONPHYSICAL);
+    return;
+  }
+  // ============================================================= service warps
+  asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(WS_REGS_SERVICE));
+  const unsigned stage_bytes = (unsigned)(2 * N + 8) * XW_BOX * sizeof(double);
+  auto stage_chunk = [&](int fc, int st) {                  // the three boxes of chunk fc -> stage st (one lane issues)
+    if (w != 0 || lane != 0) return;
+    const unsigned bar = full_bar + 8 * st;
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(smem + (size_t)st * STAGE);
+    const int c0 = (int)(P0 + fc - 3 - delta);              // even; may be negative or run past the array: zero-filled
+    mbar_expect_tx(bar, stage_bytes);
+    tma_load_span(dst, &tmU, c0, bar);
+    tma_load_span(dst + (unsigned)(OFFP * sizeof(double)), &tmP, c0, bar);
+    tma_load_span(dst + (unsigned)(OFFS * sizeof(double)), &tmS, c0, bar);
+  };
+  const double dt = E.mode == 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
+  const double ninv = -G.inv_d[0];
+  const bool need_acc = E.mode == 1 || (E.mode == 2 && E.has_acc);
+  const bool need_un = E.mode == 2 && E.alpha != 0.0;
+
+  // lane (w, lane) of the service group owns slot u of a chunk: cell fc + u - 1, between the chunk's faces u - 1 and u
+  double d[NVS];
+  auto read_fluxes = [&]() {
+#pragma unroll
+    for (int v = 0; v < NVS; ++v)
+      if (v < Nv) d[v] = (fb[v * XW_FBW + u + 1] - fb[v * XW_FBW + u]) * ninv;
+    __syncwarp();
+    if (w == 0 && lane < Nv) fb[lane * XW_FBW] = fb[lane * XW_FBW + XW_CH];   // carry: only slot 0 (this warp) reads [0]
+  };
+  auto cell_index = [&](int fc, long long &gi) -> bool {    // global index of this lane's cell; false if it is not updated
+    const int cf = fc + u - 1;
+    gi = P0 + cf;
+    if (cf < f_begin || cf >= f_end) return false;
+    const int i = cf % G.np[0];
+    return i >= G.g[0] && i < G.g[0] + G.n[0];
+  };
+  auto prefetch_operands = [&](int fc) {
+    const int cf = fc + u - 1;
+    if (!(need_acc || need_un) || (lane & 15) != 0 || cf < f_begin || cf >= f_end) return;
+    const long long gi = P0 + cf;
+    for (int v = 0; v < Nv; ++v) {
+      if (need_acc) asm volatile("prefetch.global.L2 [%0];" ::"l"(E.acc + v * G.cells + gi));
+      if (need_un) asm volatile("prefetch.global.L2 [%0];" ::"l"(E.Un + v * G.cells + gi));
+    }
+  };
+  auto write_cells = [&](int fc) {
+    long long gi;
+    if (!cell_index(fc, gi)) return;
+    constexpr int VB = 4;
+#pragma unroll
+    for (int v0 = 0; v0 < NVS; v0 += VB) {
+      double a[VB], un[VB], us[VB];
+#pragma unroll
+      for (int q = 0; q < VB; ++q) {
+        const int v = v0 + q;
+        if (v < Nv && v < NVS) {
+          const long long idx = v * G.cells + gi;
+          a[q] = need_acc ? E.acc[idx] : 0.0;
+          un[q] = need_un ? E.Un[idx] : 0.0;
+          us[q] = E.mode == 2 ? U[idx] : 0.0;
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < VB; ++q) {
+        const int v = v0 + q;
+        if (v < Nv && v < NVS) {
+          const long long idx = v * G.cells + gi;
+          if (E.mode == 0) {
+            E.out[idx] = d[v];
+          } else if (E.mode == 1) {
+            E.out[idx] = a[q] + d[v];
+          } else {
+            const double Lr = need_acc ? a[q] + d[v] : d[v];
+            E.out[idx] = need_un ? fma(E.alpha, un[q], E.beta * fma(dt, Lr, us[q])) : E.beta * fma(dt, Lr, us[q]);
+          }
+        }
+      }
+    }
+  };
+
+  stage_chunk(f_begin, 0);
+  int par = 0, fprev = 0;
+  bool first = true;
+  for (int fc = f_begin; fc <= f_end; fc += XW_CH) {
+    if (!first) {
+      named_sync(BAR_FLUX_READY + (par ^ 1), NT);           // the previous chunk's fluxes are in fb, its stage is free
+      read_fluxes();
+      named_arrive(BAR_FB_EMPTY + par, NT);
+    }
+    if (fc + XW_CH <= f_end) stage_chunk(fc + XW_CH, par ^ 1);
+    prefetch_operands(fc);
+    if (!first) write_cells(fprev);
+    fprev = fc;
+    par ^= 1;
+    first = false;
+  }
+  named_sync(BAR_FLUX_READY + (par ^ 1), NT);               // the last chunk
+  read_fluxes();
+  write_cells(fprev);
+}
+
 }  // namespace xf
 
 // Host side of the TMA path: a rank-4 tensor map {i, j, k, field} over `nf` consecutive fields of the padded box, with
 // one box = 34 cells along i (from an even index) of every field.  Returns false where TMA cannot describe the array (odd padded extents
 // make the strides no multiple of 16 bytes, or an unaligned base): the launcher then takes the cp.async kernel.
-inline bool xf_row_tensor_map(CUtensorMap *tm, const XfGrid &G, const double *base, int nf) {
-  typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                               const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
-                               CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-  static EncodeFn encode = [] {
+typedef CUresult (*XfTensorMapEncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                        const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                        CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                        CUtensorMapFloatOOBfill);
+inline XfTensorMapEncodeFn xf_tensor_map_encoder() {
+  static XfTensorMapEncodeFn encode = [] {
     void *fn = nullptr;
     cudaDriverEntryPointQueryResult q;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess ||
         q != cudaDriverEntryPointSuccess)
       fn = nullptr;
-    return reinterpret_cast<EncodeFn>(fn);
+    return reinterpret_cast<XfTensorMapEncodeFn>(fn);
   }();
+  return encode;
+}
+inline bool xf_row_tensor_map(CUtensorMap *tm, const XfGrid &G, const double *base, int nf) {
+  XfTensorMapEncodeFn encode = xf_tensor_map_encoder();
   if (!encode || (G.np[0] & 1) || (G.cells & 1) || (reinterpret_cast<uintptr_t>(base) & 15)) return false;
   const cuuint64_t dims[4] = {(cuuint64_t)G.np[0], (cuuint64_t)G.np[1], (cuuint64_t)G.np[2], (cuuint64_t)nf};
   const cuuint64_t strides[3] = {(cuuint64_t)G.st[1] * 8, (cuuint64_t)G.st[2] * 8, (cuuint64_t)G.cells * 8};
   const cuuint32_t box[4] = {xf::TMA_RW, 1, 1, (cuuint32_t)nf};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   return encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double *>(base), dims, strides, box, estr,
+                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+// x sweep: a rank-2 map {flat cell, field}; one box = XW_BOX consecutive cells (from an even index) of every field.
+inline bool xf_span_tensor_map(CUtensorMap *tm, const XfGrid &G, const double *base, int nf) {
+  XfTensorMapEncodeFn encode = xf_tensor_map_encoder();
+  if (!encode || (G.cells & 1) || (reinterpret_cast<uintptr_t>(base) & 15)) return false;
+  const cuuint64_t dims[2] = {(cuuint64_t)G.cells, (cuuint64_t)nf};
+  const cuuint64_t strides[1] = {(cuuint64_t)G.cells * 8};
+  const cuuint32_t box[2] = {xf::XW_BOX, (cuuint32_t)nf};
+  const cuuint32_t estr[2] = {1, 1};
+  return encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double *>(base), dims, strides, box, estr,
                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
