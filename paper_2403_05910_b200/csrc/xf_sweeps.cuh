@@ -308,6 +308,7 @@ __device__ __forceinline__ void tma_load_row(unsigned dst, const void *tmap, int
 }
 
 constexpr int BAR_RING_FULL = 1, BAR_FLUX_READY = 3, BAR_FB_EMPTY = 5;   // + chunk parity
+constexpr int BAR_SERVICE = 7;   // among the service warps: all have read U^s before any of them overwrites ring rows
 constexpr int WS_REGS_COMPUTE = 184, WS_REGS_SERVICE = 72;
 
 struct FluxStoreWS {
@@ -452,10 +453,14 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
 
   // cell row of face f (cell f - 1, staged at stencil row f + 2): Eq. 13 and the stage combination
   double d[NVS];
-  auto read_fluxes = [&]() {                                // part 1: everything the update needs from fb
+  auto read_fluxes = [&](int ous) {                         // part 1: everything the update needs from shared memory
 #pragma unroll
-    for (int v = 0; v < NVS; ++v)
-      if (v < Nv) d[v] = (fb[v * FBS + (w + 1) * 32 + lane] - fb[v * FBS + w * 32 + lane]) * ninv;
+    for (int v = 0; v < NVS; ++v) {
+      if (v < Nv) {
+        d[v] = (fb[v * FBS + (w + 1) * 32 + lane] - fb[v * FBS + w * 32 + lane]) * ninv;
+        if (E.mode == 2) d[v] = fma(dt, d[v], sm[v * FS + ous]);   // U^s + dt div: U^s is still in the ring
+      }
+    }
     if (w == 0) {                                           // carry the chunk's last face to row 0 (only warp 0 reads row 0)
       for (int v = 0; v < Nv; ++v) fb[v * FBS + lane] = fb[v * FBS + W * 32 + lane];
     }
@@ -474,7 +479,7 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
     constexpr int VB = 4;                                   // fields per batch: all loads of a batch fly together
 #pragma unroll
     for (int v0 = 0; v0 < NVS; v0 += VB) {
-      double a[VB], un[VB], us[VB];
+      double a[VB], un[VB];
 #pragma unroll
       for (int q = 0; q < VB; ++q) {
         const int v = v0 + q;
@@ -482,7 +487,6 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
           const long long idx = v * G.cells + gi;
           a[q] = need_acc ? E.acc[idx] : 0.0;
           un[q] = need_un ? E.Un[idx] : 0.0;
-          us[q] = E.mode == 2 ? U[idx] : 0.0;
         }
       }
 #pragma unroll
@@ -495,8 +499,8 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
           } else if (E.mode == 1) {
             E.out[idx] = a[q] + d[v];
           } else {
-            const double L = need_acc ? a[q] + d[v] : d[v];
-            E.out[idx] = need_un ? fma(E.alpha, un[q], E.beta * fma(dt, L, us[q])) : E.beta * fma(dt, L, us[q]);
+            const double L = need_acc ? fma(dt, a[q], d[v]) : d[v];   // U^s + dt (acc + div)
+            E.out[idx] = need_un ? fma(E.alpha, un[q], E.beta * L) : E.beta * L;
           }
         }
       }
@@ -514,7 +518,7 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
 
   int rb = 0, rs = 0, par = 0;
   bool first = true;
-  int fprev = 0;
+  int fprev = 0, ous = 0;
   for (int fc = f_begin; fc <= f_end; fc += W) {
     if (!TMA) {
       cp_async_wait<0>();
@@ -522,8 +526,9 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
     }
     if (!first) {
       named_sync(BAR_FLUX_READY + (par ^ 1), NT);           // the previous chunk's fluxes are in fb, its ring rows are dead
-      read_fluxes();
+      read_fluxes(ous);
       named_arrive(BAR_FB_EMPTY + par, NT);
+      if (E.mode == 2) named_sync(BAR_SERVICE, 32 * W);     // U^s was read from ring rows the next copies overwrite
     }
     if (fc + W <= f_end) {                                  // the W new rows of the next chunk: row fc + W + 5 + w
       int slot = rb + W + 5 + w;
@@ -541,6 +546,11 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
     prefetch_operands(fc + w);                              // read one chunk later
     if (!first) write_cells(fprev);
     fprev = fc + w;
+    {                                                       // where U^s of that cell row (stencil row f + 2) sits
+      int sl = rb + w + 2;
+      sl -= sl >= RR ? RR : 0;
+      ous = sl * SLOT + lane + (TMA ? 1 : 0);
+    }
     rb += W;
     rb -= rb >= RR ? RR : 0;
     rs += W;
@@ -549,7 +559,7 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
     first = false;
   }
   named_sync(BAR_FLUX_READY + (par ^ 1), NT);               // the last chunk
-  read_fluxes();
+  read_fluxes(ous);
   write_cells(fprev);
 }
 
@@ -663,10 +673,15 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
 
   // lane (w, lane) of the service group owns slot u of a chunk: cell fc + u - 1, between the chunk's faces u - 1 and u
   double d[NVS];
-  auto read_fluxes = [&]() {
+  auto read_fluxes = [&](int st) {                          // st: stage of the chunk whose cells are updated
+    const double *us = smem + (size_t)st * STAGE + u + delta + 2;   // cell fc + u - 1 = stencil cell m = 2 of face fc + u
 #pragma unroll
-    for (int v = 0; v < NVS; ++v)
-      if (v < Nv) d[v] = (fb[v * XW_FBW + u + 1] - fb[v * XW_FBW + u]) * ninv;
+    for (int v = 0; v < NVS; ++v) {
+      if (v < Nv) {
+        d[v] = (fb[v * XW_FBW + u + 1] - fb[v * XW_FBW + u]) * ninv;
+        if (E.mode == 2) d[v] = fma(dt, d[v], us[v * FS]);   // U^s + dt div: U^s is still in the stage
+      }
+    }
     __syncwarp();
     if (w == 0 && lane < Nv) fb[lane * XW_FBW] = fb[lane * XW_FBW + XW_CH];   // carry: only slot 0 (this warp) reads [0]
   };
@@ -692,7 +707,7 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
     constexpr int VB = 4;
 #pragma unroll
     for (int v0 = 0; v0 < NVS; v0 += VB) {
-      double a[VB], un[VB], us[VB];
+      double a[VB], un[VB];
 #pragma unroll
       for (int q = 0; q < VB; ++q) {
         const int v = v0 + q;
@@ -700,7 +715,6 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
           const long long idx = v * G.cells + gi;
           a[q] = need_acc ? E.acc[idx] : 0.0;
           un[q] = need_un ? E.Un[idx] : 0.0;
-          us[q] = E.mode == 2 ? U[idx] : 0.0;
         }
       }
 #pragma unroll
@@ -713,8 +727,8 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
           } else if (E.mode == 1) {
             E.out[idx] = a[q] + d[v];
           } else {
-            const double Lr = need_acc ? a[q] + d[v] : d[v];
-            E.out[idx] = need_un ? fma(E.alpha, un[q], E.beta * fma(dt, Lr, us[q])) : E.beta * fma(dt, Lr, us[q]);
+            const double Lr = need_acc ? fma(dt, a[q], d[v]) : d[v];   // U^s + dt (acc + div)
+            E.out[idx] = need_un ? fma(E.alpha, un[q], E.beta * Lr) : E.beta * Lr;
           }
         }
       }
@@ -727,8 +741,9 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
   for (int fc = f_begin; fc <= f_end; fc += XW_CH) {
     if (!first) {
       named_sync(BAR_FLUX_READY + (par ^ 1), NT);           // the previous chunk's fluxes are in fb, its stage is free
-      read_fluxes();
+      read_fluxes(par ^ 1);
       named_arrive(BAR_FB_EMPTY + par, NT);
+      if (E.mode == 2) named_sync(BAR_SERVICE, 32 * W);     // U^s was read from the stage the next copy overwrites
     }
     if (fc + XW_CH <= f_end) stage_chunk(fc + XW_CH, par ^ 1);
     prefetch_operands(fc);
@@ -738,7 +753,7 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
     first = false;
   }
   named_sync(BAR_FLUX_READY + (par ^ 1), NT);               // the last chunk
-  read_fluxes();
+  read_fluxes(par ^ 1);
   write_cells(fprev);
 }
 
