@@ -3,9 +3,9 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl b200|reference] [--workload config4]
 
-A "step" is one pass of the whole hot path over the workload: xf_max_wavespeed (the CFL reduction) followed by
-xf_rk3_step_cfl -- three times (ghost fill, primitives, x/y/z sweeps with the flux divergence and the fused
-SSP-RK3 stage combination).  One step is therefore 3 convective-RHS evaluations of every interior cell, and
+A "step" is one pass of the whole hot path over the workload, xf_step_cfl: the CFL max-wave-speed reduction (fused
+into the first stage's primitives kernel) and three times (ghost fill, primitives, x/y/z sweeps with the flux
+divergence and the fused SSP-RK3 stage combination).  One step is therefore 3 convective-RHS evaluations of every interior cell, and
 
     value = interior cells x 3 x K x N / time          [cell-updates/s per RK stage, whole job]
 
@@ -246,8 +246,7 @@ def run_b200(args, rank: int, local_rank: int, world: int) -> None:
     peak_tf, probe_ms = xf.xf_probe_fp64_peak(local_rank, 60000)
 
     def step():
-        ctx.xf_max_wavespeed(U, T, S)
-        ctx.xf_rk3_step_cfl(U, T, cfl, S, work)
+        ctx.xf_step_cfl(U, T, cfl, S, work)
 
     for _ in range(args.warmup):
         step()
@@ -348,8 +347,8 @@ def run_b200(args, rank: int, local_rank: int, world: int) -> None:
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": name, "grid": list(grid), "nspecies": N, "nvars": Nv, "interior_cells": cells,
-                       "step": "xf_max_wavespeed + xf_rk3_step_cfl = 3 x (ghost fill, primitives, x/y/z sweeps, "
-                               "RK combine)", "rhs_per_step": 3, "l2": "inputs larger than L2 (one U copy = "
+                       "step": "xf_step_cfl = max wave speed (in the first primitives kernel) + 3 x (ghost fill, "
+                               "primitives, x/y/z sweeps, RK combine)", "rhs_per_step": 3, "l2": "inputs larger than L2 (one U copy = "
                                f"{Nv * ctx.cells * 8 / 1e9:.2f} GB), no flush", "parallelism": "replicas"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
             "step_roofline": step_roofline,

@@ -98,6 +98,12 @@ int xf_rk3_step(xf_ctx *ctx, double *U, double *T, double dt, void *work, void *
  * xf_max_wavespeed on the same stream. */
 int xf_rk3_step_cfl(xf_ctx *ctx, double *U, double *T, double cfl, const double *S_dev, void *work, void *stream);
 
+/* One whole time step at a given CFL number: S (as xf_max_wavespeed defines it, of the incoming U^n) is reduced inside
+ * the primitives kernel of the first stage and written to *S_dev, and the three stages use dt = cfl / S read on the
+ * device -- the same result as xf_max_wavespeed followed by xf_rk3_step_cfl, without recovering the primitives of
+ * U^n twice.  S_dev: 1 double, device, written. */
+int xf_step_cfl(xf_ctx *ctx, double *U, double *T, double cfl, double *S_dev, void *work, void *stream);
+
 /* S = max over interior cells of sum_{d active} (|u_d| + c)/dx_d, so that dt = CFL / S (Eq. 17,
  * PAPER.md:429; reading R9).  Recovers T of the interior cells on the way (T in/out).  S_dev: 1 double, device. */
 int xf_max_wavespeed(xf_ctx *ctx, const double *U, double *T, double *S_dev, void *stream);

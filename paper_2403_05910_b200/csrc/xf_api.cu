@@ -83,7 +83,8 @@ int count_active(const XfGrid &G) { return (G.n[0] > 1) + (G.n[1] > 1) + (G.n[2]
 
 // ghosts -> primitives -> sweeps.  E_last describes what the LAST active sweep writes (residual or RK combine);
 // earlier sweeps accumulate the partial residual in `acc`.
-int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfEpilogue &E_last, cudaStream_t s) {
+int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfEpilogue &E_last, cudaStream_t s,
+             double *S_out = nullptr) {
   int rc;
   {
     Timed t(c, XF_K_GHOST, s);
@@ -93,7 +94,7 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
   double *prim = static_cast<double *>(work);  // p, c, 1/rho, Gamma, chi_1..chi_N
   {
     Timed t(c, XF_K_PRIM, s);
-    rc = xf_launch_prim(c->G, c->Th, U, T, prim, nullptr, nullptr, c->status_dev, nullptr, s);
+    rc = xf_launch_prim(c->G, c->Th, U, T, prim, nullptr, nullptr, c->status_dev, nullptr, S_out, s);
   }
   ++c->launches;
   if (rc != XF_OK) return rc;
@@ -125,7 +126,9 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
   return XF_OK;
 }
 
-int rk3(xf_ctx *c, double *U, double *T, double dt, double cfl, const double *S_dev, void *work, cudaStream_t s) {
+// S_out != nullptr: the first stage's primitives kernel reduces the max wave speed of U^n into it (xf_step_cfl)
+int rk3(xf_ctx *c, double *U, double *T, double dt, double cfl, const double *S_dev, void *work, cudaStream_t s,
+        double *S_out = nullptr) {
   const size_t n = (size_t)c->G.cells;
   double *w = static_cast<double *>(work);
   double *U1 = w + (size_t)(c->N + 4) * n;
@@ -140,7 +143,7 @@ int rk3(xf_ctx *c, double *U, double *T, double dt, double cfl, const double *S_
   E.Un = U;
   // Eq. 16: U1 = Un + dt L(Un); U2 = 3/4 Un + 1/4 (U1 + dt L(U1)); Un+1 = 1/3 Un + 2/3 (U2 + dt L(U2))
   E.alpha = 0.0; E.beta = 1.0; E.out = U1;
-  int rc = residual(c, U, T, work, acc, E, s);
+  int rc = residual(c, U, T, work, acc, E, s, S_out);
   if (rc != XF_OK) return rc;
   E.alpha = 0.75; E.beta = 0.25; E.out = U2;
   rc = residual(c, U1, T, work, acc, E, s);
@@ -284,7 +287,7 @@ int xf_primitives(xf_ctx *c, const double *U, double *T, double *p, double *cs, 
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (cudaMemsetAsync(c->itersum_dev, 0, sizeof(unsigned long long), s) != cudaSuccess) return XF_ECUDA;
   ++c->launches;
-  return xf_launch_prim(c->G, c->Th, U, T, nullptr, p, cs, c->status_dev, c->itersum_dev, s);
+  return xf_launch_prim(c->G, c->Th, U, T, nullptr, p, cs, c->status_dev, c->itersum_dev, nullptr, s);
 }
 
 int xf_convective_rhs(xf_ctx *c, double *U, double *T, double *rhs, void *work, void *stream) {
@@ -310,6 +313,13 @@ int xf_rk3_step_cfl(xf_ctx *c, double *U, double *T, double cfl, const double *S
   DeviceGuard guard(c->device);
   if (!guard.ok) return XF_ECUDA;
   return rk3(c, U, T, 0.0, cfl, S_dev, work, static_cast<cudaStream_t>(stream));
+}
+
+int xf_step_cfl(xf_ctx *c, double *U, double *T, double cfl, double *S_dev, void *work, void *stream) {
+  if (!c || !U || !T || !work || !S_dev || !(cfl > 0.0)) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  return rk3(c, U, T, 0.0, cfl, S_dev, work, static_cast<cudaStream_t>(stream), S_dev);
 }
 
 int xf_max_wavespeed(xf_ctx *c, const double *U, double *T, double *S_dev, void *stream) {
@@ -425,13 +435,7 @@ int xf_rk3_steps_host(xf_ctx *c, double *U_host, double *T_host, double cfl, int
   if (cudaMemcpyAsync(c->hT, T_host, fb, cudaMemcpyHostToDevice, s) != cudaSuccess) return XF_ECUDA;
   double t = 0.0;
   for (int k = 0; k < nsteps; ++k) {
-    ++c->launches;
-    {
-      Timed tm(c, XF_K_WAVESPEED, s);
-      rc = xf_launch_wavespeed(c->G, c->Th, c->hU, c->hT, c->S_dev, c->status_dev, s);
-    }
-    if (rc != XF_OK) return rc;
-    rc = rk3(c, c->hU, c->hT, 0.0, cfl, c->S_dev, c->hW, s);
+    rc = rk3(c, c->hU, c->hT, 0.0, cfl, c->S_dev, c->hW, s, c->S_dev);
     if (rc != XF_OK) return rc;
     if (t_advanced) {
       double S = 0.0;

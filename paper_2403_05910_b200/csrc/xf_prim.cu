@@ -1,114 +1,42 @@
 // xf_prim.cu -- primitive recovery (Eq. 21) and the CFL max-wave-speed reduction
-// (Eq. 17) for sm_100a.  One thread per cell; the species table sits in the
+// (Eq. 17) for sm_100a, one kernel.  One thread per cell; the species table sits in the
 // kernel-parameter constant bank, so every coefficient read is a uniform constant load.
 #include "xf_common.cuh"
 
 namespace {
 
+// The Newton iteration runs on the MIXTURE polynomials: with y_s = Y_s R_s fixed in a cell,
+//   sum_s y_s cp_s(T)/R_s = A0 + A1 T + ... + A4 T^4,   sum_s y_s h_s(T)/R_s = T (A0 + B1 T + ... + B4 T^4) + A5,
+// A_k = sum_s y_s a_{s,k}, B_k = sum_s y_s b_{s,k}: ten sums over the species once per cell, after which an iteration
+// costs two Horner chains instead of two per species.  Only the final e_s(T) (for chi_s) is evaluated per species.
 template <int N_T>
-struct CellState {
-  static constexpr int NS = N_T > 0 ? N_T : XF_MAXN;
-  double Y[NS];
-  double rho, rinv, vel[3], e, E;
-};
-
-// cp_s/R_s and e_s/R_s... at temperature T with the constant-cp continuation outside [Tlo, Thi] (reading R3)
-__device__ __forceinline__ void species_cp_h(const XfThermo &th, int s, double T, double Tc, double &cpR, double &hR) {
-  const double *a = th.a[s];
-  const double *b = th.b[s];
-  cpR = fma(Tc, fma(Tc, fma(Tc, fma(Tc, a[4], a[3]), a[2]), a[1]), a[0]);
-  const double hp = fma(Tc, fma(Tc, fma(Tc, fma(Tc, b[3], b[2]), b[1]), b[0]), a[0]);
-  hR = fma(Tc, hp, a[5]);
-  hR = fma(cpR, T - Tc, hR);
-}
-
-template <int N_T>
-__device__ __forceinline__ void load_cell(const XfGrid &G, int N, const double *__restrict__ U, long long idx,
-                                          CellState<N_T> &S) {
-  S.rho = U[idx];
-  S.rinv = 1.0 / S.rho;
-  double k = 0.0;
-#pragma unroll
-  for (int q = 0; q < 3; ++q) {
-    S.vel[q] = U[(1 + q) * G.cells + idx] * S.rinv;
-    k = fma(S.vel[q], S.vel[q], k);
-  }
-  S.E = U[4 * G.cells + idx];
-  S.e = fma(S.E, S.rinv, -0.5 * k);
-  double sum = 0.0;
-#pragma unroll
-  for (int i = 0; i < CellState<N_T>::NS - 1; ++i) {
-    if (i < N - 1) {
-      S.Y[i] = U[(5 + i) * G.cells + idx] * S.rinv;
-      sum += S.Y[i];
-    }
-  }
-#pragma unroll
-  for (int i = 0; i < CellState<N_T>::NS; ++i)
-    if (i == N - 1) S.Y[i] = 1.0 - sum;  // closure: no clipping, no renormalisation (reading R12)
-}
-
-// Newton iteration T^{k+1} = T^k + (e - e(T^k))/Cv(T^k) (Eq. 21); returns T, Rbar, Cv at the final T is recomputed
-// by the caller.  Stops when |dT| <= rtol |T| or after maxit steps.
-template <int N_T>
-__device__ __forceinline__ double newton_T(const XfThermo &th, int N, const CellState<N_T> &S, double T, int &iters,
-                                           bool &converged) {
-  double Rbar = 0.0;
-#pragma unroll
-  for (int s = 0; s < CellState<N_T>::NS; ++s)
-    if (s < N) Rbar = fma(S.Y[s], th.Rs[s], Rbar);
-  int k = 0;
-  converged = false;
-  while (k < th.maxit) {
-    const double Tc = fmin(fmax(T, th.Tlo), th.Thi);
-    double hm = 0.0, cpm = 0.0;  // sum Y_s h_s, sum Y_s cp_s
-#pragma unroll
-    for (int s = 0; s < CellState<N_T>::NS; ++s) {
-      if (s < N) {
-        double cpR, hR;
-        species_cp_h(th, s, T, Tc, cpR, hR);
-        const double yr = S.Y[s] * th.Rs[s];
-        hm = fma(yr, hR, hm);
-        cpm = fma(yr, cpR, cpm);
-      }
-    }
-    const double eT = fma(-Rbar, T, hm);
-    const double Cv = cpm - Rbar;
-    const double Tn = T + (S.e - eT) / Cv;
-    ++k;
-    const double dT = fabs(Tn - T);
-    T = Tn;
-    if (dT <= th.rtol * fabs(Tn)) {
-      converged = true;
-      break;
-    }
-    if (!(Tn == Tn)) break;
-  }
-  iters = k;
-  return T;
-}
-
-// One evaluation site for the species polynomials: the loop body evaluates sum Y_s h_s, sum Y_s cp_s and e_s/R_s at
-// the current T; a Newton update follows unless the previous update already converged, in which case the values
-// just computed ARE the final ones (C_v, e_s at the converged T, as the problem statement asks: p, Gamma, c, chi_s
-// follow from the final T).  One code copy instead of two keeps the kernel at 128 registers = 16 warps per SM.
-template <int N_T>
-__global__ void __launch_bounds__(128, 4)
+__global__ void __launch_bounds__(128, 6)
 prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *__restrict__ U, double *__restrict__ T,
             double *__restrict__ prim, double *__restrict__ p_out, double *__restrict__ c_out,
-            int *__restrict__ status, unsigned long long *__restrict__ itersum) {
-  constexpr int NS = CellState<N_T>::NS;
+            int *__restrict__ status, unsigned long long *__restrict__ itersum, double *__restrict__ S_out) {
+  constexpr int NS = N_T > 0 ? N_T : XF_MAXN;
   const int N = N_T > 0 ? N_T : th.N;
   const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   int it = 0;
-  if (idx < G.cells) {
+  double smax = 0.0;   // this cell's sum_d (|u_d| + c)/dx_d if it is an interior cell and S_out is wanted
+  bool interior = true;
+  if (S_out && idx < G.cells) {
+    const int i = (int)(idx % G.np[0]);
+    const long long r = idx / G.np[0];
+    const int j = (int)(r % G.np[1]), k = (int)(r / G.np[1]);
+    interior = i >= G.g[0] && i < G.g[0] + G.n[0] && j >= G.g[1] && j < G.g[1] + G.n[1] && k >= G.g[2] &&
+               k < G.g[2] + G.n[2];
+  }
+  // xf_max_wavespeed (S_out without the workspace fields) looks at interior cells only: ghosts may be unfilled
+  if (idx < G.cells && (interior || prim)) {
     const double rho = U[idx];
     const double rinv = xf_rcp(rho);
-    double k2 = 0.0;
+    double k2 = 0.0, va[3];
 #pragma unroll
     for (int q = 0; q < 3; ++q) {
       const double v = U[(1 + q) * G.cells + idx] * rinv;
       k2 = fma(v, v, k2);
+      va[q] = fabs(v);
     }
     const double e = fma(U[4 * G.cells + idx], rinv, -0.5 * k2);
     double yr[NS];  // Y_s R_s
@@ -128,25 +56,30 @@ prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *_
         yr[i] = (1.0 - sum) * th.Rs[i];
         Rbar += yr[i];
       }
+    double A[6], B[4];  // mixture coefficients (a5 = enthalpy constant)
+#pragma unroll
+    for (int q = 0; q < 6; ++q) A[q] = 0.0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) B[q] = 0.0;
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+      if (s < N) {
+#pragma unroll
+        for (int q = 0; q < 6; ++q) A[q] = fma(yr[s], th.a[s][q], A[q]);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) B[q] = fma(yr[s], th.b[s][q], B[q]);
+      }
+    }
     double Tk = T[idx];
-    double esR[NS], cpm;
+    double cpm, Tc;
     bool fin = false, conv = false;
 #pragma unroll 1
     for (;;) {
-      const double Tc = fmin(fmax(Tk, th.Tlo), th.Thi);
-      double hm = 0.0;
-      cpm = 0.0;
-#pragma unroll
-      for (int s = 0; s < NS; ++s) {
-        if (s < N) {
-          double cpR, hR;
-          species_cp_h(th, s, Tk, Tc, cpR, hR);
-          hm = fma(yr[s], hR, hm);
-          cpm = fma(yr[s], cpR, cpm);
-          esR[s] = hR - Tk;  // e_s / R_s
-        }
-      }
+      Tc = fmin(fmax(Tk, th.Tlo), th.Thi);
+      cpm = fma(Tc, fma(Tc, fma(Tc, fma(Tc, A[4], A[3]), A[2]), A[1]), A[0]);
       if (fin) break;
+      const double hp = fma(Tc, fma(Tc, fma(Tc, fma(Tc, B[3], B[2]), B[1]), B[0]), A[0]);
+      const double hm = fma(cpm, Tk - Tc, fma(Tc, hp, A[5]));   // constant-cp continuation outside [Tlo, Thi] (R3)
       // Eq. 21: T <- T + (e - e(T)) / C_v(T)
       const double Tn = fma(e - fma(-Rbar, Tk, hm), xf_rcp(cpm - Rbar), Tk);
       ++it;
@@ -159,6 +92,13 @@ prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *_
     const double Gam = Rbar * iCv;
     const double cs = sqrt((1.0 + Gam) * pr * rinv);
     T[idx] = Tk;
+    if (S_out) {   // Eq. 17 / reading R9, interior cells only
+      double sc = 0.0;
+#pragma unroll
+      for (int q = 0; q < 3; ++q)
+        if (G.n[q] > 1) sc = fma(va[q] + cs, G.inv_d[q], sc);
+      if (interior && sc == sc) smax = sc;
+    }
     if (p_out) p_out[idx] = pr;
     if (c_out) c_out[idx] = cs;
     if (prim) {  // what the sweeps stage per cell: p, c, 1/rho, Gamma, chi_s
@@ -166,9 +106,19 @@ prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *_
       prim[G.cells + idx] = cs;
       prim[2 * G.cells + idx] = rinv;
       prim[3 * G.cells + idx] = Gam;
+      const double dTc = Tk - Tc;
+      const bool outside = __any_sync(__activemask(), dTc != 0.0);   // warp-uniform: cp_s only where it is needed
 #pragma unroll
-      for (int s = 0; s < NS; ++s)
-        if (s < N) prim[(4 + s) * G.cells + idx] = th.Rs[s] * fma(-Gam, esR[s], Tk);  // chi_s = R_s T - Gamma e_s
+      for (int s = 0; s < NS; ++s) {
+        if (s < N) {   // chi_s = R_s T - Gamma e_s,  e_s/R_s = h_s/R_s - T
+          const double *a = th.a[s];
+          const double *b = th.b[s];
+          const double hp = fma(Tc, fma(Tc, fma(Tc, fma(Tc, b[3], b[2]), b[1]), b[0]), a[0]);
+          double hR = fma(Tc, hp, a[5]);
+          if (outside) hR = fma(fma(Tc, fma(Tc, fma(Tc, fma(Tc, a[4], a[3]), a[2]), a[1]), a[0]), dTc, hR);
+          prim[(4 + s) * G.cells + idx] = th.Rs[s] * fma(-Gam, hR - Tk, Tk);
+        }
+      }
     }
     int flag = 0;
     if (!(rho > 0.0) || !(Tk > 0.0) || !(pr > 0.0)) flag |= XF_FLAG_NONPHYSICAL;
@@ -180,64 +130,10 @@ prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *_
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
     if ((threadIdx.x & 31) == 0) atomicAdd(itersum, (unsigned long long)v);
   }
-}
-
-// S = max over interior cells of sum_d (|u_d| + c)/dx_d.  Non-negative doubles order like their bit patterns,
-// so the grid-wide maximum is one 64-bit atomicMax per block.
-template <int N_T>
-__global__ void __launch_bounds__(256)
-wavespeed_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *__restrict__ U,
-                 double *__restrict__ T, double *__restrict__ S_dev, int *__restrict__ status) {
-  const int N = N_T > 0 ? N_T : th.N;
-  const long long interior = (long long)G.n[0] * G.n[1] * G.n[2];
-  double smax = 0.0;
-  for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < interior;
-       q += (long long)gridDim.x * blockDim.x) {
-    const int i = (int)(q % G.n[0]);
-    const long long r = q / G.n[0];
-    const int j = (int)(r % G.n[1]);
-    const int k = (int)(r / G.n[1]);
-    const long long idx = (long long)(k + G.g[2]) * G.st[2] + (long long)(j + G.g[1]) * G.st[1] + (i + G.g[0]);
-    CellState<N_T> S;
-    load_cell<N_T>(G, N, U, idx, S);
-    int it;
-    bool conv;
-    const double Tn = newton_T<N_T>(th, N, S, T[idx], it, conv);
-    const double Tc = fmin(fmax(Tn, th.Tlo), th.Thi);
-    double Rbar = 0.0, cpm = 0.0;
-#pragma unroll
-    for (int s = 0; s < CellState<N_T>::NS; ++s) {
-      if (s < N) {
-        double cpR, hR;
-        species_cp_h(th, s, Tn, Tc, cpR, hR);
-        const double yr = S.Y[s] * th.Rs[s];
-        Rbar += yr;
-        cpm = fma(yr, cpR, cpm);
-      }
-    }
-    const double Cv = cpm - Rbar;
-    const double pr = S.rho * Rbar * Tn;
-    const double Gam = Rbar / Cv;
-    const double cs = sqrt((1.0 + Gam) * pr * S.rinv);
-    T[idx] = Tn;
-    double s = 0.0;
-#pragma unroll
-    for (int d = 0; d < 3; ++d)
-      if (G.n[d] > 1) s = fma(fabs(S.vel[d]) + cs, G.inv_d[d], s);
-    int flag = 0;
-    if (!(S.rho > 0.0) || !(Tn > 0.0) || !(pr > 0.0)) flag |= XF_FLAG_NONPHYSICAL;
-    if (!conv) flag |= XF_FLAG_NOCONV;
-    if (flag) atomicOr(status, flag);
-    if (s == s) smax = fmax(smax, s);
-  }
-  for (int o = 16; o > 0; o >>= 1) smax = fmax(smax, __shfl_down_sync(0xffffffffu, smax, o));
-  __shared__ double wmax[8];
-  if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = smax;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    double m = wmax[0];
-    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) m = fmax(m, wmax[w]);
-    atomicMax(reinterpret_cast<unsigned long long *>(S_dev), (unsigned long long)__double_as_longlong(m));
+  if (S_out) {   // non-negative doubles order like their bit patterns: one 64-bit atomicMax per warp
+    for (int o = 16; o > 0; o >>= 1) smax = fmax(smax, __shfl_down_sync(0xffffffffu, smax, o));
+    if ((threadIdx.x & 31) == 0 && smax > 0.0)
+      atomicMax(reinterpret_cast<unsigned long long *>(S_out), (unsigned long long)__double_as_longlong(smax));
   }
 }
 
@@ -254,10 +150,11 @@ wavespeed_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const doub
   }
 
 int xf_launch_prim(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *prim, double *p,
-                   double *c, int *status, unsigned long long *itersum, cudaStream_t s) {
+                   double *c, int *status, unsigned long long *itersum, double *S_out, cudaStream_t s) {
+  if (S_out && cudaMemsetAsync(S_out, 0, sizeof(double), s) != cudaSuccess) return XF_ECUDA;
   const int threads = 128;
   const unsigned blocks = (unsigned)((G.cells + threads - 1) / threads);
-#define CALL(NT) prim_kernel<NT><<<blocks, threads, 0, s>>>(G, Th, U, T, prim, p, c, status, itersum)
+#define CALL(NT) prim_kernel<NT><<<blocks, threads, 0, s>>>(G, Th, U, T, prim, p, c, status, itersum, S_out)
   XF_DISPATCH_N(Th.N, CALL)
 #undef CALL
   return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
@@ -265,13 +162,5 @@ int xf_launch_prim(const XfGrid &G, const XfThermo &Th, const double *U, double 
 
 int xf_launch_wavespeed(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *S_dev, int *status,
                         cudaStream_t s) {
-  if (cudaMemsetAsync(S_dev, 0, sizeof(double), s) != cudaSuccess) return XF_ECUDA;
-  const int threads = 256;
-  const long long interior = (long long)G.n[0] * G.n[1] * G.n[2];
-  long long want = (interior + threads - 1) / threads;
-  const unsigned blocks = (unsigned)(want < 148 * 8 ? want : 148 * 8);
-#define CALL(NT) wavespeed_kernel<NT><<<blocks, threads, 0, s>>>(G, Th, U, T, S_dev, status)
-  XF_DISPATCH_N(Th.N, CALL)
-#undef CALL
-  return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
+  return xf_launch_prim(G, Th, U, T, nullptr, nullptr, nullptr, status, nullptr, S_dev, s);
 }

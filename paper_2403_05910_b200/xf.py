@@ -23,7 +23,8 @@ XF_MAX_SPECIES = 16
 # every symbol include/xf.h declares (tests check that the library exports all of them)
 ABI_SYMBOLS = (
     "xf_create", "xf_destroy", "xf_num_vars", "xf_padded_cells", "xf_rhs_workspace_bytes", "xf_workspace_bytes",
-    "xf_fill_ghosts", "xf_primitives", "xf_convective_rhs", "xf_rk3_step", "xf_rk3_step_cfl", "xf_max_wavespeed",
+    "xf_fill_ghosts", "xf_primitives", "xf_convective_rhs", "xf_rk3_step", "xf_rk3_step_cfl", "xf_step_cfl",
+    "xf_max_wavespeed",
     "xf_status", "xf_newton_mean_iterations", "xf_launch_count", "xf_convective_rhs_host", "xf_rk3_steps_host",
     "xf_probe_fp64_peak", "xf_strerror", "xf_timing_enable", "xf_timing_read",
 )
@@ -70,6 +71,7 @@ def lib() -> C.CDLL:
         L.xf_convective_rhs.argtypes = [ctx, dp, dp, dp, vp, vp]
         L.xf_rk3_step.argtypes = [ctx, dp, dp, C.c_double, vp, vp]
         L.xf_rk3_step_cfl.argtypes = [ctx, dp, dp, C.c_double, dp, vp, vp]
+        L.xf_step_cfl.argtypes = [ctx, dp, dp, C.c_double, dp, vp, vp]
         L.xf_max_wavespeed.argtypes = [ctx, dp, dp, dp, vp]
         L.xf_status.argtypes = [ctx, vp]
         L.xf_newton_mean_iterations.argtypes = [ctx, vp, C.POINTER(C.c_double)]
@@ -210,6 +212,11 @@ class Context:
         assert work.numel() * work.element_size() >= self.workspace_bytes
         _check(lib().xf_rk3_step_cfl(self._h, _ptr(U), _ptr(T), float(cfl), _ptr(S_dev), _ptr(work), _stream(stream)),
                "xf_rk3_step_cfl")
+
+    def xf_step_cfl(self, U, T, cfl: float, S_dev, work, stream=None) -> None:
+        assert work.numel() * work.element_size() >= self.workspace_bytes
+        _check(lib().xf_step_cfl(self._h, _ptr(U), _ptr(T), float(cfl), _ptr(S_dev), _ptr(work), _stream(stream)),
+               "xf_step_cfl")
 
     def xf_max_wavespeed(self, U, T, S_dev, stream=None) -> None:
         _check(lib().xf_max_wavespeed(self._h, _ptr(U), _ptr(T), _ptr(S_dev), _stream(stream)), "xf_max_wavespeed")

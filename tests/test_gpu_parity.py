@@ -275,6 +275,28 @@ def test_rk3_step_cfl_matches_host_dt():
     b.close()
 
 
+def test_step_cfl_matches_wavespeed_then_rk3():
+    """xf_step_cfl (S reduced inside the first stage's primitives kernel) == xf_max_wavespeed + xf_rk3_step_cfl."""
+    for shape, n in (((30, 22, 18), 4), ((64, 1, 1), 2), ((26, 31, 1), 10)):
+        w = wl.random_smooth_box(*shape, nspecies=n, seed=5)
+        a, b = _gpu(w), _gpu(w)
+        a.ctx.xf_max_wavespeed(a.U, a.T, a.S)
+        a.ctx.xf_rk3_step_cfl(a.U, a.T, w.cfl, a.S, a.work)
+        b.ctx.xf_step_cfl(b.U, b.T, w.cfl, b.S, b.work)
+        assert a.ctx.xf_status() == 0 and b.ctx.xf_status() == 0
+        assert float(a.S.item()) == float(b.S.item())
+        # not bitwise: in (a) the first stage's Newton iteration starts from the T xf_max_wavespeed left
+        ua, ub = w_interior(a.U, w), w_interior(b.U, w)
+        assert float((ua - ub).abs().max() / ua.abs().max()) < 1e-13
+        a.close()
+        b.close()
+
+
+def w_interior(U, w):
+    gx, gy, gz = (3 if w.nx > 1 else 0), (3 if w.ny > 1 else 0), (3 if w.nz > 1 else 0)
+    return U[:, gz:gz + w.nz, gy:gy + w.ny, gx:gx + w.nx]
+
+
 def test_host_entry_points_match_device_calls():
     w = wl.random_smooth_box(30, 14, 9, nspecies=4, seed=8)
     g = _gpu(w)
@@ -285,10 +307,9 @@ def test_host_entry_points_match_device_calls():
     assert np.array_equal(w.interior(rh), w.interior(r_dev))
     g.reset()
     t = 0.0
-    for _ in range(3):
-        S = g.max_wavespeed()
-        g.ctx.xf_rk3_step_cfl(g.U, g.T, 0.5, g.S, g.work)
-        t += 0.5 / S
+    for _ in range(3):                                        # the host call runs xf_step_cfl per step
+        g.ctx.xf_step_cfl(g.U, g.T, 0.5, g.S, g.work)
+        t += 0.5 / float(g.S.item())
     Uh, Th = w.U.copy(), w.T_guess.copy()
     t_host = g.ctx.xf_rk3_steps_host(Uh, Th, 0.5, 3)
     assert np.array_equal(w.interior(Uh), w.interior(g.host_U()))
