@@ -22,7 +22,7 @@ namespace xf {
 // with P0 = (s1 s2)^2, P1 = (s0 s2)^2, P2 = (s0 s1)^2, s_k = 4 (eps + beta_k): the Jiang-Shu weights
 // d_k/(eps+beta_k)^2 brought to a common denominator, so one reciprocal instead of four divisions.
 #ifndef XF_SPECIES_UNROLL
-#define XF_SPECIES_UNROLL 1
+#define XF_SPECIES_UNROLL 3   // measured: 1 (nothing to overlap) and 9 (instruction cache) are both slower
 #endif
 #define XF_PRAGMA(x) _Pragma(#x)
 #define XF_UNROLL(n) XF_PRAGMA(unroll n)
@@ -195,10 +195,12 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const d
 
   // ---- fields travelling with u: two shear fields, N-1 species fields.  alpha_m = V_m - C rho_m with
   //      C = Roe average of V/rho; L F_m = u_m alpha_m, so f+-_m = (u_m +- Lambda)/2 * alpha_m.
-#define XF_LINEAR_FIELD(VIDX, DEXPR, VNEXT)                                                            \
+  //      The stencil values of the NEXT field are loaded before the current one is reconstructed (software
+  //      pipeline): the emit is a store, no later load may be moved above it, and a warp issues in order.
+#define XF_LOAD_FIELD(VIDX, V) _Pragma("unroll") for (int m = 0; m < 6; ++m) V[m] = XS(VIDX, m);
+#define XF_LINEAR_FIELD(VIDX, V, DEXPR, VNEXT)                                                         \
   {                                                                                                    \
-    double V[6], fp[6], fm[6];                                                                         \
-    _Pragma("unroll") for (int m = 0; m < 6; ++m) V[m] = XS(VIDX, m);                                  \
+    double fp[6], fm[6];                                                                               \
     const double C = fma(oma, V[2], omb * V[3]);                                                       \
     _Pragma("unroll") for (int m = 0; m < 6; ++m) {                                                    \
       const double a = fma(-C, rho[m], V[m]);                                                          \
@@ -209,14 +211,31 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const d
     F4 = fma((DEXPR), g, F4);                                                                          \
     emit(VIDX, fma(C, s, g), VNEXT);                                                                   \
   }
-  XF_LINEAR_FIELD(1 + t1, C, 1 + t2)
-  XF_LINEAR_FIELD(1 + t2, C, N > 1 ? 5 : 4)
+  {
+    double Va[6], Vb[6];
+    XF_LOAD_FIELD(1 + t1, Va)
+    XF_LOAD_FIELD(1 + t2, Vb)
+    XF_LINEAR_FIELD(1 + t1, Va, C, 1 + t2)
+    double zn = 0.0;
+    if (N > 1) {
+      XF_LOAD_FIELD(5, Va)
+      zn = fma(oa, XA(1), ob * XB(1)) - chiN;
+    }
+    XF_LINEAR_FIELD(1 + t2, Vb, C, N > 1 ? 5 : 4)
 XF_UNROLL(XF_SPECIES_UNROLL)
-  for (int i = 0; i < N - 1; ++i) {
-    const double zeta = fma(oa, XA(1 + i), ob * XB(1 + i)) - chiN;
-    XF_LINEAR_FIELD(5 + i, -zeta * invG, i + 2 < N ? 6 + i : 4)
+    for (int i = 0; i < N - 1; ++i) {
+      double V[6];
+      _Pragma("unroll") for (int m = 0; m < 6; ++m) V[m] = Va[m];
+      const double zeta = zn;
+      if (i + 2 < N) {
+        XF_LOAD_FIELD(6 + i, Va)
+        zn = fma(oa, XA(2 + i), ob * XB(2 + i)) - chiN;
+      }
+      XF_LINEAR_FIELD(5 + i, V, -zeta * invG, i + 2 < N ? 6 + i : 4)
+    }
   }
 #undef XF_LINEAR_FIELD
+#undef XF_LOAD_FIELD
   emit(4, F4, -1);
 #undef XS
 #undef XA

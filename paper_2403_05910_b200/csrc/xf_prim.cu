@@ -132,7 +132,9 @@ prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *_
   }
   if (S_out) {   // non-negative doubles order like their bit patterns: one 64-bit atomicMax per warp
     for (int o = 16; o > 0; o >>= 1) smax = fmax(smax, __shfl_down_sync(0xffffffffu, smax, o));
-    if ((threadIdx.x & 31) == 0 && smax > 0.0)
+    // the running maximum only grows: a warp whose own maximum is not above it has nothing to add (a million
+    // atomics on one address would serialise in L2)
+    if ((threadIdx.x & 31) == 0 && smax > *reinterpret_cast<volatile double *>(S_out))
       atomicMax(reinterpret_cast<unsigned long long *>(S_out), (unsigned long long)__double_as_longlong(smax));
   }
 }

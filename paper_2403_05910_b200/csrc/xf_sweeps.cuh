@@ -270,7 +270,7 @@ __host__ __device__ inline size_t yz_smem_doubles(int N, int W) {   // ring(s), 
 //   * W COMPUTE warps (warp w = face row fc + w) run xf::face_flux back to back and nothing else;
 //   * W SERVICE warps keep the ring one chunk ahead (cp.async) and, concurrently with the next chunk's arithmetic,
 //     difference the fluxes of the chunk just finished and write the cells (Eq. 13, Eq. 16).
-// setmaxnreg moves registers from the service group (72) to the compute group (184): two blocks per SM.
+// setmaxnreg moves registers from the service group (88) to the compute group (168): two blocks per SM.
 // Named barriers (ids alternate with the chunk parity): RING_FULL  service -> compute  rows of chunk c landed
 //                                                        FLUX_READY compute -> service  fluxes of chunk c in fb
 //                                                        FB_EMPTY   service -> compute  fb of chunk c - 1 consumed
@@ -309,7 +309,12 @@ __device__ __forceinline__ void tma_load_row(unsigned dst, const void *tmap, int
 
 constexpr int BAR_RING_FULL = 1, BAR_FLUX_READY = 3, BAR_FB_EMPTY = 5;   // + chunk parity
 constexpr int BAR_SERVICE = 7;   // among the service warps: all have read U^s before any of them overwrites ring rows
-constexpr int WS_REGS_COMPUTE = 184, WS_REGS_SERVICE = 72;
+#ifndef XF_WS_RC
+#define XF_WS_RC 168   // 2 blocks x 128 threads x (168 + 88) registers = the SM's 64 K
+#define XF_WS_RS 88
+#define XF_WS_VB 7     // fields whose global operands a service lane keeps in flight together
+#endif
+constexpr int WS_REGS_COMPUTE = XF_WS_RC, WS_REGS_SERVICE = XF_WS_RS;
 
 struct FluxStoreWS {
   double *dst;   // fb + row * 32 + lane
@@ -476,7 +481,7 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
   auto write_cells = [&](int f) {                           // part 2: global operands, Eq. 16, stores
     if (!(f > f_begin && f <= f_end) || !lane_ok) return;
     const long long gi = colbase + (long long)(f + 2) * sst;
-    constexpr int VB = 4;                                   // fields per batch: all loads of a batch fly together
+    constexpr int VB = XF_WS_VB;                                   // fields per batch: all loads of a batch fly together
 #pragma unroll
     for (int v0 = 0; v0 < NVS; v0 += VB) {
       double a[VB], un[VB];
@@ -704,7 +709,7 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
   auto write_cells = [&](int fc) {
     long long gi;
     if (!cell_index(fc, gi)) return;
-    constexpr int VB = 4;
+    constexpr int VB = XF_WS_VB;
 #pragma unroll
     for (int v0 = 0; v0 < NVS; v0 += VB) {
       double a[VB], un[VB];
