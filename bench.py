@@ -166,7 +166,7 @@ def run_reference(args, rank: int, world: int) -> None:
     if rank != 0:
         return
     name = args.workload
-    grid = WORKLOADS[name][3]
+    grid = tuple(args.grid) if args.grid else WORKLOADS[name][3]
     w = make_workload(name, grid)
     sec = oracle_step_seconds(w, args.steps, args.warmup)
     value = w.interior_cells * 3 * args.steps / sec
@@ -187,6 +187,47 @@ def run_reference(args, rank: int, world: int) -> None:
 # ---------------------------------------------------------------------------------------------------------------
 # the B200 arm
 # ---------------------------------------------------------------------------------------------------------------
+class Ranks:
+    """The N > 1 plumbing of the bench: one process per GPU, independent replicas (the path has
+    no exchange step on one GPU), a barrier on both sides of the timed region and the MAX over ranks of the device
+    time.  backend "nccl" on the GPU box; the CPU test drives the same class over "gloo" with world_size 2."""
+
+    def __init__(self, world: int, backend: str = "nccl", device=None):
+        self.world, self.device, self.dist = world, device, None
+        if world > 1:
+            import torch.distributed as dist
+
+            if not dist.is_initialized():
+                kw = {"device_id": device} if backend == "nccl" and device is not None else {}
+                dist.init_process_group(backend, **kw)
+            self.dist = dist
+
+    def barrier(self) -> None:
+        import torch
+
+        if self.dist is not None:
+            self.dist.barrier()
+        if self.device is not None and self.device.type == "cuda":
+            torch.cuda.synchronize()
+
+    def max(self, x: float) -> float:
+        if self.dist is None:
+            return x
+        import torch
+
+        t = torch.tensor([x], dtype=torch.float64, device=self.device if self.device is not None else "cpu")
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def whole_job_value(self, cells_per_rank: int, rhs_per_step: int, ms_per_step_local: float) -> float:
+        """cell-updates/s of ALL ranks: every rank does the same work, the slowest rank sets the time."""
+        return cells_per_rank * rhs_per_step * self.world / (self.max(ms_per_step_local) * 1e-3)
+
+    def close(self) -> None:
+        if self.dist is not None and self.dist.is_initialized():
+            self.dist.destroy_process_group()
+
+
 def measured_peaks() -> dict:
     p = ROOT / "MEASURED_PEAKS.json"
     if p.exists():
@@ -212,23 +253,8 @@ def run_b200(args, rank: int, local_rank: int, world: int) -> None:
         raise RuntimeError("bench.py needs a CUDA device: the product has no CPU path")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-
-        dist.init_process_group("nccl", device_id=dev)
-
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def max_over_ranks(x: float) -> float:
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    ranks = Ranks(world, "nccl", dev)
+    barrier, max_over_ranks = ranks.barrier, ranks.max
 
     name = args.workload
     grid = tuple(args.grid) if args.grid else WORKLOADS[name][1]
@@ -280,7 +306,7 @@ def run_b200(args, rank: int, local_rank: int, world: int) -> None:
     newton_its = ctx.xf_newton_mean_iterations()
     del Tn
 
-    ms_per_step = ms_total / args.steps
+    ms_per_step = ms_total / args.steps                      # ms_total is already the max over ranks
     value = cells * 3 * world / (ms_per_step * 1e-3)
 
     # ---- roofline of the dominant kernel (per launch, CUDA events on the launching stream inside the timed region)
@@ -356,8 +382,7 @@ def run_b200(args, rank: int, local_rank: int, world: int) -> None:
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline(name)
         print(json.dumps(line), flush=True)
-    if dist is not None:
-        dist.destroy_process_group()
+    ranks.close()
 
 
 def main() -> None:

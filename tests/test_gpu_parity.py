@@ -380,3 +380,50 @@ def test_repeated_runs_are_bitwise_identical(shape):
         else:
             assert torch.equal(U, ref), f"run {rep} differs from run 0"
     g.close()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# BASELINE.json's full sizes, in the launch configuration bench.py times: one RHS of the whole field on the GPU,
+# the oracle recomputes sampled cells one by one (xo_rhs_cells: its own primitives for the 7-cell cross of every
+# direction, two face fluxes per direction)
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["config2", "config3", "config4"])
+def test_full_size_rhs_on_sampled_cells(oracle_mod, name):
+    w = {"config2": lambda: wl.config2_shock_bubble_2d(2048, 1024),
+         "config3": lambda: wl.config3_shock_bubble_3d(256),
+         "config4": lambda: wl.config4_shock_bubble_3d_10sp(512, 256, 256)}[name]()
+    g = _gpu(w)
+    r = g.rhs()                                               # [Nv, nzp, nyp, nxp], ghost entries zero
+    Ug = g.host_U()                                           # ghosts filled by the GPU
+    g.close()
+    orc = oracle_mod.Oracle.from_workload(w)
+    Uo = w.U.copy()
+    orc.fill_ghosts(Uo)
+    assert np.array_equal(Ug, Uo)                             # ghost fill: bit-exact at full size
+    nv = w.nvars
+    scale = np.abs(w.interior(r)).reshape(nv, -1).max(axis=1)
+    scale[1:4] = scale[1:4].max()                             # momentum components share their scale (R14)
+    scale[5:] = np.maximum(scale[5:], scale[0])               # a trace species is measured against the density row:
+    #   its flux differences carry the round-off of the O(1) characteristic variables they are assembled from
+    # samples: the cells with the largest |rhs| of the density equation (shock, bubble surface), a seeded uniform
+    # draw, and the domain corners / block-boundary neighbourhoods of the sweeps (i around multiples of 32 and 128)
+    rng = np.random.default_rng(wl.SEED_BASE + 99)
+    gz, gy, gx = (3 if w.nz > 1 else 0), (3 if w.ny > 1 else 0), (3 if w.nx > 1 else 0)
+    nzp, nyp, nxp = r.shape[1:]
+    rho_rhs = np.abs(w.interior(r)[0]).ravel()
+    top = np.argpartition(rho_rhs, -1500)[-1500:]
+    kk, jj, ii = np.unravel_index(top, (w.nz, w.ny, w.nx))
+    ks = [kk, rng.integers(0, w.nz, 2000), rng.integers(0, w.nz, 500)]
+    js = [jj, rng.integers(0, w.ny, 2000), rng.integers(0, w.ny, 500)]
+    edge = np.concatenate([np.arange(0, 4), np.arange(w.nx - 4, w.nx), 32 * rng.integers(1, w.nx // 32, 200) - 1,
+                           128 * rng.integers(1, max(w.nx // 128, 2), 200), rng.integers(0, w.nx, 92)])[:500] % w.nx
+    is_ = [ii, rng.integers(0, w.nx, 2000), edge]
+    k = np.concatenate(ks) + gz
+    j = np.concatenate(js) + gy
+    i = np.concatenate(is_) + gx
+    idx = (k.astype(np.int64) * nyp + j) * nxp + i
+    ro = orc.rhs_cells(Uo, w.T_guess, idx)                    # [samples, Nv]
+    assert orc.last_status == 0
+    rg = r.reshape(nv, -1)[:, idx].T
+    err = np.abs(rg - ro).max(axis=0) / scale
+    assert err.max() < RHS_TOL, err
