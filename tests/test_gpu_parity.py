@@ -7,6 +7,8 @@ components share one scale so that an identically zero component does not divide
 """
 from __future__ import annotations
 
+import os
+
 import numpy as np
 import pytest
 
@@ -427,3 +429,50 @@ def test_full_size_rhs_on_sampled_cells(oracle_mod, name):
     rg = r.reshape(nv, -1)[:, idx].T
     err = np.abs(rg - ro).max(axis=0) / scale
     assert err.max() < RHS_TOL, err
+
+
+@pytest.mark.skipif(os.environ.get("XF_FULL_CONFIG5") != "1",
+                    reason="3 min of host-side generation (94 M cells): set XF_FULL_CONFIG5=1; result in DESIGN.md section 8")
+def test_config5_full_size_subblock(oracle_mod):
+    """BASELINE.json configs[4] as stated: 640x384x384 periodic random states, 50 back-to-back RHS evaluations (status
+    only), then one RK3 step checked against the oracle on a seeded 64^3 sub-block (+9 cells of margin)."""
+    import torch
+
+    w = wl.config5_random_states()
+    g = _gpu(w)
+    out = torch.empty_like(g.U)
+    g.ctx.xf_convective_rhs(g.U, g.T, out, g.work)
+    Tconv = g.T.clone()
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(5)
+    Tg = Tconv * (1 + 0.02 * (2 * torch.rand(Tconv.shape, generator=gen, device="cuda", dtype=torch.float64) - 1))
+    for _ in range(50):
+        g.T.copy_(Tg)
+        g.ctx.xf_convective_rhs(g.U, g.T, out, g.work)
+    assert g.ctx.xf_status() == 0
+    g.T.copy_(Tg)
+    S = g.max_wavespeed()
+    dt = w.cfl / S
+    g.T.copy_(Tg)
+    g.step(dt)
+    assert g.ctx.xf_status() == 0
+    Ug = w.interior(g.host_U())
+    rng = np.random.default_rng(wl.SEED_BASE + 55)
+    origin = (int(rng.integers(0, w.nx)), int(rng.integers(0, w.ny)), int(rng.integers(0, w.nz)))
+    size, margin = 64, 9
+    w.T_guess = Tg.cpu().numpy()
+    sub = wl.periodic_subblock(w, origin, size, margin)
+    orc = oracle_mod.Oracle.from_workload(sub)
+    Uo, To = sub.U.copy(), sub.T_guess.copy()
+    orc.rk3_step(Uo, To, dt)
+    inner_o = sub.interior(Uo)[:, margin:margin + size, margin:margin + size, margin:margin + size]
+    ix = (np.arange(size) + origin[0]) % w.nx
+    iy = (np.arange(size) + origin[1]) % w.ny
+    iz = (np.arange(size) + origin[2]) % w.nz
+    inner_g = Ug[:, iz][:, :, iy][:, :, :, ix]
+    nv = w.nvars
+    num = np.abs(inner_g - inner_o).reshape(nv, -1).max(axis=1)
+    den = np.abs(inner_o).reshape(nv, -1).max(axis=1)
+    den[1:4] = np.abs(inner_o[0]).max() * S * w.dx
+    assert (num / den).max() < STEPS_TOL
+    g.close()
