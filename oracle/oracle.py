@@ -23,7 +23,8 @@ class OConfig(C.Structure):
         ("W", C.c_double * MAXN), ("a", (C.c_double * 7) * MAXN),
         ("Tlo", C.c_double), ("Thi", C.c_double),
         ("bc", C.c_int * 6), ("bc_state", (C.c_double * MAXNV) * 6),
-        ("rtol", C.c_double), ("maxit", C.c_int), ("ideal_weights", C.c_int),
+        ("rtol", C.c_double), ("maxit", C.c_int), ("ideal_weights", C.c_int), ("viscosity", C.c_int),
+        ("lam_glob", (C.c_double * 3) * 3),
     ]
 
 
@@ -103,7 +104,7 @@ class Oracle:
     """One oracle context: grid, species table and boundary data (mirrors xf_config of include/xf.h)."""
 
     def __init__(self, nx, ny, nz, dx, dy, dz, W, nasa7, Ru, Tlo, Thi, bc=(0,) * 6, bc_state=None,
-                 rtol: float = 1e-13, maxit: int = 50, ideal_weights: bool = False):
+                 rtol: float = 1e-13, maxit: int = 50, ideal_weights: bool = False, viscosity: int = 0):
         W = np.asarray(W, dtype=np.float64)
         nasa7 = np.asarray(nasa7, dtype=np.float64)
         n = W.shape[0]
@@ -125,6 +126,7 @@ class Oracle:
                 for v in range(n + 4):
                     cfg.bc_state[q][v] = bs[q, v]
         cfg.rtol, cfg.maxit, cfg.ideal_weights = float(rtol), int(maxit), int(ideal_weights)
+        cfg.viscosity = int(viscosity)   # 0 LLF, 1 ROE, 2 GLF (xf_oracle.h)
         self.cfg = cfg
         self.N = n
         self.Nv = n + 4

@@ -276,8 +276,8 @@ double xo_weno5(const double v[5], int ideal_weights) {
 /* ------------------------------------------------------------------------------------------------------------ */
 int xo_face_flux(const xo_config *c, int d, const double *Ust, const xo_prim *Pst, double *Fhat) {
   const int Nv = c->N + 4;
-  double L[XO_MAXNV * XO_MAXNV], R[XO_MAXNV * XO_MAXNV];
-  int status = xo_eigensystem(c, &Pst[2], &Pst[3], d, L, R, NULL);
+  double L[XO_MAXNV * XO_MAXNV], R[XO_MAXNV * XO_MAXNV], roe[6];
+  int status = xo_eigensystem(c, &Pst[2], &Pst[3], d, L, R, roe);
 
   double aF[6][XO_MAXNV], aU[6][XO_MAXNV], lam[6][3];
   for (int m = 0; m < 6; ++m) {
@@ -299,8 +299,14 @@ int xo_face_flux(const xo_config *c, int d, const double *Ust, const xo_prim *Ps
   double g[XO_MAXNV];
   for (int n = 0; n < Nv; ++n) {
     const int kind = n == 0 ? 0 : (n == Nv - 1 ? 2 : 1);
-    double Lam = 0.0;                        /* LLF: max over the 6 stencil cells, factor 1 */
-    for (int m = 0; m < 6; ++m) Lam = fmax(Lam, fabs(lam[m][kind]));
+    double Lam = 0.0;
+    if (c->viscosity == XO_VISC_ROE) {       /* |lambda_n| of the Roe-averaged state: u~_d -+ c~ (roe[5] = c~) */
+      Lam = fabs(roe[d] + (kind - 1) * roe[5]);
+    } else if (c->viscosity == XO_VISC_GLF) {
+      Lam = c->lam_glob[d][kind];            /* global maximum, set by the caller */
+    } else {                                 /* LLF: max over the 6 stencil cells, factor 1 */
+      for (int m = 0; m < 6; ++m) Lam = fmax(Lam, fabs(lam[m][kind]));
+    }
     double fp[6], fm[6];
     for (int m = 0; m < 6; ++m) {            /* Eq. 14 */
       fp[m] = 0.5 * (aF[m][n] + Lam * aU[m][n]);
@@ -379,13 +385,36 @@ static void pencil_prims(const xo_config *c, const double *U, const double *T, l
 }
 
 /* U must have its ghosts filled; T: in guess, out converged temperature (whole padded field) */
-int xo_rhs_nofill(const xo_config *c, const double *U, double *T, double *rhs) {
+/* GLF: max over all padded cells (ghosts filled) of |u_d - c|, |u_d|, |u_d + c| per direction, from each cell's own
+ * primitives at the T guess given */
+static void global_wavespeeds(const xo_config *c, const double *U, const double *T, double lam[3][3]) {
+  const long cells = xo_padded_cells(c);
+  const int Nv = c->N + 4;
+  for (int d = 0; d < 3; ++d)
+    for (int k = 0; k < 3; ++k) lam[d][k] = 0.0;
+  for (long id = 0; id < cells; ++id) {
+    double Uc[XO_MAXNV];
+    xo_prim P;
+    for (int v = 0; v < Nv; ++v) Uc[v] = U[(long)v * cells + id];
+    xo_cell_primitives(c, Uc, T[id], &P);
+    for (int d = 0; d < 3; ++d) {
+      lam[d][0] = fmax(lam[d][0], fabs(P.vel[d] - P.c));
+      lam[d][1] = fmax(lam[d][1], fabs(P.vel[d]));
+      lam[d][2] = fmax(lam[d][2], fabs(P.vel[d] + P.c));
+    }
+  }
+}
+
+int xo_rhs_nofill(const xo_config *c_in, const double *U, double *T, double *rhs) {
+  xo_config cc = *c_in;
+  const xo_config *c = &cc;
   const int Nv = c->N + 4;
   int np[3], n[3], g[3];
   long st[3];
   grid(c, np, n, g, st);
   const long cells = xo_padded_cells(c);
   int status = xo_primitives(c, U, T, NULL, NULL, NULL);   /* "after updating the primitive variables" PAPER.md:411 */
+  if (c->viscosity == XO_VISC_GLF) global_wavespeeds(c, U, T, cc.lam_glob);
   memset(rhs, 0, sizeof(double) * Nv * cells);
   const double dxs[3] = {c->dx, c->dy, c->dz};
   for (int d = 0; d < 3; ++d) {
@@ -427,8 +456,11 @@ int xo_rhs(const xo_config *c, double *U, double *T, double *rhs) {
 /* rhs at a list of sampled interior cells, each computed on its own from U (ghosts filled) and the T guess:
  * primitives by Newton for the 7-cell cross of every direction, two faces per direction.  Used for parity at
  * sizes where the whole-field oracle would take too long. rhs_out[q][v]. */
-int xo_rhs_cells(const xo_config *c, const double *U, const double *Tguess, long ncells, const long *idx,
+int xo_rhs_cells(const xo_config *c_in, const double *U, const double *Tguess, long ncells, const long *idx,
                  double *rhs_out) {
+  xo_config cc = *c_in;
+  const xo_config *c = &cc;
+  if (c->viscosity == XO_VISC_GLF) global_wavespeeds(c, U, Tguess, cc.lam_glob);
   const int Nv = c->N + 4;
   int np[3], n[3], g[3];
   long st[3];

@@ -49,7 +49,13 @@ typedef struct {
   double rtol;                /* Newton |dT| <= rtol |T|, 1e-13                                               */
   int maxit;                  /* 50                                                                           */
   int ideal_weights;          /* test switch: WENO5 with the linear weights               */
+  int viscosity;              /* artificial viscosity of Eq. 14 (options PAPER.md:374):          */
+                              /*   0 LLF: per field, max over the six stencil cells of |lambda_n| (reading R8)  */
+                              /*   1 ROE: |lambda_n| of the Roe-averaged face state, no maximum                 */
+                              /*   2 GLF: per field and direction, max of |lambda_n| over ALL padded cells      */
+  double lam_glob[3][3];      /* GLF maxima [direction][u-c, u, u+c]; filled by the residual routines           */
 } xo_config;
+enum { XO_VISC_LLF = 0, XO_VISC_ROE = 1, XO_VISC_GLF = 2 };
 
 /* all primitive quantities of one cell (C2) */
 typedef struct {
