@@ -61,7 +61,15 @@ typedef struct {
   double newton_rtol;      /* |dT| <= rtol |T|; 0 -> 1e-13 (reading R4)                                         */
   int newton_maxit;        /* 0 -> 50                                                                           */
   int device;              /* CUDA ordinal                                                                      */
+  int viscosity;           /* XF_VISC_*: the artificial viscosity Lambda~ of Eq. 14 (options 374)  */
 } xf_config;
+
+/* Lambda~_n of the flux splitting f+- = (L F +- Lambda~ L U)/2, per characteristic field n:
+ *   LLF  max over the six stencil cells of |lambda_n| of each cell's own state (reading R8; the default)
+ *   ROE  |lambda_n| of the Roe-averaged face state (u~_d - c~, u~_d, u~_d + c~), no maximum
+ *   GLF  max of |lambda_n| over ALL padded cells, per direction, reduced inside the primitives kernel of the same
+ *        residual evaluation (ghosts filled) */
+enum { XF_VISC_LLF = 0, XF_VISC_ROE = 1, XF_VISC_GLF = 2 };
 
 /* Create a context: validates cfg, copies every host table, uploads boundary states.  Synchronous. */
 int xf_create(xf_ctx **out, const xf_config *cfg);

@@ -22,6 +22,8 @@ struct xf_ctx {
   unsigned long long *itersum_dev;    // Newton iteration counter of the last xf_primitives launch
   double *bc_state_dev;               // [6][XF_MAXNV]
   double *S_dev;                      // max wave speed scalar used by the host-buffer entry points
+  double *lam_glob_dev;               // GLF: [3][3] global maxima of the current residual evaluation
+  int visc;                           // XF_VISC_*
   long launches;
   // lazily allocated device mirrors for the *_host entry points
   double *hU, *hT, *hR;
@@ -94,7 +96,8 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
   double *prim = static_cast<double *>(work);  // p, c, 1/rho, Gamma, chi_1..chi_N
   {
     Timed t(c, XF_K_PRIM, s);
-    rc = xf_launch_prim(c->G, c->Th, U, T, prim, nullptr, nullptr, c->status_dev, nullptr, S_out, s);
+    rc = xf_launch_prim(c->G, c->Th, U, T, prim, nullptr, nullptr, c->status_dev, nullptr, S_out,
+                        c->visc == XF_VISC_GLF ? c->lam_glob_dev : nullptr, s);
   }
   ++c->launches;
   if (rc != XF_OK) return rc;
@@ -115,6 +118,8 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
       E.acc = acc;
       E.out = acc;
     }
+    E.visc = c->visc;
+    E.lam_glob = c->lam_glob_dev;
     Timed t(c, XF_K_SWEEP_X + d, s);
     if (d == 0) rc = xf_launch_sweep_x(c->G, c->N, U, prim, E, c->status_dev, s);
     else if (d == 1) rc = xf_launch_sweep_y(c->G, c->N, U, prim, E, c->status_dev, s);
@@ -188,6 +193,7 @@ int xf_create(xf_ctx **out, const xf_config *cfg) {
   for (int s = 0; s < N; ++s)
     if (!(cfg->W[s] > 0.0)) return XF_EINVAL;
   if (n[0] == 1 && n[1] == 1 && n[2] == 1) return XF_EINVAL;
+  if (cfg->viscosity < XF_VISC_LLF || cfg->viscosity > XF_VISC_GLF) return XF_EINVAL;
   if (n[1] > 65535 || n[2] > 65535) return XF_EINVAL;  // they index the y dimension of the y/z sweep grids
 
   int ndev = 0;
@@ -201,6 +207,7 @@ int xf_create(xf_ctx **out, const xf_config *cfg) {
   c->N = N;
   c->Nv = N + 4;
   c->device = cfg->device;
+  c->visc = cfg->viscosity;
   XfGrid &G = c->G;
   for (int d = 0; d < 3; ++d) {
     G.n[d] = n[d];
@@ -230,7 +237,8 @@ int xf_create(xf_ctx **out, const xf_config *cfg) {
   bool ok = cudaMalloc(&c->status_dev, sizeof(int)) == cudaSuccess &&
             cudaMalloc(&c->itersum_dev, sizeof(unsigned long long)) == cudaSuccess &&
             cudaMalloc(&c->bc_state_dev, sizeof(double) * 6 * XF_MAXNV) == cudaSuccess &&
-            cudaMalloc(&c->S_dev, sizeof(double)) == cudaSuccess;
+            cudaMalloc(&c->S_dev, sizeof(double)) == cudaSuccess &&
+            cudaMalloc(&c->lam_glob_dev, 9 * sizeof(double)) == cudaSuccess;
   if (ok) {
     double bs[6 * XF_MAXNV];
     memset(bs, 0, sizeof(bs));
@@ -257,6 +265,7 @@ int xf_destroy(xf_ctx *c) {
   cudaFree(c->itersum_dev);
   cudaFree(c->bc_state_dev);
   cudaFree(c->S_dev);
+  cudaFree(c->lam_glob_dev);
   cudaFree(c->hU);
   cudaFree(c->hT);
   cudaFree(c->hR);
@@ -287,7 +296,7 @@ int xf_primitives(xf_ctx *c, const double *U, double *T, double *p, double *cs, 
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (cudaMemsetAsync(c->itersum_dev, 0, sizeof(unsigned long long), s) != cudaSuccess) return XF_ECUDA;
   ++c->launches;
-  return xf_launch_prim(c->G, c->Th, U, T, nullptr, p, cs, c->status_dev, c->itersum_dev, nullptr, s);
+  return xf_launch_prim(c->G, c->Th, U, T, nullptr, p, cs, c->status_dev, c->itersum_dev, nullptr, nullptr, s);
 }
 
 int xf_convective_rhs(xf_ctx *c, double *U, double *T, double *rhs, void *work, void *stream) {

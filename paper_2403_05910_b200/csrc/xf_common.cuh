@@ -51,14 +51,18 @@ struct XfEpilogue {
   const double *acc;  // partial rhs of earlier sweeps [Nv][padded]
   const double *Un;   // U^n  [Nv][padded] (mode 2)
   double *out;        // rhs or U^{s+1} [Nv][padded]
+  int visc;           // XF_VISC_*: Lambda~ of Eq. 14
+  const double *lam_glob;  // GLF: [direction][u-c, u, u+c] global maxima on the device
 };
 
 // launch helpers implemented per translation unit
 // prim: the N + 4 workspace fields p, c, 1/rho, Gamma, chi_1..chi_N ([field][padded cells]); NULL = do
 // not store them (xf_primitives), p_out / c_out: optional separate copies of p and c for the caller.
 // S_out (may be NULL): max over INTERIOR cells of sum_d (|u_d| + c)/dx_d, reduced with atomicMax into a zeroed double.
+// lam_glob (may be NULL; GLF): [3][3] maxima over ALL cells the launch visits of |u_d - c|, |u_d|, |u_d + c|.
 int xf_launch_prim(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *prim, double *p_out,
-                   double *c_out, int *status, unsigned long long *itersum, double *S_out, cudaStream_t s);
+                   double *c_out, int *status, unsigned long long *itersum, double *S_out, double *lam_glob,
+                   cudaStream_t s);
 int xf_launch_wavespeed(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *S_dev, int *status,
                         cudaStream_t s);
 int xf_launch_ghosts(const XfGrid &G, int Nv, const XfBc &bc, const double *bc_state_dev, double *U, cudaStream_t s,

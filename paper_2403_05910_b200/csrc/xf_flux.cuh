@@ -70,6 +70,7 @@ __host__ __device__ constexpr int nprimfields(int N) { return N + 4; }
 // Numerical flux at one face.  sm: staged fields, field f of stencil cell m at sm[f*FS + o[m]] (m = 0..5 <-> i-2..i+3;
 // the face lies between m = 2 and m = 3).  emit(v, Fhat_v, vnext) is called once per component, in the order
 // 0, 1+nd, 1+t1, 1+t2, 5, ..., Nv-1, 4 (vnext = the component that follows, -1 after the last).
+// visc: XF_VISC_* (include/xf.h); lamg: this direction's three global maxima (GLF only).
 // Returns false if the Roe-averaged c~^2 is not positive.
 // The fields needed only at the two cells next to the face (Gamma, chi_1..chi_N) are read through a second
 // accessor: field g (0 = Gamma, 1 + s = chi_s) of the cell below / above the face at ss[g*SS + s2] / ss[g*SS + s3],
@@ -79,7 +80,7 @@ __host__ __device__ constexpr int nprimfields(int N) { return N + 4; }
 template <int DIR, class Emit>
 __device__ __forceinline__ bool face_flux(const int N, const double *sm, const double *sp, const int FS,
                                           const int (&o)[6], const double *ss, const int SS, const int s2,
-                                          const int s3, Emit &emit) {
+                                          const int s3, const int visc, const double *__restrict__ lamg, Emit &emit) {
   constexpr int nd = Axes<DIR>::nd, t1 = Axes<DIR>::t1, t2 = Axes<DIR>::t2;
   
 #define XS(f, m) sm[(f) * FS + o[m]]
@@ -138,12 +139,23 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const d
     nuU[m] = fma(-ut[nd], rho[m], mn);
     ud[m] = mn * XRI(m);
     const double cm = XC(m);
-    lam_m = fmax(lam_m, fabs(ud[m] - cm));
-    lam_0 = fmax(lam_0, fabs(ud[m]));
-    lam_p = fmax(lam_p, fabs(ud[m] + cm));
+    if (visc == XF_VISC_LLF) {
+      lam_m = fmax(lam_m, fabs(ud[m] - cm));
+      lam_0 = fmax(lam_0, fabs(ud[m]));
+      lam_p = fmax(lam_p, fabs(ud[m] + cm));
+    }
     const double ph = 0.5 * XP(m) * h;             // p_m / (4 c~^2)
     qp[m] = Gt * (ud[m] - ut[nd]) * ph;                // pressure terms of L F_m
     rp[m] = ct * ph;
+  }
+  if (visc == XF_VISC_ROE) {          // |lambda_n| of the Roe-averaged state (warp-uniform branch)
+    lam_m = fabs(ut[nd] - ct);
+    lam_0 = fabs(ut[nd]);
+    lam_p = fabs(ut[nd] + ct);
+  } else if (visc == XF_VISC_GLF) {   // global maxima of this direction, left by the primitives kernel
+    lam_m = lamg[0];
+    lam_0 = lamg[1];
+    lam_p = lamg[2];
   }
 
   // ---- acoustic (u-c), entropy (u) and acoustic (u+c) fields

@@ -13,11 +13,13 @@ template <int N_T>
 __global__ void __launch_bounds__(128, 6)
 prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *__restrict__ U, double *__restrict__ T,
             double *__restrict__ prim, double *__restrict__ p_out, double *__restrict__ c_out,
-            int *__restrict__ status, unsigned long long *__restrict__ itersum, double *__restrict__ S_out) {
+            int *__restrict__ status, unsigned long long *__restrict__ itersum, double *__restrict__ S_out,
+            double *__restrict__ lam_glob) {
   constexpr int NS = N_T > 0 ? N_T : XF_MAXN;
   const int N = N_T > 0 ? N_T : th.N;
   const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   int it = 0;
+  double lg[9] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
   double smax = 0.0;   // this cell's sum_d (|u_d| + c)/dx_d if it is an interior cell and S_out is wanted
   bool interior = true;
   if (S_out && idx < G.cells) {
@@ -31,12 +33,13 @@ prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *_
   if (idx < G.cells && (interior || prim)) {
     const double rho = U[idx];
     const double rinv = xf_rcp(rho);
-    double k2 = 0.0, va[3];
+    double k2 = 0.0, va[3], vs[3];
 #pragma unroll
     for (int q = 0; q < 3; ++q) {
       const double v = U[(1 + q) * G.cells + idx] * rinv;
       k2 = fma(v, v, k2);
       va[q] = fabs(v);
+      vs[q] = v;
     }
     const double e = fma(U[4 * G.cells + idx], rinv, -0.5 * k2);
     double yr[NS];  // Y_s R_s
@@ -99,6 +102,14 @@ prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *_
         if (G.n[q] > 1) sc = fma(va[q] + cs, G.inv_d[q], sc);
       if (interior && sc == sc) smax = sc;
     }
+    if (lam_glob) {   // GLF (include/xf.h): this cell's |u_d - c|, |u_d|, |u_d + c|
+#pragma unroll
+      for (int q = 0; q < 3; ++q) {
+        lg[3 * q] = fabs(vs[q] - cs);
+        lg[3 * q + 1] = va[q];
+        lg[3 * q + 2] = fabs(vs[q] + cs);
+      }
+    }
     if (p_out) p_out[idx] = pr;
     if (c_out) c_out[idx] = cs;
     if (prim) {  // what the sweeps stage per cell: p, c, 1/rho, Gamma, chi_s
@@ -130,6 +141,15 @@ prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *_
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
     if ((threadIdx.x & 31) == 0) atomicAdd(itersum, (unsigned long long)v);
   }
+  if (lam_glob) {   // uniform branch; same reduction as S below, nine values
+#pragma unroll
+    for (int q = 0; q < 9; ++q) {
+      double v = lg[q] == lg[q] ? lg[q] : 0.0;
+      for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+      if ((threadIdx.x & 31) == 0 && v > *reinterpret_cast<volatile double *>(lam_glob + q))
+        atomicMax(reinterpret_cast<unsigned long long *>(lam_glob + q), (unsigned long long)__double_as_longlong(v));
+    }
+  }
   if (S_out) {   // non-negative doubles order like their bit patterns: one 64-bit atomicMax per warp
     for (int o = 16; o > 0; o >>= 1) smax = fmax(smax, __shfl_down_sync(0xffffffffu, smax, o));
     // the running maximum only grows: a warp whose own maximum is not above it has nothing to add (a million
@@ -152,11 +172,13 @@ prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *_
   }
 
 int xf_launch_prim(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *prim, double *p,
-                   double *c, int *status, unsigned long long *itersum, double *S_out, cudaStream_t s) {
+                   double *c, int *status, unsigned long long *itersum, double *S_out, double *lam_glob,
+                   cudaStream_t s) {
   if (S_out && cudaMemsetAsync(S_out, 0, sizeof(double), s) != cudaSuccess) return XF_ECUDA;
+  if (lam_glob && cudaMemsetAsync(lam_glob, 0, 9 * sizeof(double), s) != cudaSuccess) return XF_ECUDA;
   const int threads = 128;
   const unsigned blocks = (unsigned)((G.cells + threads - 1) / threads);
-#define CALL(NT) prim_kernel<NT><<<blocks, threads, 0, s>>>(G, Th, U, T, prim, p, c, status, itersum, S_out)
+#define CALL(NT) prim_kernel<NT><<<blocks, threads, 0, s>>>(G, Th, U, T, prim, p, c, status, itersum, S_out, lam_glob)
   XF_DISPATCH_N(Th.N, CALL)
 #undef CALL
   return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
@@ -164,5 +186,5 @@ int xf_launch_prim(const XfGrid &G, const XfThermo &Th, const double *U, double 
 
 int xf_launch_wavespeed(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *S_dev, int *status,
                         cudaStream_t s) {
-  return xf_launch_prim(G, Th, U, T, nullptr, nullptr, nullptr, status, nullptr, S_dev, s);
+  return xf_launch_prim(G, Th, U, T, nullptr, nullptr, nullptr, status, nullptr, S_dev, nullptr, s);
 }

@@ -219,7 +219,7 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
     W.carry_rd = carry + par * Nv * LI;
     W.carry_wr = carry + (par ^ 1) * Nv * LI;
     W.preload(0);
-    const bool c2ok = face_flux<DIR>(N, sm, sm + Nv * FS, FS, o, sm + (Nv + 3) * FS, FS, o[2], o[3], W);
+    const bool c2ok = face_flux<DIR>(N, sm, sm + Nv * FS, FS, o, sm + (Nv + 3) * FS, FS, o[2], o[3], E.visc, E.lam_glob + 3 * DIR, W);
     bad = bad || (!c2ok && lane_ok && f <= f_end);
     __syncwarp();         // all lanes are done with the rows the next iteration's prefetch overwrites
     if (PF < LJ) {        // the remaining LJ - PF rows of the next chunk go where this chunk's first rows were
@@ -404,7 +404,7 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
       asm volatile("" : "+r"(s2), "+r"(s3));
       if (f <= f_end) {                                     // warp-uniform
         FluxStoreWS st{fb + (w + 1) * 32 + lane, FBS, first ? -1 : BAR_FB_EMPTY + par, NT};
-        const bool c2ok = face_flux<DIR>(N, sm, smp, FS, o, sms, FS, s2, s3, st);
+        const bool c2ok = face_flux<DIR>(N, sm, smp, FS, o, sms, FS, s2, s3, E.visc, E.lam_glob + 3 * DIR, st);
         bad = bad || (!c2ok && lane_ok);
       } else if (!first) {
         named_sync(BAR_FB_EMPTY + par, NT);                 // keep the barrier counts whole
@@ -644,7 +644,7 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
       for (int m = 0; m < 6; ++m) o[m] = u + delta + m;
       // every lane of the block passes the same barriers; lanes past f_end compute on staged (valid or zero) data
       FluxStoreWS fsw{fb + u + 1, XW_FBW, first ? -1 : BAR_FB_EMPTY + par, NT};
-      const bool c2ok = face_flux<0>(N, st, st + OFFP, FS, o, st + OFFS, FS, o[2], o[3], fsw);
+      const bool c2ok = face_flux<0>(N, st, st + OFFP, FS, o, st + OFFS, FS, o[2], o[3], E.visc, E.lam_glob, fsw);
       {
         const int ia = (f - 1 + G.np[0]) % G.np[0], ib = f % G.np[0];
         const bool used = f <= f_end && ((ia >= G.g[0] && ia < G.g[0] + G.n[0]) || (ib >= G.g[0] && ib < G.g[0] + G.n[0]));

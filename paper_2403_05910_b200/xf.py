@@ -18,6 +18,7 @@ LIB_PATH = _HERE / "libxf.so"
 
 XF_OK, XF_EINVAL, XF_ECUDA, XF_ENOMEM, XF_ENONPHYSICAL, XF_ENOCONV = 0, -1, -2, -3, -4, -5
 XF_BC_PERIODIC, XF_BC_TRANSMISSIVE, XF_BC_REFLECTIVE, XF_BC_DIRICHLET = 0, 1, 2, 3
+XF_VISC_LLF, XF_VISC_ROE, XF_VISC_GLF = 0, 1, 2
 XF_MAX_SPECIES = 16
 
 # every symbol include/xf.h declares (tests check that the library exports all of them)
@@ -39,7 +40,7 @@ class XfConfig(C.Structure):
         ("W", C.POINTER(C.c_double)), ("nasa7", C.POINTER(C.c_double)),
         ("Tlo", C.c_double), ("Thi", C.c_double),
         ("bc", C.c_int * 6), ("bc_state", C.POINTER(C.c_double)),
-        ("newton_rtol", C.c_double), ("newton_maxit", C.c_int), ("device", C.c_int),
+        ("newton_rtol", C.c_double), ("newton_maxit", C.c_int), ("device", C.c_int), ("viscosity", C.c_int),
     ]
 
 
@@ -131,7 +132,7 @@ class Context:
 
     def __init__(self, nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, W: Sequence[float], nasa7, Ru: float,
                  Tlo: float, Thi: float, bc=(0,) * 6, bc_state=None, newton_rtol: float = 0.0, newton_maxit: int = 0,
-                 device: int = 0):
+                 device: int = 0, viscosity: int = XF_VISC_LLF):
         W = np.ascontiguousarray(W, dtype=np.float64)
         nasa7 = np.ascontiguousarray(nasa7, dtype=np.float64)
         n = int(W.shape[0])
@@ -151,6 +152,7 @@ class Context:
             assert bs.shape == (6, n + 4)
             cfg.bc_state = bs.ctypes.data_as(C.POINTER(C.c_double))
         cfg.newton_rtol, cfg.newton_maxit, cfg.device = float(newton_rtol), int(newton_maxit), int(device)
+        cfg.viscosity = int(viscosity)
         self._h = C.c_void_p()
         _check(lib().xf_create(C.byref(self._h), C.byref(cfg)), "xf_create")
         self.device = int(device)

@@ -476,3 +476,40 @@ def test_config5_full_size_subblock(oracle_mod):
     den[1:4] = np.abs(inner_o[0]).max() * S * w.dx
     assert (num / den).max() < STEPS_TOL
     g.close()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# ROE and GLF artificial viscosity (include/xf.h XF_VISC_*): same bar as LLF
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("visc", [1, 2])
+@pytest.mark.parametrize("shape,n,bc", [((400, 1, 1), 1, (0,) * 6), ((150, 37, 1), 3, (3, 1, 2, 2, 0, 0)),
+                                         ((45, 19, 23), 4, (3, 1, 0, 0, 0, 0)), ((70, 9, 8), 10, (3, 1, 2, 2, 2, 2)),
+                                         ((20, 18, 40), 7, (1, 2, 2, 1, 0, 0))])
+def test_rhs_parity_viscosity_variants(oracle_mod, visc, shape, n, bc):
+    w = wl.random_smooth_box(*shape, nspecies=n, seed=2000 + n + shape[0], bc=bc)
+    orc = oracle_mod.Oracle.from_workload(w, viscosity=visc)
+    ro = orc.rhs(w.U.copy(), w.T_guess.copy())
+    assert orc.last_status == 0
+    g = _gpu(w, viscosity=visc)
+    err = field_err(w.interior(g.rhs()), w.interior(ro))
+    assert err.max() < RHS_TOL, err
+    g.close()
+
+
+@pytest.mark.parametrize("visc", [1, 2])
+def test_shock_tube_and_bubble_steps_viscosity_variants(oracle_mod, visc):
+    for w, steps in ((wl.config1_shock_tube(), 100), (wl.config3_shock_bubble_3d(32), 12)):
+        orc = oracle_mod.Oracle.from_workload(w, viscosity=visc)
+        Uo, To = w.U.copy(), w.T_guess.copy()
+        g = _gpu(w, viscosity=visc)
+        worst = 0.0
+        for _ in range(steps):
+            So = orc.max_wavespeed(Uo, To)
+            dt = w.cfl / So
+            assert orc.rk3_step(Uo, To, dt) == 0
+            g.step(dt)
+            cmax = So * min(w.dx, w.dy, w.dz)
+            worst = max(worst, state_err(w, g.host_U(), Uo, cmax).max())
+        assert g.ctx.xf_status() == 0
+        assert worst < STEPS_TOL, worst
+        g.close()
