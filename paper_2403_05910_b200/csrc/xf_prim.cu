@@ -141,14 +141,18 @@ prim_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const double *_
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
     if ((threadIdx.x & 31) == 0) atomicAdd(itersum, (unsigned long long)v);
   }
-  if (lam_glob) {   // uniform branch; same reduction as S below, nine values
+  if (lam_glob) {   // uniform branch; same idea as S below for nine values: lane q of a warp ends up owning maximum q,
+                    // so a warp costs one load of the nine running maxima and, rarely, an atomic
+    double mine = 0.0;
 #pragma unroll
     for (int q = 0; q < 9; ++q) {
       double v = lg[q] == lg[q] ? lg[q] : 0.0;
-      for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
-      if ((threadIdx.x & 31) == 0 && v > *reinterpret_cast<volatile double *>(lam_glob + q))
-        atomicMax(reinterpret_cast<unsigned long long *>(lam_glob + q), (unsigned long long)__double_as_longlong(v));
+      for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+      if ((threadIdx.x & 31) == q) mine = v;
     }
+    const int q = threadIdx.x & 31;
+    if (q < 9 && mine > *reinterpret_cast<volatile double *>(lam_glob + q))
+      atomicMax(reinterpret_cast<unsigned long long *>(lam_glob + q), (unsigned long long)__double_as_longlong(mine));
   }
   if (S_out) {   // non-negative doubles order like their bit patterns: one 64-bit atomicMax per warp
     for (int o = 16; o > 0; o >>= 1) smax = fmax(smax, __shfl_down_sync(0xffffffffu, smax, o));
