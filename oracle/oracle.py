@@ -24,7 +24,7 @@ class OConfig(C.Structure):
         ("Tlo", C.c_double), ("Thi", C.c_double),
         ("bc", C.c_int * 6), ("bc_state", (C.c_double * MAXNV) * 6),
         ("rtol", C.c_double), ("maxit", C.c_int), ("ideal_weights", C.c_int), ("viscosity", C.c_int),
-        ("lam_glob", (C.c_double * 3) * 3),
+        ("lam_glob", (C.c_double * 3) * 3), ("recon", C.c_int),
     ]
 
 
@@ -76,6 +76,8 @@ def lib():
         L.xo_eigensystem.argtypes = [cp, pp, pp, C.c_int, dp, dp, dp]
         L.xo_weno5.argtypes = [dp, C.c_int]
         L.xo_weno5.restype = C.c_double
+        L.xo_wenocu6.argtypes = [dp, C.c_int, dp, dp]
+        L.xo_wenocu6.restype = C.c_double
         L.xo_face_flux.argtypes = [cp, C.c_int, dp, pp, dp]
         L.xo_fill_ghosts.argtypes = [cp, dp]
         L.xo_fill_ghosts.restype = None
@@ -94,6 +96,15 @@ def _dp(a: np.ndarray):
     return a.ctypes.data_as(C.POINTER(C.c_double))
 
 
+def wenocu6(v, ideal: bool = False):
+    """-> (value at +1/2, [beta0, beta1, beta2, beta6], [four normalised weights])"""
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    assert v.shape == (6,)
+    beta, w = np.zeros(4), np.zeros(4)
+    val = float(lib().xo_wenocu6(_dp(v), int(ideal), _dp(beta), _dp(w)))
+    return val, beta, w
+
+
 def weno5(v, ideal: bool = False) -> float:
     v = np.ascontiguousarray(v, dtype=np.float64)
     assert v.shape == (5,)
@@ -104,7 +115,7 @@ class Oracle:
     """One oracle context: grid, species table and boundary data (mirrors xf_config of include/xf.h)."""
 
     def __init__(self, nx, ny, nz, dx, dy, dz, W, nasa7, Ru, Tlo, Thi, bc=(0,) * 6, bc_state=None,
-                 rtol: float = 1e-13, maxit: int = 50, ideal_weights: bool = False, viscosity: int = 0):
+                 rtol: float = 1e-13, maxit: int = 50, ideal_weights: bool = False, viscosity: int = 0, recon: int = 0):
         W = np.asarray(W, dtype=np.float64)
         nasa7 = np.asarray(nasa7, dtype=np.float64)
         n = W.shape[0]
@@ -127,6 +138,7 @@ class Oracle:
                     cfg.bc_state[q][v] = bs[q, v]
         cfg.rtol, cfg.maxit, cfg.ideal_weights = float(rtol), int(maxit), int(ideal_weights)
         cfg.viscosity = int(viscosity)   # 0 LLF, 1 ROE, 2 GLF (xf_oracle.h)
+        cfg.recon = int(recon)           # 0 WENO5-JS, 1 WENO-CU6
         self.cfg = cfg
         self.N = n
         self.Nv = n + 4

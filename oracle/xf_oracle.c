@@ -271,6 +271,50 @@ double xo_weno5(const double v[5], int ideal_weights) {
 }
 
 /* ------------------------------------------------------------------------------------------------------------ */
+/* C6'. WENO-CU6 (PAPER.md:107 names it, ref 34, and prints no formula: reading R16).  Six-point stencil v_{-2}..v_{+3};   */
+/* candidates q_0..q_2 as in WENO5 plus the downwind q_3; linear weights 1/20, 9/20, 9/20, 1/20 (the sixth-order        */
+/* central scheme); beta_0..beta_2 as Jiang-Shu; the fourth indicator is beta_6, the Jiang-Shu measure                 */
+/*   sum_{l=1..5} dx^(2l-1) int (d^l p/dx^l)^2 dx  of the degree-5 polynomial over all six cells (its quadratic form,  */
+/* over 120960, is derived exactly in tests/golden/make_golden.py and pinned against quadrature in the tests);          */
+/* tau_6 = beta_6 - (beta_0 + 4 beta_1 + beta_2)/6;  alpha_k = d_k (C + tau_6/(beta_k + eps)), C = 20, eps = 1e-40.    */
+/* ------------------------------------------------------------------------------------------------------------ */
+double xo_wenocu6(const double v[6], int ideal_weights, double *beta_out, double *w_out) {
+  static const double d[4] = {1.0 / 20.0, 9.0 / 20.0, 9.0 / 20.0, 1.0 / 20.0};
+  /* upper-triangular coefficients of beta_6 * 120960: entry [a][b], b >= a, multiplies v_a v_b */
+  static const double B6[6][6] = {
+      {271779.0, -2380800.0, 4086352.0, -3462252.0, 1458762.0, -245620.0},
+      {0.0, 5653317.0, -20427884.0, 17905032.0, -7727988.0, 1325006.0},
+      {0.0, 0.0, 19510972.0, -35817664.0, 15929912.0, -2792660.0},
+      {0.0, 0.0, 0.0, 17195652.0, -15880404.0, 2863984.0},
+      {0.0, 0.0, 0.0, 0.0, 3824847.0, -1429976.0},
+      {0.0, 0.0, 0.0, 0.0, 0.0, 139633.0}};
+  double q[4], a[4], beta[4];
+  q[0] = (2.0 * v[0] - 7.0 * v[1] + 11.0 * v[2]) / 6.0;
+  q[1] = (-v[1] + 5.0 * v[2] + 2.0 * v[3]) / 6.0;
+  q[2] = (2.0 * v[2] + 5.0 * v[3] - v[4]) / 6.0;
+  q[3] = (11.0 * v[3] - 7.0 * v[4] + 2.0 * v[5]) / 6.0;
+  for (int k = 0; k < 3; ++k) {
+    const double t = v[k] - 2.0 * v[k + 1] + v[k + 2];
+    const double s = k == 0 ? v[0] - 4.0 * v[1] + 3.0 * v[2] : (k == 1 ? v[1] - v[3] : 3.0 * v[2] - 4.0 * v[3] + v[4]);
+    beta[k] = 13.0 / 12.0 * t * t + 0.25 * s * s;
+  }
+  double b6 = 0.0;
+  for (int i = 0; i < 6; ++i)
+    for (int j = i; j < 6; ++j) b6 += B6[i][j] * v[i] * v[j];
+  beta[3] = b6 / 120960.0;
+  if (ideal_weights) {
+    for (int k = 0; k < 4; ++k) a[k] = d[k];
+  } else {
+    const double tau = beta[3] - (beta[0] + 4.0 * beta[1] + beta[2]) / 6.0;
+    for (int k = 0; k < 4; ++k) a[k] = d[k] * (20.0 + tau / (beta[k] + 1e-40));
+  }
+  const double sum = a[0] + a[1] + a[2] + a[3];
+  if (beta_out) for (int k = 0; k < 4; ++k) beta_out[k] = beta[k];
+  if (w_out) for (int k = 0; k < 4; ++k) w_out[k] = a[k] / sum;
+  return (a[0] * q[0] + a[1] * q[1] + a[2] * q[2] + a[3] * q[3]) / sum;
+}
+
+/* ------------------------------------------------------------------------------------------------------------ */
 /* C5 + C6 + C7. Numerical flux at one face (Eq. 14-15; LLF: PAPER.md:374, reading R8)        */
 /* Ust[m][v], Pst[m], m = 0..5 <-> cells i-2..i+3; the face lies between m = 2 and m = 3.                       */
 /* ------------------------------------------------------------------------------------------------------------ */
@@ -312,9 +356,15 @@ int xo_face_flux(const xo_config *c, int d, const double *Ust, const xo_prim *Ps
       fp[m] = 0.5 * (aF[m][n] + Lam * aU[m][n]);
       fm[m] = 0.5 * (aF[m][n] - Lam * aU[m][n]);
     }
-    const double vp[5] = {fp[0], fp[1], fp[2], fp[3], fp[4]};
-    const double vm[5] = {fm[5], fm[4], fm[3], fm[2], fm[1]};
-    g[n] = xo_weno5(vp, c->ideal_weights) + xo_weno5(vm, c->ideal_weights);
+    if (c->recon == XO_RECON_WENOCU6) {      /* six points: i-2..i+3 for f+, mirrored for f- */
+      const double vp[6] = {fp[0], fp[1], fp[2], fp[3], fp[4], fp[5]};
+      const double vm[6] = {fm[5], fm[4], fm[3], fm[2], fm[1], fm[0]};
+      g[n] = xo_wenocu6(vp, c->ideal_weights, NULL, NULL) + xo_wenocu6(vm, c->ideal_weights, NULL, NULL);
+    } else {
+      const double vp[5] = {fp[0], fp[1], fp[2], fp[3], fp[4]};
+      const double vm[5] = {fm[5], fm[4], fm[3], fm[2], fm[1]};
+      g[n] = xo_weno5(vp, c->ideal_weights) + xo_weno5(vm, c->ideal_weights);
+    }
   }
   for (int j = 0; j < Nv; ++j) {             /* Eq. 15: Fhat = R (F+ + F-) */
     double s = 0.0;

@@ -54,7 +54,9 @@ typedef struct {
                               /*   1 ROE: |lambda_n| of the Roe-averaged face state, no maximum                 */
                               /*   2 GLF: per field and direction, max of |lambda_n| over ALL padded cells      */
   double lam_glob[3][3];      /* GLF maxima [direction][u-c, u, u+c]; filled by the residual routines           */
+  int recon;                  /* reconstruction of Eq. 15: 0 WENO5-JS (reading R7), 1 WENO-CU6 ("[34]")  */
 } xo_config;
+enum { XO_RECON_WENO5 = 0, XO_RECON_WENOCU6 = 1 };
 enum { XO_VISC_LLF = 0, XO_VISC_ROE = 1, XO_VISC_GLF = 2 };
 
 /* all primitive quantities of one cell (C2) */
@@ -84,6 +86,9 @@ int xo_eigensystem(const xo_config *c, const xo_prim *A, const xo_prim *B, int d
 
 /* C6 WENO5-JS: v[0..4] = v_{-2}..v_{+2}, value at +1/2 */
 double xo_weno5(const double v[5], int ideal_weights);
+/* WENO-CU6 value at +1/2 from v[0..5] = v_{-2}..v_{+3}; beta_out (may be NULL) receives beta_0, beta_1, beta_2, beta_6 and
+ * w_out (may be NULL) the four normalised weights */
+double xo_wenocu6(const double v[6], int ideal_weights, double *beta_out, double *w_out);
 
 /* C5-C7 numerical flux at one face from the 6 stencil cells (Ust[m][v], m = 0..5 <-> i-2..i+3) */
 int xo_face_flux(const xo_config *c, int d, const double *Ust, const xo_prim *Pst, double *Fhat);

@@ -3,6 +3,11 @@
 weno5_js_example.txt -- the Jiang-Shu WENO5 value (ref 35; eps = 1e-6, exponent 2, reading R7) for
 the point values v = (1, 3, 2, 5, 4.5), evaluated in EXACT rational arithmetic (fractions.Fraction) from the
 definition, then rounded once to double.  It uses neither oracle/ nor the CUDA path.
+
+wenocu6_beta6_form.txt -- the quadratic form of the six-point Jiang-Shu smoothness measure used by WENO-CU6
+(PAPER.md:107 names the scheme, ref 34, and prints no formula; reading R16), derived here in exact rational
+arithmetic from its DEFINITION: beta_6 = sum_{l=1..5} dx^(2l-1) int_cell (d^l p/dx^l)^2 dx with p the degree-5 polynomial
+whose cell averages over cells i-2..i+3 are f_0..f_5.  Coefficients of f_a f_b (a <= b) times 120960.
 """
 from fractions import Fraction as Fr
 from pathlib import Path
@@ -22,3 +27,53 @@ out.write_text(
     "# arithmetic, written by tests/golden/make_golden.py\n"
     f"v=1,3,2,5,4.5\nvalue={float(val)!r}\nvalue_exact={val.numerator}/{val.denominator}\n")
 print(float(val))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# WENO-CU6: quadratic form of beta_6 from its definition
+# ---------------------------------------------------------------------------------------------------------------
+def _polymul(a, b):
+    r = [Fr(0)] * (len(a) + len(b) - 1)
+    for i, x in enumerate(a):
+        for j, y in enumerate(b):
+            r[i + j] += x * y
+    return r
+
+
+def _polyder(a):
+    return [a[k] * k for k in range(1, len(a))]
+
+
+def _polyint(a, lo, hi):
+    return sum(c * (hi ** (k + 1) - lo ** (k + 1)) / (k + 1) for k, c in enumerate(a))
+
+
+n = 6
+A = [[_polyint([Fr(0)] * k + [Fr(1)], Fr(2 * (j - 2) - 1, 2), Fr(2 * (j - 2) + 1, 2)) for k in range(n)] for j in range(n)]
+M = [row[:] + [Fr(int(i == j)) for j in range(n)] for i, row in enumerate(A)]
+for c in range(n):                                    # exact Gauss-Jordan inverse
+    piv = next(r for r in range(c, n) if M[r][c] != 0)
+    M[c], M[piv] = M[piv], M[c]
+    pv = M[c][c]
+    M[c] = [x / pv for x in M[c]]
+    for r in range(n):
+        if r != c and M[r][c] != 0:
+            f = M[r][c]
+            M[r] = [x - f * y for x, y in zip(M[r], M[c])]
+Ainv = [row[n:] for row in M]
+P = [[Ainv[k][j] for k in range(n)] for j in range(n)]   # basis polynomial of f_j
+lines = ["# beta_6 * 120960 = sum_{a<=b} C[a][b] f_a f_b, f_0..f_5 = cells i-2..i+3; exact, from the definition",
+         "# written by tests/golden/make_golden.py"]
+for a_ in range(n):
+    row = []
+    for b_ in range(a_, n):
+        pa, pb, acc = P[a_], P[b_], Fr(0)
+        for _ in range(1, 6):
+            pa, pb = _polyder(pa), _polyder(pb)
+            acc += _polyint(_polymul(pa, pb), Fr(-1, 2), Fr(1, 2))
+        coef = acc * (1 if a_ == b_ else 2) * 120960
+        assert coef.denominator == 1
+        row.append(str(coef.numerator))
+    lines.append(f"row{a_}=" + ",".join(row))
+(Path(__file__).resolve().parent / "wenocu6_beta6_form.txt").write_text("\n".join(lines) + "\n")
+print("\n".join(lines))
