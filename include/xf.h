@@ -62,7 +62,15 @@ typedef struct {
   int newton_maxit;        /* 0 -> 50                                                                           */
   int device;              /* CUDA ordinal                                                                      */
   int viscosity;           /* XF_VISC_*: the artificial viscosity Lambda~ of Eq. 14 (options 374)  */
+  int reconstruction;      /* XF_RECON_*: the reconstruction of Eq. 15                            */
 } xf_config;
+
+/* Reconstruction of the split characteristic fluxes at a face:
+ *   WENO5   Jiang-Shu, eps = 1e-6, exponent 2 (reading R7; the default), points i-2..i+2 / mirrored
+ *   WENOCU6 the six-point central-upwind scheme of the paper's ref 34 (reading R16: linear weights 1/20, 9/20, 9/20,
+ *           1/20; fourth indicator = the six-point Jiang-Shu measure beta_6; tau_6 = beta_6 - (beta_0 + 4 beta_1 +
+ *           beta_2)/6; alpha_k = d_k (20 + tau_6/(beta_k + 1e-40))), points i-2..i+3 / mirrored: same ghost width */
+enum { XF_RECON_WENO5 = 0, XF_RECON_WENOCU6 = 1 };
 
 /* Lambda~_n of the flux splitting f+- = (L F +- Lambda~ L U)/2, per characteristic field n:
  *   LLF  max over the six stencil cells of |lambda_n| of each cell's own state (reading R8; the default)

@@ -280,14 +280,16 @@ double xo_weno5(const double v[5], int ideal_weights) {
 /* ------------------------------------------------------------------------------------------------------------ */
 double xo_wenocu6(const double v[6], int ideal_weights, double *beta_out, double *w_out) {
   static const double d[4] = {1.0 / 20.0, 9.0 / 20.0, 9.0 / 20.0, 1.0 / 20.0};
-  /* upper-triangular coefficients of beta_6 * 120960: entry [a][b], b >= a, multiplies v_a v_b */
-  static const double B6[6][6] = {
-      {271779.0, -2380800.0, 4086352.0, -3462252.0, 1458762.0, -245620.0},
-      {0.0, 5653317.0, -20427884.0, 17905032.0, -7727988.0, 1325006.0},
-      {0.0, 0.0, 19510972.0, -35817664.0, 15929912.0, -2792660.0},
-      {0.0, 0.0, 0.0, 17195652.0, -15880404.0, 2863984.0},
-      {0.0, 0.0, 0.0, 0.0, 3824847.0, -1429976.0},
-      {0.0, 0.0, 0.0, 0.0, 0.0, 139633.0}};
+  /* beta_6 * 120960 as a quadratic form of the five first differences D_k = v_{k+1} - v_k (the measure is translation
+   * invariant; in terms of the values themselves the form has coefficients up to 3.6e7 that cancel to round-off on
+   * smooth data).  Entry [k][l], l >= k, multiplies D_k D_l; obtained from the value form of
+   * tests/golden/wenocu6_beta6_form.txt by v_j = v_0 + sum_{k<j} D_k. */
+  static const double G6[5][5] = {
+      {271779.0, -1837242.0, 2249110.0, -1213142.0, 245620.0},
+      {0.0, 3544296.0, -9252940.0, 5189840.0, -1079386.0},
+      {0.0, 0.0, 6713736.0, -7947412.0, 1713274.0},
+      {0.0, 0.0, 0.0, 2534504.0, -1150710.0},
+      {0.0, 0.0, 0.0, 0.0, 139633.0}};
   double q[4], a[4], beta[4];
   q[0] = (2.0 * v[0] - 7.0 * v[1] + 11.0 * v[2]) / 6.0;
   q[1] = (-v[1] + 5.0 * v[2] + 2.0 * v[3]) / 6.0;
@@ -298,9 +300,10 @@ double xo_wenocu6(const double v[6], int ideal_weights, double *beta_out, double
     const double s = k == 0 ? v[0] - 4.0 * v[1] + 3.0 * v[2] : (k == 1 ? v[1] - v[3] : 3.0 * v[2] - 4.0 * v[3] + v[4]);
     beta[k] = 13.0 / 12.0 * t * t + 0.25 * s * s;
   }
-  double b6 = 0.0;
-  for (int i = 0; i < 6; ++i)
-    for (int j = i; j < 6; ++j) b6 += B6[i][j] * v[i] * v[j];
+  double D[5], b6 = 0.0;
+  for (int k = 0; k < 5; ++k) D[k] = v[k + 1] - v[k];
+  for (int k = 0; k < 5; ++k)
+    for (int l = k; l < 5; ++l) b6 += G6[k][l] * D[k] * D[l];
   beta[3] = b6 / 120960.0;
   if (ideal_weights) {
     for (int k = 0; k < 4; ++k) a[k] = d[k];

@@ -23,7 +23,7 @@ struct xf_ctx {
   double *bc_state_dev;               // [6][XF_MAXNV]
   double *S_dev;                      // max wave speed scalar used by the host-buffer entry points
   double *lam_glob_dev;               // GLF: [3][3] global maxima of the current residual evaluation
-  int visc;                           // XF_VISC_*
+  int visc, recon;                    // XF_VISC_*, XF_RECON_*
   long launches;
   // lazily allocated device mirrors for the *_host entry points
   double *hU, *hT, *hR;
@@ -119,6 +119,7 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
       E.out = acc;
     }
     E.visc = c->visc;
+    E.recon = c->recon;
     E.lam_glob = c->lam_glob_dev;
     Timed t(c, XF_K_SWEEP_X + d, s);
     if (d == 0) rc = xf_launch_sweep_x(c->G, c->N, U, prim, E, c->status_dev, s);
@@ -194,6 +195,7 @@ int xf_create(xf_ctx **out, const xf_config *cfg) {
     if (!(cfg->W[s] > 0.0)) return XF_EINVAL;
   if (n[0] == 1 && n[1] == 1 && n[2] == 1) return XF_EINVAL;
   if (cfg->viscosity < XF_VISC_LLF || cfg->viscosity > XF_VISC_GLF) return XF_EINVAL;
+  if (cfg->reconstruction < XF_RECON_WENO5 || cfg->reconstruction > XF_RECON_WENOCU6) return XF_EINVAL;
   if (n[1] > 65535 || n[2] > 65535) return XF_EINVAL;  // they index the y dimension of the y/z sweep grids
 
   int ndev = 0;
@@ -208,6 +210,7 @@ int xf_create(xf_ctx **out, const xf_config *cfg) {
   c->Nv = N + 4;
   c->device = cfg->device;
   c->visc = cfg->viscosity;
+  c->recon = cfg->reconstruction;
   XfGrid &G = c->G;
   for (int d = 0; d < 3; ++d) {
     G.n[d] = n[d];

@@ -52,6 +52,7 @@ struct XfEpilogue {
   const double *Un;   // U^n  [Nv][padded] (mode 2)
   double *out;        // rhs or U^{s+1} [Nv][padded]
   int visc;           // XF_VISC_*: Lambda~ of Eq. 14
+  int recon;          // XF_RECON_*: reconstruction of Eq. 15 (host-side dispatch of the kernel instantiation)
   const double *lam_glob;  // GLF: [direction][u-c, u, u+c] global maxima on the device
 };
 

@@ -52,8 +52,47 @@ __device__ __forceinline__ double weno5(double v0, double v1, double v2, double 
   return fma(num, xf_rcp(den), base);
 }
 
-// g = WENO5(f+ at i-2..i+2) + WENO5(f- at i+3..i-1)  (Eq. 15)
-__device__ __forceinline__ double weno5_pair(const double (&fp)[6], const double (&fm)[6]) {
+// WENO-CU6 (include/xf.h XF_RECON_WENOCU6; PAPER.md:107 ref 34) value at +1/2 from v0..v5 = v_{-2}..v_{+3}.
+// Candidates on first differences: q_k = v2 + c_k/6 with c_0 = 5 D2 - 2 D1, c_1 = D2 + 2 D3, c_2 = 4 D3 - D4,
+// c_3 = 6 D3 - 5 D4 + 2 D5; beta_0..2 as Jiang-Shu; beta_6 is the six-point measure, a quadratic form of the five
+// first differences (translation invariant: no cancellation of large terms; coefficients over 120960, derived exactly
+// from the form in tests/golden/wenocu6_beta6_form.txt); tau = beta_6 - (beta_0 + 4 beta_1 + beta_2)/6 and
+// alpha_k = d_k (C + tau/(beta_k + eps)), C = 20, eps = 1e-40, brought to the common denominator prod (beta_j + eps):
+// one reciprocal per reconstruction.
+__device__ __forceinline__ double wenocu6(double v0, double v1, double v2, double v3, double v4, double v5) {
+  const double D1 = v1 - v0, D2 = v2 - v1, D3 = v3 - v2, D4 = v4 - v3, D5 = v5 - v4;
+  const double d0 = D2 - D1, d1 = D3 - D2, d2 = D4 - D3;
+  const double e0 = fma(3.0, D2, -D1), e1 = D2 + D3, e2 = fma(-3.0, D3, D4);
+  const double k1312 = 13.0 / 12.0, eps = 1e-40;
+  const double b0 = fma(0.25 * e0, e0, fma(k1312 * d0, d0, eps));   // beta_k + eps
+  const double b1 = fma(0.25 * e1, e1, fma(k1312 * d1, d1, eps));
+  const double b2 = fma(0.25 * e2, e2, fma(k1312 * d2, d2, eps));
+  constexpr double s = 1.0 / 120960.0;
+  const double t1 = fma(271779.0 * s, D1, fma(-1837242.0 * s, D2, fma(2249110.0 * s, D3, fma(-1213142.0 * s, D4, 245620.0 * s * D5))));
+  const double t2 = fma(3544296.0 * s, D2, fma(-9252940.0 * s, D3, fma(5189840.0 * s, D4, -1079386.0 * s * D5)));
+  const double t3 = fma(6713736.0 * s, D3, fma(-7947412.0 * s, D4, 1713274.0 * s * D5));
+  const double t4 = fma(2534504.0 * s, D4, -1150710.0 * s * D5);
+  const double beta6 = fma(D1, t1, fma(D2, t2, fma(D3, t3, fma(D4, t4, 139633.0 * s * D5 * D5))));
+  const double tau = beta6 - (b0 + fma(4.0, b1, b2) - 6.0 * eps) * (1.0 / 6.0);
+  const double b3 = beta6 + eps;
+  // A_k = d_k (20 b_k + tau) prod_{j != k} b_j,  d = (1, 9, 9, 1)/20
+  const double p01 = b0 * b1, p23 = b2 * b3;
+  const double A0 = fma(20.0, b0, tau) * (b1 * p23);
+  const double A1 = 9.0 * fma(20.0, b1, tau) * (b0 * p23);
+  const double A2 = 9.0 * fma(20.0, b2, tau) * (p01 * b3);
+  const double A3 = fma(20.0, b3, tau) * (p01 * b2);
+  const double c0 = fma(5.0, D2, -2.0 * D1), c1 = fma(2.0, D3, D2), c2 = fma(4.0, D3, -D4);
+  const double c3 = fma(6.0, D3, fma(-5.0, D4, 2.0 * D5));
+  const double num = fma(A0, c0, fma(A1, c1, fma(A2, c2, A3 * c3)));
+  const double den = 6.0 * ((A0 + A1) + (A2 + A3));
+  return fma(num, xf_rcp(den), v2);
+}
+
+// g = R(f+ at i-2..) + R(f- mirrored)  (Eq. 15); RECON: 0 WENO5-JS (five points each), 1 WENO-CU6 (all six)
+template <int RECON>
+__device__ __forceinline__ double weno_pair(const double (&fp)[6], const double (&fm)[6]) {
+  if (RECON == 1)
+    return wenocu6(fp[0], fp[1], fp[2], fp[3], fp[4], fp[5]) + wenocu6(fm[5], fm[4], fm[3], fm[2], fm[1], fm[0]);
   return weno5(fp[0], fp[1], fp[2], fp[3], fp[4]) + weno5(fm[5], fm[4], fm[3], fm[2], fm[1]);
 }
 
@@ -77,7 +116,7 @@ __host__ __device__ constexpr int nprimfields(int N) { return N + 4; }
 // so a sweep may keep them in a shallower ring than the six-deep stencil fields.
 // p, c, 1/rho (six-deep like U) are read through their own base pointer sp (field g at sp[g*FS + o[m]]) so that a
 // sweep may place them in a separately aligned box of the same ring row.
-template <int DIR, class Emit>
+template <int DIR, int RECON, class Emit>
 __device__ __forceinline__ bool face_flux(const int N, const double *sm, const double *sp, const int FS,
                                           const int (&o)[6], const double *ss, const int SS, const int s2,
                                           const int s3, const int visc, const double *__restrict__ lamg, Emit &emit) {
@@ -169,7 +208,7 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const d
       fp[m] = fma(0.5 * (ud[m] + lam_m), a, pt);
       fm[m] = fma(0.5 * (ud[m] - lam_m), a, pt);
     }
-    g0 = weno5_pair(fp, fm);
+    g0 = weno_pair<RECON>(fp, fm);
 #pragma unroll
     for (int m = 0; m < 6; ++m) {
       const double a = h * fma(ct, nuU[m], piU[m]);
@@ -177,7 +216,7 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const d
       fp[m] = fma(0.5 * (ud[m] + lam_p), a, pt);
       fm[m] = fma(0.5 * (ud[m] - lam_p), a, pt);
     }
-    gL = weno5_pair(fp, fm);
+    gL = weno_pair<RECON>(fp, fm);
   }
   double ap[6], am[6];  // (u_m +- Lambda_u)/2 for all fields that travel with u
 #pragma unroll
@@ -194,7 +233,7 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const d
       fp[m] = fma(ap[m], a, pt);
       fm[m] = fma(am[m], a, pt);
     }
-    g1 = weno5_pair(fp, fm);
+    g1 = weno_pair<RECON>(fp, fm);
   }
 
   // ---- back-projection Fhat = R g (Eq. 15), structured
@@ -219,7 +258,7 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const d
       fp[m] = ap[m] * a;                                                                               \
       fm[m] = am[m] * a;                                                                               \
     }                                                                                                  \
-    const double g = weno5_pair(fp, fm);                                                               \
+    const double g = weno_pair<RECON>(fp, fm);                                                               \
     F4 = fma((DEXPR), g, F4);                                                                          \
     emit(VIDX, fma(C, s, g), VNEXT);                                                                   \
   }

@@ -6,7 +6,7 @@
 namespace {
 using namespace xf;
 
-template <int NT>
+template <int NT, int RC>
 int launch(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status, cudaStream_t s) {
   CUtensorMap tmU, tmP, tmS;   // U [N + 4]; p, c, 1/rho [3]; Gamma, chi_s [N + 1]
   static const bool no_tma = getenv("XF_NO_TMA") != nullptr;
@@ -17,7 +17,7 @@ int launch(const XfGrid &G, int N, const double *U, const double *prim, const Xf
     const int segs = (int)((Lf + segc - 1) / segc);
     const unsigned blocks = (unsigned)(segs * G.n[2]);
     const size_t smem = sizeof(double) * xw_smem_doubles(N);
-    sweep_x_ws_kernel<NT><<<blocks, dim3(32, 2 * XW_W), smem, s>>>(G, N, U, E, status, segs, tmU, tmP, tmS);
+    sweep_x_ws_kernel<NT, RC><<<blocks, dim3(32, 2 * XW_W), smem, s>>>(G, N, U, E, status, segs, tmU, tmP, tmS);
     return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
   }
   const long long L = (long long)G.n[1] * G.np[0];
@@ -25,14 +25,14 @@ int launch(const XfGrid &G, int N, const double *U, const double *prim, const Xf
   const int segs = (int)((L + SEGC - 1) / SEGC);
   const unsigned blocks = (unsigned)(segs * G.n[2]);
   const size_t smem = sizeof(double) * warp_smem_doubles(N, X_LI, X_RR);
-  sweep_kernel<NT, 0, X_LI, X_LJ, X_RR, X_MINB><<<blocks, 32, smem, s>>>(G, N, U, prim, E, status, segs);
+  sweep_kernel<NT, 0, X_LI, X_LJ, X_RR, X_MINB, RC><<<blocks, 32, smem, s>>>(G, N, U, prim, E, status, segs);
   return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
 }
 }  // namespace
 
 int xf_launch_sweep_x(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
                       cudaStream_t s) {
-#define CALL(NT) return launch<NT>(G, N, U, prim, E, status, s)
+#define CALL(NT) return E.recon == 1 ? launch<NT, 1>(G, N, U, prim, E, status, s) : launch<NT, 0>(G, N, U, prim, E, status, s)
   XF_DISPATCH_SWEEP_N(N, CALL)
 #undef CALL
   return XF_EINVAL;
@@ -40,14 +40,17 @@ int xf_launch_sweep_x(const XfGrid &G, int N, const double *U, const double *pri
 
 int xf_sweep_x_init() {
   cudaError_t e = cudaSuccess;
-#define CALL(NT)                                                                                                   \
-  e = cudaFuncSetAttribute(sweep_kernel<NT, 0, X_LI, X_LJ, X_RR, X_MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                           (int)(sizeof(double) * warp_smem_doubles(NT > 0 ? NT : XF_MAXN, X_LI, X_RR)));         \
-  if (e != cudaSuccess) return XF_ECUDA;                                                                           \
-  e = cudaFuncSetAttribute(sweep_x_ws_kernel<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize,                     \
-                           (int)(sizeof(double) * xw_smem_doubles(NT > 0 ? NT : XF_MAXN)));                        \
+#define CALL2(NT, RC)                                                                                                  \
+  e = cudaFuncSetAttribute(sweep_kernel<NT, 0, X_LI, X_LJ, X_RR, X_MINB, RC>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                           (int)(sizeof(double) * warp_smem_doubles(NT > 0 ? NT : XF_MAXN, X_LI, X_RR)));             \
+  if (e != cudaSuccess) return XF_ECUDA;                                                                               \
+  e = cudaFuncSetAttribute(sweep_x_ws_kernel<NT, RC>, cudaFuncAttributeMaxDynamicSharedMemorySize,                     \
+                           (int)(sizeof(double) * xw_smem_doubles(NT > 0 ? NT : XF_MAXN)));                            \
   if (e != cudaSuccess) return XF_ECUDA;
+#define CALL(NT)                                                                                                   \
+  CALL2(NT, 0) CALL2(NT, 1)
   CALL(0) CALL(1) CALL(2) CALL(3) CALL(4) CALL(10)
 #undef CALL
+#undef CALL2
   return XF_OK;
 }

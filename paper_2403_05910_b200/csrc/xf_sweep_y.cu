@@ -6,7 +6,7 @@
 namespace {
 constexpr int DIR = 1, OD = DIR == 1 ? 2 : 1;
 
-template <int NT>
+template <int NT, int RC>
 int launch(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status, cudaStream_t s) {
   using namespace xf;
   const int strips = (G.n[0] + 31) / 32;
@@ -23,16 +23,16 @@ int launch(const XfGrid &G, int N, const double *U, const double *prim, const Xf
   static const bool no_tma = getenv("XF_NO_TMA") != nullptr;
   if (!no_tma && G.g[0] == XF_NG && xf_row_tensor_map(&tmU, G, U, N + 4) && xf_row_tensor_map(&tmP, G, prim, 3) &&
       xf_row_tensor_map(&tmS, G, prim + 3 * G.cells, N + 1))
-    sweep_yz_ws_kernel<NT, DIR, YZ_W, true><<<grid, block, smem, s>>>(G, N, U, prim, E, status, seg_len, tmU, tmP, tmS);
+    sweep_yz_ws_kernel<NT, DIR, YZ_W, true, RC><<<grid, block, smem, s>>>(G, N, U, prim, E, status, seg_len, tmU, tmP, tmS);
   else
-    sweep_yz_ws_kernel<NT, DIR, YZ_W, false><<<grid, block, smem, s>>>(G, N, U, prim, E, status, seg_len, tmU, tmP, tmS);
+    sweep_yz_ws_kernel<NT, DIR, YZ_W, false, RC><<<grid, block, smem, s>>>(G, N, U, prim, E, status, seg_len, tmU, tmP, tmS);
   return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
 }
 }  // namespace
 
 int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
                       cudaStream_t s) {
-#define CALL(NT) return launch<NT>(G, N, U, prim, E, status, s)
+#define CALL(NT) return E.recon == 1 ? launch<NT, 1>(G, N, U, prim, E, status, s) : launch<NT, 0>(G, N, U, prim, E, status, s)
   XF_DISPATCH_SWEEP_N(N, CALL)
 #undef CALL
   return XF_EINVAL;
@@ -41,14 +41,13 @@ int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *pri
 int xf_sweep_y_init() {
   using namespace xf;
   cudaError_t e = cudaSuccess;
-#define CALL(NT)                                                                                             \
-  e = cudaFuncSetAttribute(sweep_yz_ws_kernel<NT, DIR, YZ_W, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
-                           (int)(sizeof(double) * yz_smem_doubles(NT > 0 ? NT : XF_MAXN, YZ_W)));            \
-  if (e != cudaSuccess) return XF_ECUDA;                                                                     \
-  e = cudaFuncSetAttribute(sweep_yz_ws_kernel<NT, DIR, YZ_W, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                           (int)(sizeof(double) * yz_smem_doubles(NT > 0 ? NT : XF_MAXN, YZ_W)));            \
+#define CALL2(NT, TM, RC)                                                                                        \
+  e = cudaFuncSetAttribute(sweep_yz_ws_kernel<NT, DIR, YZ_W, TM, RC>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
+                           (int)(sizeof(double) * yz_smem_doubles(NT > 0 ? NT : XF_MAXN, YZ_W)));                    \
   if (e != cudaSuccess) return XF_ECUDA;
+#define CALL(NT) CALL2(NT, true, 0) CALL2(NT, false, 0) CALL2(NT, true, 1) CALL2(NT, false, 1)
   CALL(0) CALL(1) CALL(2) CALL(3) CALL(4) CALL(10)
 #undef CALL
+#undef CALL2
   return XF_OK;
 }

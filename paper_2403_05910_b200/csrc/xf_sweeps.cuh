@@ -88,7 +88,7 @@ struct CellWriter {
 
 // One warp = one segment of one pencil group.  DIR = 0: blockIdx.x enumerates (k-plane, segment of the flat pencil).
 // DIR = 1, 2: blockIdx = (group of LI pencils along i, index along the other transverse direction, segment).
-template <int N_T, int DIR, int LI, int LJ, int RR, int MINB>
+template <int N_T, int DIR, int LI, int LJ, int RR, int MINB, int RECON>
 __global__ void __launch_bounds__(32, MINB)
 sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const double *__restrict__ prim,
              const XfEpilogue E, int *__restrict__ status, const int seg_param) {
@@ -219,7 +219,7 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
     W.carry_rd = carry + par * Nv * LI;
     W.carry_wr = carry + (par ^ 1) * Nv * LI;
     W.preload(0);
-    const bool c2ok = face_flux<DIR>(N, sm, sm + Nv * FS, FS, o, sm + (Nv + 3) * FS, FS, o[2], o[3], E.visc, E.lam_glob + 3 * DIR, W);
+    const bool c2ok = face_flux<DIR, RECON>(N, sm, sm + Nv * FS, FS, o, sm + (Nv + 3) * FS, FS, o[2], o[3], E.visc, E.lam_glob + 3 * DIR, W);
     bad = bad || (!c2ok && lane_ok && f <= f_end);
     __syncwarp();         // all lanes are done with the rows the next iteration's prefetch overwrites
     if (PF < LJ) {        // the remaining LJ - PF rows of the next chunk go where this chunk's first rows were
@@ -327,7 +327,7 @@ struct FluxStoreWS {
   }
 };
 
-template <int N_T, int DIR, int W, bool TMA>
+template <int N_T, int DIR, int W, bool TMA, int RECON>
 __global__ void __launch_bounds__(64 * W, 2)
 sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const double *__restrict__ prim,
                    const XfEpilogue E, int *__restrict__ status, const int seg_len,
@@ -404,7 +404,7 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
       asm volatile("" : "+r"(s2), "+r"(s3));
       if (f <= f_end) {                                     // warp-uniform
         FluxStoreWS st{fb + (w + 1) * 32 + lane, FBS, first ? -1 : BAR_FB_EMPTY + par, NT};
-        const bool c2ok = face_flux<DIR>(N, sm, smp, FS, o, sms, FS, s2, s3, E.visc, E.lam_glob + 3 * DIR, st);
+        const bool c2ok = face_flux<DIR, RECON>(N, sm, smp, FS, o, sms, FS, s2, s3, E.visc, E.lam_glob + 3 * DIR, st);
         bad = bad || (!c2ok && lane_ok);
       } else if (!first) {
         named_sync(BAR_FB_EMPTY + par, NT);                 // keep the barrier counts whole
@@ -595,7 +595,7 @@ __device__ __forceinline__ void tma_load_span(unsigned dst, const void *tmap, in
       : "memory");
 }
 
-template <int N_T>
+template <int N_T, int RECON>
 __global__ void __launch_bounds__(64 * XW_W, 2)
 sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const XfEpilogue E,
                   int *__restrict__ status, const int segs_per_plane, const __grid_constant__ CUtensorMap tmU,
@@ -644,7 +644,7 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
       for (int m = 0; m < 6; ++m) o[m] = u + delta + m;
       // every lane of the block passes the same barriers; lanes past f_end compute on staged (valid or zero) data
       FluxStoreWS fsw{fb + u + 1, XW_FBW, first ? -1 : BAR_FB_EMPTY + par, NT};
-      const bool c2ok = face_flux<0>(N, st, st + OFFP, FS, o, st + OFFS, FS, o[2], o[3], E.visc, E.lam_glob, fsw);
+      const bool c2ok = face_flux<0, RECON>(N, st, st + OFFP, FS, o, st + OFFS, FS, o[2], o[3], E.visc, E.lam_glob, fsw);
       {
         const int ia = (f - 1 + G.np[0]) % G.np[0], ib = f % G.np[0];
         const bool used = f <= f_end && ((ia >= G.g[0] && ia < G.g[0] + G.n[0]) || (ib >= G.g[0] && ib < G.g[0] + G.n[0]));

@@ -19,6 +19,7 @@ LIB_PATH = _HERE / "libxf.so"
 XF_OK, XF_EINVAL, XF_ECUDA, XF_ENOMEM, XF_ENONPHYSICAL, XF_ENOCONV = 0, -1, -2, -3, -4, -5
 XF_BC_PERIODIC, XF_BC_TRANSMISSIVE, XF_BC_REFLECTIVE, XF_BC_DIRICHLET = 0, 1, 2, 3
 XF_VISC_LLF, XF_VISC_ROE, XF_VISC_GLF = 0, 1, 2
+XF_RECON_WENO5, XF_RECON_WENOCU6 = 0, 1
 XF_MAX_SPECIES = 16
 
 # every symbol include/xf.h declares (tests check that the library exports all of them)
@@ -40,7 +41,7 @@ class XfConfig(C.Structure):
         ("W", C.POINTER(C.c_double)), ("nasa7", C.POINTER(C.c_double)),
         ("Tlo", C.c_double), ("Thi", C.c_double),
         ("bc", C.c_int * 6), ("bc_state", C.POINTER(C.c_double)),
-        ("newton_rtol", C.c_double), ("newton_maxit", C.c_int), ("device", C.c_int), ("viscosity", C.c_int),
+        ("newton_rtol", C.c_double), ("newton_maxit", C.c_int), ("device", C.c_int), ("viscosity", C.c_int), ("reconstruction", C.c_int),
     ]
 
 
@@ -132,7 +133,7 @@ class Context:
 
     def __init__(self, nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, W: Sequence[float], nasa7, Ru: float,
                  Tlo: float, Thi: float, bc=(0,) * 6, bc_state=None, newton_rtol: float = 0.0, newton_maxit: int = 0,
-                 device: int = 0, viscosity: int = XF_VISC_LLF):
+                 device: int = 0, viscosity: int = XF_VISC_LLF, reconstruction: int = XF_RECON_WENO5):
         W = np.ascontiguousarray(W, dtype=np.float64)
         nasa7 = np.ascontiguousarray(nasa7, dtype=np.float64)
         n = int(W.shape[0])
@@ -153,6 +154,7 @@ class Context:
             cfg.bc_state = bs.ctypes.data_as(C.POINTER(C.c_double))
         cfg.newton_rtol, cfg.newton_maxit, cfg.device = float(newton_rtol), int(newton_maxit), int(device)
         cfg.viscosity = int(viscosity)
+        cfg.reconstruction = int(reconstruction)
         self._h = C.c_void_p()
         _check(lib().xf_create(C.byref(self._h), C.byref(cfg)), "xf_create")
         self.device = int(device)

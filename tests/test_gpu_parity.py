@@ -513,3 +513,49 @@ def test_shock_tube_and_bubble_steps_viscosity_variants(oracle_mod, visc):
         assert g.ctx.xf_status() == 0
         assert worst < STEPS_TOL, worst
         g.close()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# WENO-CU6 reconstruction (include/xf.h XF_RECON_WENOCU6): same bar, with each viscosity
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("visc", [0, 1, 2])
+@pytest.mark.parametrize("shape,n,bc", [((400, 1, 1), 1, (0,) * 6), ((150, 37, 1), 3, (3, 1, 2, 2, 0, 0)),
+                                         ((45, 19, 23), 4, (3, 1, 0, 0, 0, 0)), ((70, 9, 8), 10, (3, 1, 2, 2, 2, 2)),
+                                         ((131, 6, 5), 16, (0,) * 6)])
+def test_rhs_parity_wenocu6(oracle_mod, visc, shape, n, bc):
+    w = wl.random_smooth_box(*shape, nspecies=n, seed=3000 + n + shape[0], bc=bc)
+    orc = oracle_mod.Oracle.from_workload(w, viscosity=visc, recon=1)
+    ro = orc.rhs(w.U.copy(), w.T_guess.copy())
+    assert orc.last_status == 0
+    g = _gpu(w, viscosity=visc, reconstruction=1)
+    err = field_err(w.interior(g.rhs()), w.interior(ro))
+    assert err.max() < RHS_TOL, err
+    g.close()
+
+
+def test_rhs_parity_wenocu6_shocked_states(oracle_mod):
+    w = wl.config3_shock_bubble_3d(24)
+    orc = oracle_mod.Oracle.from_workload(w, recon=1)
+    ro = orc.rhs(w.U.copy(), w.T_guess.copy())
+    g = _gpu(w, reconstruction=1)
+    err = field_err(w.interior(g.rhs()), w.interior(ro))
+    assert err.max() < RHS_TOL, err
+    g.close()
+
+
+def test_shock_tube_and_bubble_steps_wenocu6(oracle_mod):
+    for w, steps in ((wl.config1_shock_tube(), 100), (wl.config3_shock_bubble_3d(32), 12)):
+        orc = oracle_mod.Oracle.from_workload(w, recon=1)
+        Uo, To = w.U.copy(), w.T_guess.copy()
+        g = _gpu(w, reconstruction=1)
+        worst = 0.0
+        for _ in range(steps):
+            So = orc.max_wavespeed(Uo, To)
+            dt = w.cfl / So
+            assert orc.rk3_step(Uo, To, dt) == 0
+            g.step(dt)
+            cmax = So * min(w.dx, w.dy, w.dz)
+            worst = max(worst, state_err(w, g.host_U(), Uo, cmax).max())
+        assert g.ctx.xf_status() == 0
+        assert worst < STEPS_TOL, worst
+        g.close()

@@ -49,6 +49,8 @@ def test_beta6_quadratic_form_matches_the_exact_derivation(oracle_mod):
         f = rng.uniform(-1, 1, 6)
         ref = sum(C[a, b] * f[a] * f[b] for a in range(6) for b in range(a, 6)) / 120960.0
         assert abs(oracle_mod.wenocu6(f)[1][3] - ref) <= 1e-12 * abs(ref)
+    # translation invariance, which the oracle's first-difference form relies on: the value form annihilates constants
+    assert abs(sum(C[a, b] for a in range(6) for b in range(a, 6))) == 0.0
 
 
 def test_ideal_weights_give_the_sixth_order_central_flux(oracle_mod):
