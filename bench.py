@@ -261,7 +261,7 @@ def run_b200(args, rank: int, local_rank: int, world: int) -> None:
     w = make_workload(name, grid)
     N, Nv, cells = w.nspecies, w.nvars, w.interior_cells
     D = sum(1 for n in (w.nx, w.ny, w.nz) if n > 1)
-    ctx = xf.Context.from_workload(w, device=local_rank)
+    ctx = xf.Context.from_workload(w, device=local_rank, viscosity=args.viscosity, reconstruction=args.reconstruction)
     U = torch.from_numpy(w.U).to(dev)
     T = torch.from_numpy(w.T_guess).to(dev)
     work = ctx.workspace()
@@ -375,7 +375,8 @@ def run_b200(args, rank: int, local_rank: int, world: int) -> None:
             "config": {"workload": name, "grid": list(grid), "nspecies": N, "nvars": Nv, "interior_cells": cells,
                        "step": "xf_step_cfl = max wave speed (in the first primitives kernel) + 3 x (ghost fill, "
                                "primitives, x/y/z sweeps, RK combine)", "rhs_per_step": 3, "l2": "inputs larger than L2 (one U copy = "
-                               f"{Nv * ctx.cells * 8 / 1e9:.2f} GB), no flush", "parallelism": "replicas"},
+                               f"{Nv * ctx.cells * 8 / 1e9:.2f} GB), no flush", "parallelism": "replicas", "viscosity": ["LLF", "ROE", "GLF"][args.viscosity],
+                       "reconstruction": ["WENO5-JS", "WENO-CU6"][args.reconstruction]},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
             "step_roofline": step_roofline,
         }
@@ -395,6 +396,8 @@ def main() -> None:
     ap.add_argument("--grid", type=int, nargs=3, default=None, help="override the grid (debugging only)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--viscosity", type=int, default=0, help="0 LLF (the benchmark), 1 ROE, 2 GLF")
+    ap.add_argument("--reconstruction", type=int, default=0, help="0 WENO5-JS (the benchmark), 1 WENO-CU6")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

@@ -1,18 +1,22 @@
-// xf_sweeps.cuh -- the marching sweep kernel built around xf::face_flux (see xf_flux.cuh).
+// xf_sweeps.cuh -- the directional sweep kernels built around xf::face_flux (see xf_flux.cuh): staging of the stencil
+// data, flux divergence (Eq. 13) and the fused Runge-Kutta stage combination (Eq. 16).
 //
-// Every WARP is autonomous: it owns a private ring of staged stencil rows in shared memory, fills it with
-// cp.async (LDGSTS) one chunk ahead of the arithmetic, exchanges face fluxes with warp shuffles, and never meets
-// a block-wide barrier -- the fp64 pipe is the bound and must not wait on memory.
+// Production kernels (second half of this file), all warp-specialised with TMA staging:
+//   sweep_x_ws_kernel        x: one k-plane = one flat pencil, 128-face chunks in two stages
+//   sweep_yz_ws_kernel<DIR>  y, z: 32 lanes along i x 4 face rows, ring of 13 / 9 rows
+// Fallbacks for arrays TMA cannot describe (odd padded extents): the same y/z kernel with cp.async staging, and for x
+// the warp-autonomous sweep_kernel below (first half of this file):
 //
+// sweep_kernel: every WARP is autonomous: it owns a private ring of staged stencil rows in shared memory, fills it
+// with cp.async (LDGSTS), exchanges face fluxes with warp shuffles, and never meets a block-wide barrier.
 // A warp's 32 lanes are laid out LI (contiguous, along i) x LJ (along the sweep direction); one lane = one face.
 //   x sweep: LI = 1, LJ = 32.  All interior rows of one k-plane are contiguous in memory (row pitch = padded nx),
 //     so a plane is swept as ONE long flat pencil; the few faces whose stencil straddles a row end are computed
 //     on valid (ghost) data and never used (5 of every nx+6).
-//   y / z sweeps: LI x LJ = 4 x 8: four neighbouring pencils (one 32-byte sector per row) marched 8 faces at a time.
-// A chunk of LJ face rows needs LJ + 5 stencil rows; the ring holds 2 LJ + 5 rows so that the LJ new rows of the
-// next chunk land while the current chunk is computed.  Face row f of a segment is the lower face of cell f; its
-// stencil is rows f .. f+5; the lane that owns face f updates cell f-1 from its own flux and that of face f-1
-// (the lane LI below it, or the carry left in shared memory by the previous chunk).
+// A chunk of LJ face rows needs LJ + 5 stencil rows; the ring holds RR rows (LJ + 5 .. 2 LJ + 5: the rows beyond LJ + 5
+// let part of the next chunk land while the current one is computed).  Face row f of a segment is the lower face of
+// cell f; its stencil is rows f .. f+5; the lane that owns face f updates cell f-1 from its own flux and that of face
+// f-1 (the lane LI below it, or the carry left in shared memory by the previous chunk).
 #pragma once
 #include <cuda.h>
 
