@@ -107,14 +107,22 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
     const int d = dd;
     if (c->G.n[d] == 1) continue;
     XfEpilogue E;
+    // a stage with alpha != 0 and more than one sweep: the first sweep adds alpha/(beta dt) U^n to the partial
+    // residual and the last one no longer reads U^n (XfEpilogue mode 3)
+    const bool un_first = E_last.mode == 2 && E_last.alpha != 0.0 && nact > 1;
     if (done == nact - 1) {
       E = E_last;
       E.has_acc = done > 0;
       if (E.mode != 2) E.mode = done > 0 ? 1 : 0;
+      if (un_first) E.alpha = 0.0;
       E.acc = acc;
     } else {
       memset(&E, 0, sizeof(E));
       E.mode = done > 0 ? 1 : 0;
+      if (done == 0 && un_first) {
+        E = E_last;
+        E.mode = 3;
+      }
       E.acc = acc;
       E.out = acc;
     }

@@ -42,7 +42,10 @@ struct XfBc {
 
 // How a sweep writes its flux divergence: out = alpha*Un + beta*(Us + dt*(acc + div)).
 struct XfEpilogue {
-  int mode;           // 0: out = div (first sweep of a plain rhs); 1: out = acc + div; 2: RK stage combine
+  int mode;           // 0: out = div (first sweep of a plain rhs); 1: out = acc + div; 2: RK stage combine;
+                      // 3: out = div + alpha/(beta dt) U^n -- the FIRST sweep of a stage with alpha != 0 carries the
+                      //    U^n term in the partial residual, so that the last sweep (mode 2 with alpha = 0: out =
+                      //    beta (U^s + dt (acc + div))) need not read U^n: the traffic of the three sweeps is balanced
   int has_acc;        // mode 2: whether a previous sweep left a partial rhs in `acc`
   double alpha, beta; // mode 2: stage weights of Eq. 16
   double dt;          // mode 2: time step, used when S_dev == nullptr

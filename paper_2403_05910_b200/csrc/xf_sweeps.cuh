@@ -52,7 +52,7 @@ struct CellWriter {
   const double *sm_us;    // staged U^s of the cell this lane updates: sm_us[v * FS]
   double *carry_rd, *carry_wr;
   long long gi, cells;
-  double dt, ninv, nacc, nun;
+  double dt, ninv, nacc, nun, kappa;
   int FS, li;
   bool write_ok, first_row, last_row, need_acc, need_un;
 
@@ -71,6 +71,8 @@ struct CellWriter {
       const long long idx = v * cells + gi;
       if (E.mode == 0) {
         E.out[idx] = div;
+      } else if (E.mode == 3) {
+        E.out[idx] = fma(kappa, nun, div);
       } else if (E.mode == 1) {
         E.out[idx] = nacc + div;
       } else {
@@ -162,7 +164,7 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
   }
   cp_async_commit();
 
-  const double dt = E.mode == 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
+  const double dt = E.mode >= 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
   CellWriter<LI> W{E};
   W.cells = G.cells;
   W.dt = dt;
@@ -172,7 +174,8 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
   W.first_row = lj == 0;
   W.last_row = lj == LJ - 1;
   W.need_acc = E.mode == 1 || (E.mode == 2 && E.has_acc);
-  W.need_un = E.mode == 2 && E.alpha != 0.0;
+  W.need_un = (E.mode == 2 && E.alpha != 0.0) || E.mode == 3;
+  W.kappa = E.mode == 3 ? E.alpha / (E.beta * dt) : 0.0;
   W.nacc = 0.0;
   W.nun = 0.0;
   const bool lane_ok = DIR == 0 || i0 + li <= imax;
@@ -455,10 +458,11 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
       tma_load_row((unsigned)__cvta_generic_to_shared(sms + (size_t)slot * SSLOT), &tmS, c0, DIR == 1 ? rc : co,
                    DIR == 1 ? co : rc, bar);
   };
-  const double dt = E.mode == 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
+  const double dt = E.mode >= 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
+  const double kappa = E.mode == 3 ? E.alpha / (E.beta * dt) : 0.0;   // mode 3: out = div + kappa U^n (see XfEpilogue)
   const double ninv = -G.inv_d[DIR];
   const bool need_acc = E.mode == 1 || (E.mode == 2 && E.has_acc);
-  const bool need_un = E.mode == 2 && E.alpha != 0.0;
+  const bool need_un = (E.mode == 2 && E.alpha != 0.0) || E.mode == 3;
 
   // cell row of face f (cell f - 1, staged at stencil row f + 2): Eq. 13 and the stage combination
   double d[NVS];
@@ -505,6 +509,8 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
           const long long idx = v * G.cells + gi;
           if (E.mode == 0) {
             E.out[idx] = d[v];
+          } else if (E.mode == 3) {
+            E.out[idx] = fma(kappa, un[q], d[v]);
           } else if (E.mode == 1) {
             E.out[idx] = a[q] + d[v];
           } else {
@@ -675,10 +681,11 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
     tma_load_span(dst + (unsigned)(OFFP * sizeof(double)), &tmP, c0, bar);
     tma_load_span(dst + (unsigned)(OFFS * sizeof(double)), &tmS, c0, bar);
   };
-  const double dt = E.mode == 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
+  const double dt = E.mode >= 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
+  const double kappa = E.mode == 3 ? E.alpha / (E.beta * dt) : 0.0;   // mode 3: out = div + kappa U^n (see XfEpilogue)
   const double ninv = -G.inv_d[0];
   const bool need_acc = E.mode == 1 || (E.mode == 2 && E.has_acc);
-  const bool need_un = E.mode == 2 && E.alpha != 0.0;
+  const bool need_un = (E.mode == 2 && E.alpha != 0.0) || E.mode == 3;
 
   // lane (w, lane) of the service group owns slot u of a chunk: cell fc + u - 1, between the chunk's faces u - 1 and u
   double d[NVS];
@@ -733,6 +740,8 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
           const long long idx = v * G.cells + gi;
           if (E.mode == 0) {
             E.out[idx] = d[v];
+          } else if (E.mode == 3) {
+            E.out[idx] = fma(kappa, un[q], d[v]);
           } else if (E.mode == 1) {
             E.out[idx] = a[q] + d[v];
           } else {
