@@ -559,3 +559,40 @@ def test_shock_tube_and_bubble_steps_wenocu6(oracle_mod):
         assert g.ctx.xf_status() == 0
         assert worst < STEPS_TOL, worst
         g.close()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# edge sizes: the smallest box the ghost fill admits, extents around the chunk sizes of the sweeps (x: 128 faces per
+# chunk, 16 chunks per segment; y/z: 4 face rows per chunk, 32 columns per strip), TMA and fallback paths
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape,n,bc", [
+    ((3, 3, 3), 2, (0,) * 6), ((3, 4, 5), 3, (1, 1, 2, 2, 0, 0)), ((4, 3, 1), 1, (2, 2, 1, 1, 0, 0)),
+    ((122, 4, 4), 2, (0,) * 6), ((123, 5, 3), 2, (0,) * 6), ((250, 8, 1), 3, (1, 1, 0, 0, 0, 0)),
+    ((32, 4, 8), 4, (0,) * 6), ((33, 5, 9), 4, (0,) * 6), ((64, 3, 12), 2, (0,) * 6), ((26, 13, 4), 10, (0,) * 6),
+])
+def test_rhs_parity_edge_sizes(oracle_mod, shape, n, bc):
+    w = wl.random_smooth_box(*shape, nspecies=n, seed=4000 + n + shape[0], bc=bc)
+    orc = oracle_mod.Oracle.from_workload(w)
+    Uo, To = w.U.copy(), w.T_guess.copy()
+    ro = orc.rhs(Uo, To)
+    assert orc.last_status == 0
+    g = _gpu(w)
+    err = field_err(w.interior(g.rhs()), w.interior(ro))
+    assert err.max() < RHS_TOL, err
+    S = g.max_wavespeed()
+    g.reset()
+    orc.rk3_step(Uo := w.U.copy(), To := w.T_guess.copy(), 0.4 / S)
+    g.step(0.4 / S)
+    assert state_err(w, g.host_U(), Uo, S * min(w.dx, w.dy, w.dz)).max() < 1e-12
+    g.close()
+
+
+def test_long_pencil_several_segments(oracle_mod):
+    """1-D, 2500 cells: two segments of the x sweep (2047 cells each) and a ragged last chunk; shock-tube data."""
+    w = wl.config1_shock_tube(nx=2500)
+    orc = oracle_mod.Oracle.from_workload(w)
+    ro = orc.rhs(w.U.copy(), w.T_guess.copy())
+    g = _gpu(w)
+    err = field_err(w.interior(g.rhs()), w.interior(ro))
+    assert err.max() < RHS_TOL, err
+    g.close()
