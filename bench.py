@@ -39,7 +39,7 @@ UNIT = "cell-updates/s"
 
 WORKLOADS = {
     # name: (generator, full grid, grid of the bounded oracle sample for cpu_baseline, grid of a --impl reference step)
-    "config4": ("config4_shock_bubble_3d_10sp", (512, 256, 256), (192, 96, 96), (128, 64, 64)),
+    "config4": ("config4_shock_bubble_3d_10sp", (512, 256, 256), (320, 160, 160), (128, 64, 64)),
     "config3": ("config3_shock_bubble_3d", (256, 256, 256), (128, 128, 128), (96, 96, 96)),
     "config2": ("config2_shock_bubble_2d", (2048, 1024, 1), (1024, 512, 1), (1024, 512, 1)),
 }
