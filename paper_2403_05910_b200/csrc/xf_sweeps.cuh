@@ -319,7 +319,6 @@ constexpr int BAR_SERVICE = 7;   // among the service warps: all have read U^s b
 #ifndef XF_WS_RC
 #define XF_WS_RC 168   // 2 blocks x 128 threads x (168 + 88) registers = the SM's 64 K
 #define XF_WS_RS 88
-#define XF_WS_VB 7     // fields whose global operands a service lane keeps in flight together
 #endif
 constexpr int WS_REGS_COMPUTE = XF_WS_RC, WS_REGS_SERVICE = XF_WS_RS;
 
@@ -478,45 +477,36 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
       for (int v = 0; v < Nv; ++v) fb[v * FBS + lane] = fb[v * FBS + W * 32 + lane];
     }
   };
-  auto prefetch_operands = [&](int f) {                     // the update's global operands of cell row f -> L2
-    if (!(f > f_begin && f <= f_end) || (lane & 15) != 0) return;
+  // The update reads ONE global operand per component: the partial residual (modes 1, 2 after an earlier sweep) or U^n
+  // (mode 3, or mode 2 when this is the only sweep) -- never both (xf_api.cu: residual()).  It is requested BEFORE the
+  // service warp waits for the chunk's fluxes, so the loads fly while the compute warps are still at work and the
+  // part after the barrier is short.
+  const double *__restrict__ opnd_src = need_acc ? E.acc : E.Un;
+  const bool need_opnd = need_acc || need_un;
+  double opnd[NVS];
+  auto load_operands = [&](int f) {
+    if (!need_opnd || !(f > f_begin && f <= f_end) || !lane_ok) return;
     const long long gi = colbase + (long long)(f + 2) * sst;
-    for (int v = 0; v < Nv; ++v) {
-      if (need_acc) asm volatile("prefetch.global.L2 [%0];" ::"l"(E.acc + v * G.cells + gi));
-      if (need_un) asm volatile("prefetch.global.L2 [%0];" ::"l"(E.Un + v * G.cells + gi));
-    }
+#pragma unroll
+    for (int v = 0; v < NVS; ++v)
+      if (v < Nv) opnd[v] = opnd_src[v * G.cells + gi];
   };
-  auto write_cells = [&](int f) {                           // part 2: global operands, Eq. 16, stores
+  auto write_cells = [&](int f) {                           // part 2: Eq. 13 / Eq. 16 and the stores
     if (!(f > f_begin && f <= f_end) || !lane_ok) return;
     const long long gi = colbase + (long long)(f + 2) * sst;
-    constexpr int VB = XF_WS_VB;                                   // fields per batch: all loads of a batch fly together
 #pragma unroll
-    for (int v0 = 0; v0 < NVS; v0 += VB) {
-      double a[VB], un[VB];
-#pragma unroll
-      for (int q = 0; q < VB; ++q) {
-        const int v = v0 + q;
-        if (v < Nv && v < NVS) {
-          const long long idx = v * G.cells + gi;
-          a[q] = need_acc ? E.acc[idx] : 0.0;
-          un[q] = need_un ? E.Un[idx] : 0.0;
-        }
-      }
-#pragma unroll
-      for (int q = 0; q < VB; ++q) {
-        const int v = v0 + q;
-        if (v < Nv && v < NVS) {
-          const long long idx = v * G.cells + gi;
-          if (E.mode == 0) {
-            E.out[idx] = d[v];
-          } else if (E.mode == 3) {
-            E.out[idx] = fma(kappa, un[q], d[v]);
-          } else if (E.mode == 1) {
-            E.out[idx] = a[q] + d[v];
-          } else {
-            const double L = need_acc ? fma(dt, a[q], d[v]) : d[v];   // U^s + dt (acc + div)
-            E.out[idx] = need_un ? fma(E.alpha, un[q], E.beta * L) : E.beta * L;
-          }
+    for (int v = 0; v < NVS; ++v) {
+      if (v < Nv) {
+        const long long idx = v * G.cells + gi;
+        if (E.mode == 0) {
+          E.out[idx] = d[v];
+        } else if (E.mode == 3) {
+          E.out[idx] = fma(kappa, opnd[v], d[v]);
+        } else if (E.mode == 1) {
+          E.out[idx] = opnd[v] + d[v];
+        } else {
+          const double L = need_acc ? fma(dt, opnd[v], d[v]) : d[v];   // U^s + dt (acc + div)
+          E.out[idx] = need_un ? fma(E.alpha, opnd[v], E.beta * L) : E.beta * L;
         }
       }
     }
@@ -540,6 +530,7 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
       named_arrive(BAR_RING_FULL + par, NT);                // this chunk's rows have landed
     }
     if (!first) {
+      load_operands(fprev);
       named_sync(BAR_FLUX_READY + (par ^ 1), NT);           // the previous chunk's fluxes are in fb, its ring rows are dead
       read_fluxes(ous);
       named_arrive(BAR_FB_EMPTY + par, NT);
@@ -558,7 +549,6 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
       }
     }
     cp_async_commit();
-    prefetch_operands(fc + w);                              // read one chunk later
     if (!first) write_cells(fprev);
     fprev = fc + w;
     {                                                       // where U^s of that cell row (stencil row f + 2) sits
@@ -573,6 +563,7 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
     par ^= 1;
     first = false;
   }
+  load_operands(fprev);
   named_sync(BAR_FLUX_READY + (par ^ 1), NT);               // the last chunk
   read_fluxes(ous);
   write_cells(fprev);
@@ -708,46 +699,33 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
     const int i = cf % G.np[0];
     return i >= G.g[0] && i < G.g[0] + G.n[0];
   };
-  auto prefetch_operands = [&](int fc) {
-    const int cf = fc + u - 1;
-    if (!(need_acc || need_un) || (lane & 15) != 0 || cf < f_begin || cf >= f_end) return;
-    const long long gi = P0 + cf;
-    for (int v = 0; v < Nv; ++v) {
-      if (need_acc) asm volatile("prefetch.global.L2 [%0];" ::"l"(E.acc + v * G.cells + gi));
-      if (need_un) asm volatile("prefetch.global.L2 [%0];" ::"l"(E.Un + v * G.cells + gi));
-    }
+  // one global operand per component, requested before the wait for the chunk's fluxes (see the y/z kernel)
+  const double *__restrict__ opnd_src = need_acc ? E.acc : E.Un;
+  const bool need_opnd = need_acc || need_un;
+  double opnd[NVS];
+  auto load_operands = [&](int fc) {
+    long long gi;
+    if (!need_opnd || !cell_index(fc, gi)) return;
+#pragma unroll
+    for (int v = 0; v < NVS; ++v)
+      if (v < Nv) opnd[v] = opnd_src[v * G.cells + gi];
   };
   auto write_cells = [&](int fc) {
     long long gi;
     if (!cell_index(fc, gi)) return;
-    constexpr int VB = XF_WS_VB;
 #pragma unroll
-    for (int v0 = 0; v0 < NVS; v0 += VB) {
-      double a[VB], un[VB];
-#pragma unroll
-      for (int q = 0; q < VB; ++q) {
-        const int v = v0 + q;
-        if (v < Nv && v < NVS) {
-          const long long idx = v * G.cells + gi;
-          a[q] = need_acc ? E.acc[idx] : 0.0;
-          un[q] = need_un ? E.Un[idx] : 0.0;
-        }
-      }
-#pragma unroll
-      for (int q = 0; q < VB; ++q) {
-        const int v = v0 + q;
-        if (v < Nv && v < NVS) {
-          const long long idx = v * G.cells + gi;
-          if (E.mode == 0) {
-            E.out[idx] = d[v];
-          } else if (E.mode == 3) {
-            E.out[idx] = fma(kappa, un[q], d[v]);
-          } else if (E.mode == 1) {
-            E.out[idx] = a[q] + d[v];
-          } else {
-            const double Lr = need_acc ? fma(dt, a[q], d[v]) : d[v];   // U^s + dt (acc + div)
-            E.out[idx] = need_un ? fma(E.alpha, un[q], E.beta * Lr) : E.beta * Lr;
-          }
+    for (int v = 0; v < NVS; ++v) {
+      if (v < Nv) {
+        const long long idx = v * G.cells + gi;
+        if (E.mode == 0) {
+          E.out[idx] = d[v];
+        } else if (E.mode == 3) {
+          E.out[idx] = fma(kappa, opnd[v], d[v]);
+        } else if (E.mode == 1) {
+          E.out[idx] = opnd[v] + d[v];
+        } else {
+          const double Lr = need_acc ? fma(dt, opnd[v], d[v]) : d[v];   // U^s + dt (acc + div)
+          E.out[idx] = need_un ? fma(E.alpha, opnd[v], E.beta * Lr) : E.beta * Lr;
         }
       }
     }
@@ -758,18 +736,19 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
   bool first = true;
   for (int fc = f_begin; fc <= f_end; fc += XW_CH) {
     if (!first) {
+      load_operands(fprev);
       named_sync(BAR_FLUX_READY + (par ^ 1), NT);           // the previous chunk's fluxes are in fb, its stage is free
       read_fluxes(par ^ 1);
       named_arrive(BAR_FB_EMPTY + par, NT);
       if (E.mode == 2) named_sync(BAR_SERVICE, 32 * W);     // U^s was read from the stage the next copy overwrites
     }
     if (fc + XW_CH <= f_end) stage_chunk(fc + XW_CH, par ^ 1);
-    prefetch_operands(fc);
     if (!first) write_cells(fprev);
     fprev = fc;
     par ^= 1;
     first = false;
   }
+  load_operands(fprev);
   named_sync(BAR_FLUX_READY + (par ^ 1), NT);               // the last chunk
   read_fluxes(par ^ 1);
   write_cells(fprev);
