@@ -18,7 +18,7 @@ namespace xf {
 
 // WENO5-JS value at +1/2 from point values v0..v4 = v_{-2}..v_{+2} (Jiang & Shu; eps = 1e-6, exponent 2).
 // Written on first differences D_k; smoothness indicators scaled by 4 (cancels in the weights);
-//   result = v2 + (D2 + 2 D3)/6 + [ (2/3) P0 (d0 - d1) + P2 (d1 - d2) ] / [ 2 P0 + 12 P1 + 6 P2 ],
+//   result = v2 + (D2 + 2 D3)/6 + [ (2/3) P0 (d0 - d1) + P2 (d1 - d2) ] / [ 2 (P0 + 6 P1 + 3 P2) ],
 // with P0 = (s1 s2)^2, P1 = (s0 s2)^2, P2 = (s0 s1)^2, s_k = 4 (eps + beta_k): the Jiang-Shu weights
 // d_k/(eps+beta_k)^2 brought to a common denominator, so one reciprocal instead of four divisions.
 #ifndef XF_SPECIES_UNROLL
@@ -42,14 +42,16 @@ __device__ __forceinline__ void weno5_parts(double v0, double v1, double v2, dou
   const double p12 = s1 * s2, p02 = s0 * s2, p01 = s0 * s1;
   const double P0 = p12 * p12, P1 = p02 * p02, P2 = p01 * p01;
   num = fma(P0 * (d0 - d1), 2.0 / 3.0, P2 * (d1 - d2));
-  den = fma(2.0, P0, fma(12.0, P1, 6.0 * P2));
+  den = fma(6.0, P1, fma(3.0, P2, P0));   // HALF the common denominator: the caller halves the reciprocal (exponent - 1)
   base = fma(fma(2.0, D3, D2), 1.0 / 6.0, v2);
 }
 
 __device__ __forceinline__ double weno5(double v0, double v1, double v2, double v3, double v4) {
   double num, den, base;
   weno5_parts(v0, v1, v2, v3, v4, num, den, base);
-  return fma(num, xf_rcp(den), base);
+  // 1/(2 den): the factor 1/2 is an integer subtraction on the exponent field, not an fp64-pipe instruction
+  const double rh = __longlong_as_double(__double_as_longlong(xf_rcp(den)) - (1ll << 52));
+  return fma(num, rh, base);
 }
 
 // WENO-CU6 (include/xf.h XF_RECON_WENOCU6; PAPER.md:107 ref 34) value at +1/2 from v0..v5 = v_{-2}..v_{+3}.
