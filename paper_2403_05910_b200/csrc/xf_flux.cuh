@@ -199,6 +199,11 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const d
     lam_p = lamg[2];
   }
 
+  double hud[6];
+#pragma unroll
+  for (int m = 0; m < 6; ++m) hud[m] = 0.5 * ud[m];
+  const double hlm = 0.5 * lam_m, hl0 = 0.5 * lam_0, hlp = 0.5 * lam_p;
+
   // ---- acoustic (u-c), entropy (u) and acoustic (u+c) fields
   double g0, g1, gL;
   {
@@ -207,24 +212,24 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const d
     for (int m = 0; m < 6; ++m) {
       const double a = h * fma(-ct, nuU[m], piU[m]);
       const double pt = qp[m] - rp[m];
-      fp[m] = fma(0.5 * (ud[m] + lam_m), a, pt);
-      fm[m] = fma(0.5 * (ud[m] - lam_m), a, pt);
+      fp[m] = fma(hud[m] + hlm, a, pt);   // (u_m + Lambda)/2: halving is exact, so the halves are formed once
+      fm[m] = fma(hud[m] - hlm, a, pt);
     }
     g0 = weno_pair<RECON>(fp, fm);
 #pragma unroll
     for (int m = 0; m < 6; ++m) {
       const double a = h * fma(ct, nuU[m], piU[m]);
       const double pt = qp[m] + rp[m];
-      fp[m] = fma(0.5 * (ud[m] + lam_p), a, pt);
-      fm[m] = fma(0.5 * (ud[m] - lam_p), a, pt);
+      fp[m] = fma(hud[m] + hlp, a, pt);
+      fm[m] = fma(hud[m] - hlp, a, pt);
     }
     gL = weno_pair<RECON>(fp, fm);
   }
   double ap[6], am[6];  // (u_m +- Lambda_u)/2 for all fields that travel with u
 #pragma unroll
   for (int m = 0; m < 6; ++m) {
-    ap[m] = 0.5 * (ud[m] + lam_0);
-    am[m] = 0.5 * (ud[m] - lam_0);
+    ap[m] = hud[m] + hl0;
+    am[m] = hud[m] - hl0;
   }
   {
     double fp[6], fm[6];
