@@ -238,7 +238,7 @@ def measured_peaks() -> dict:
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
 # capture (profiles/); None until a capture of that (workload, kernel) exists.
-NCU_TRAFFIC_BYTES = {  # profiles/r1d_ncu_full.md
+NCU_TRAFFIC_BYTES = {  # profiles/r1e_ncu_full.md
     ("config4", "sweep_x"): 11.55e9, ("config4", "sweep_y"): 15.40e9, ("config4", "sweep_z"): 15.45e9,
 }
 
