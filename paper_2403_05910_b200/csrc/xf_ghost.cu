@@ -46,14 +46,28 @@ ghost_kernel(const XfGrid G, int Nv, int d, int bc_lo, int bc_hi, const double *
   const long long base = (long long)p1 * G.st[a1] + (long long)p2 * G.st[a2];
   const long long ig = base + (long long)ighost * G.st[d];
   const long long is = base + (long long)isrc * G.st[d];
-  for (int v = 0; v < Nv; ++v) {
-    double val;
-    if (bc == XF_BC_DIRICHLET) val = bc_state[(2 * d + side) * XF_MAXNV + v];
-    else {
-      val = U[v * G.cells + is];
-      if (bc == XF_BC_REFLECTIVE && v == 1 + d) val = -val;  // wall-normal momentum negated
+  // U is read and written: the compiler must keep every load behind the previous store.  Batches of loads first, then
+  // their stores (a ghost cell is never a source of the same launch: sources are interior along d), so a thread has
+  // several loads in flight instead of one.
+  constexpr int VB = 7;
+  for (int v0 = 0; v0 < Nv; v0 += VB) {
+    double val[VB];
+#pragma unroll
+    for (int q = 0; q < VB; ++q) {
+      const int v = v0 + q;
+      if (v < Nv) {
+        if (bc == XF_BC_DIRICHLET) val[q] = bc_state[(2 * d + side) * XF_MAXNV + v];
+        else {
+          val[q] = U[v * G.cells + is];
+          if (bc == XF_BC_REFLECTIVE && v == 1 + d) val[q] = -val[q];  // wall-normal momentum negated
+        }
+      }
     }
-    U[v * G.cells + ig] = val;
+#pragma unroll
+    for (int q = 0; q < VB; ++q) {
+      const int v = v0 + q;
+      if (v < Nv) U[v * G.cells + ig] = val[q];
+    }
   }
 }
 
