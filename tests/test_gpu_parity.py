@@ -596,3 +596,32 @@ def test_long_pencil_several_segments(oracle_mod):
     err = field_err(w.interior(g.rhs()), w.interior(ro))
     assert err.max() < RHS_TOL, err
     g.close()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# BASELINE.json's step counts at full size (beyond the oracle's reach, checked by properties that hold
+# at any size): the run stays physical (status word clean, rho, T > 0, all finite), the time step from the device
+# and the part of the domain no wave has reached yet is still the initial state
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,steps", [("config2", 500), ("config3", 200), ("config4", 100)])
+def test_full_size_runs_stay_physical(name, steps):
+    import torch
+
+    w = {"config2": lambda: wl.config2_shock_bubble_2d(2048, 1024),
+         "config3": lambda: wl.config3_shock_bubble_3d(256),
+         "config4": lambda: wl.config4_shock_bubble_3d_10sp(512, 256, 256)}[name]()
+    g = _gpu(w)
+    U0 = g.U.clone()
+    for _ in range(steps):
+        g.ctx.xf_step_cfl(g.U, g.T, w.cfl, g.S, g.work)
+    assert g.ctx.xf_status() == 0
+    Ui = w_interior(g.U, w)
+    assert bool(torch.isfinite(Ui).all()) and float(Ui[0].min()) > 0.0
+    Ti = w_interior(g.T.unsqueeze(0), w)
+    assert float(Ti.min()) > 0.0
+    # the quiescent gas far downstream (last tenth of the x extent) has not been reached by any wave and is untouched
+    # (not bit for bit: 1/3 U + 2/3 U rounds)
+    far = slice(int(0.9 * w.nx), w.nx)
+    a, b = w_interior(g.U, w)[..., far], w_interior(U0, w)[..., far]
+    assert float((a - b).abs().max()) <= 1e-12 * float(b.abs().max())
+    g.close()
