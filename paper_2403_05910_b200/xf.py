@@ -172,7 +172,8 @@ class Context:
 
     def close(self) -> None:
         if getattr(self, "_h", None) is not None and self._h.value:
-            lib().xf_destroy(self._h)
+            if _lib is not None:                   # at interpreter shutdown the module globals may be gone already
+                _lib.xf_destroy(self._h)
             self._h = C.c_void_p()
 
     __del__ = close
