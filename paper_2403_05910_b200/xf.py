@@ -171,10 +171,10 @@ class Context:
         return cls(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, t.W, t.nasa7, t.Ru, t.Tlo, t.Thi, wl.bc, wl.bc_state, **kw)
 
     def close(self) -> None:
-        if getattr(self, "_h", None) is not None and self._h.value:
-            if _lib is not None:                   # at interpreter shutdown the module globals may be gone already
-                _lib.xf_destroy(self._h)
-            self._h = C.c_void_p()
+        h = getattr(self, "_h", None)
+        if h is not None and h.value and _lib is not None:   # at interpreter shutdown the module globals may be gone
+            _lib.xf_destroy(h)
+        self._h = None
 
     __del__ = close
 
