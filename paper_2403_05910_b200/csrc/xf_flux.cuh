@@ -170,6 +170,7 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const d
   const double h = 0.5 * xf_rcp(c2);  // 1/(2 c~^2)
   const double Prho = fma(Gt, kt, chiN);
 
+  const double hh = 0.5 * h, ghh = Gt * hh, chh = ct * hh;
   double nuU[6], ud[6], qp[6], rp[6];
   double lam_m = 0.0, lam_0 = 0.0, lam_p = 0.0;  // LLF: max over the stencil of |u-c|, |u|, |u+c| (reading R8)
 #pragma unroll
@@ -185,9 +186,9 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const d
       lam_0 = fmax(lam_0, fabs(ud[m]));
       lam_p = fmax(lam_p, fabs(ud[m] + cm));
     }
-    const double ph = 0.5 * XP(m) * h;             // p_m / (4 c~^2)
-    qp[m] = Gt * (ud[m] - ut[nd]) * ph;                // pressure terms of L F_m
-    rp[m] = ct * ph;
+    const double pm = XP(m);                           // pressure terms of L F_m, with p_m / (4 c~^2) = hh p_m:
+    qp[m] = (ghh * pm) * (ud[m] - ut[nd]);             //   Gamma~ (u_m - u~) p_m / (4 c~^2)
+    rp[m] = chh * pm;                                  //   c~ p_m / (4 c~^2)
   }
   if (visc == XF_VISC_ROE) {          // |lambda_n| of the Roe-averaged state (warp-uniform branch)
     lam_m = fabs(ut[nd] - ct);
