@@ -153,13 +153,39 @@ def oracle_step_seconds(w, steps: int, warmup: int = 0):
     return time.perf_counter() - t0
 
 
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def cpu_baseline(name: str) -> dict:
     grid = WORKLOADS[name][2]
     w = make_workload(name, grid)
     sec = oracle_step_seconds(w, 1)
-    return {"value": w.interior_cells * 3 / sec, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle",
-            "sample": f"1 step (max wave speed + RK3 = 3 RHS) of {name} generated at {grid[0]}x{grid[1]}x{grid[2]} "
-                      f"(same set-up, reduced grid), {sec:.1f} s, oracle/xf_oracle.c with OpenMP"}
+    out = {"value": w.interior_cells * 3 / sec, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle",
+           "cpu": cpu_model(),
+           "sample": f"1 step (max wave speed + RK3 = 3 RHS) of {name} generated at {grid[0]}x{grid[1]}x{grid[2]} "
+                     f"(same set-up, reduced grid), {sec:.1f} s, oracle/xf_oracle.c with OpenMP"}
+    # the one-thread figure on a smaller sample of the same set-up
+    try:
+        import ctypes
+
+        gomp = ctypes.CDLL("libgomp.so.1")
+        small = tuple(max(8, g // 4) for g in grid)
+        w1 = make_workload(name, small)
+        gomp.omp_set_num_threads(1)
+        sec1 = oracle_step_seconds(w1, 1)
+        gomp.omp_set_num_threads(oracle_threads())
+        out["one_thread_value"] = w1.interior_cells * 3 / sec1
+        out["one_thread_sample"] = f"{small[0]}x{small[1]}x{small[2]}, {sec1:.1f} s"
+    except OSError:
+        pass
+    return out
 
 
 def run_reference(args, rank: int, world: int) -> None:
