@@ -339,6 +339,7 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
                    const XfEpilogue E, int *__restrict__ status, const int seg_len,
                    const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmP,
                    const __grid_constant__ CUtensorMap tmS) {
+  static_assert(W >= 3, "the service warps' ring-row hand-over needs W >= 3");
   const int N = N_T > 0 ? N_T : Nrt;
   const int Nv = N + 4, NST = nstaged(N);
   constexpr int NVS = N_T > 0 ? N_T + 4 : XF_MAXNV;        // static bound of Nv for register arrays
@@ -534,14 +535,17 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
       named_sync(BAR_FLUX_READY + (par ^ 1), NT);           // the previous chunk's fluxes are in fb, its ring rows are dead
       read_fluxes(ous);
       named_arrive(BAR_FB_EMPTY + par, NT);
-      if (E.mode == 2) named_sync(BAR_SERVICE, 32 * W);     // U^s was read from ring rows the next copies overwrite
     }
-    if (fc + W <= f_end) {                                  // the W new rows of the next chunk: row fc + W + 5 + w
-      int slot = rb + W + 5 + w;
+    if (fc + W <= f_end) {                                  // the W new rows of the next chunk: rows fc + W + 5 + q
+      // warp w fetches row q = (w + 2) mod W: it lands in the ring slot of the previous chunk's row q, and the only
+      // service warp that has just read U^s from that slot (stencil row f + 2 of its cell row) is warp q - 2 = w
+      // itself; rows 0 and 1 hold no cell of the previous chunk.  So no barrier among the service warps is needed.
+      const int q = w + 2 < W ? w + 2 : w + 2 - W;
+      int slot = rb + W + 5 + q;
       slot -= slot >= RR ? RR : 0;
       const unsigned bar = full_bar + 8 * (par ^ 1);
       if (TMA && lane == 0) mbar_expect_tx(bar, deep_bytes + shallow_bytes);
-      stage_row(slot, fc + W + 5 + w, bar);
+      stage_row(slot, fc + W + 5 + q, bar);
       if (TMA) {                                            // shallow row fc + W + 3 + w
         int q = rs + W + 1 + w;
         q -= q >= RS ? RS : 0;
