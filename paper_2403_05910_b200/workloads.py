@@ -450,6 +450,92 @@ def config5_random_states(nx: int = 640, ny: int = 384, nz: int = 384, seed: Opt
                    rng, steps=1, notes={"Ru": Ru})
 
 
+def config5_random_states_device(nx: int = 640, ny: int = 384, nz: int = 384, device="cuda:0", seed: Optional[int] = None):
+    """BASELINE.json configs[4] at its stated size, generated ON THE DEVICE with torch (94 M cells x 14 variables take
+    minutes with numpy on the host, seconds here).  Same recipe as ``config5_random_states`` -- log-uniform rho and p,
+    Dirichlet(0.5) mass fractions, velocities in +-2 local sound speeds, Ru such that the median T is 1000 K, three
+    passes of a periodic 3x3x3 box filter on the conserved variables -- with torch's seeded CUDA generator, so the
+    numbers differ from the numpy variant's.  Returns a ``Workload`` whose ``U`` / ``T_guess`` are padded torch tensors
+    on ``device`` (ghosts unfilled: the path fills them); the oracle side of the parity test receives a sub-block copied
+    to the host (``periodic_subblock_arrays``)."""
+    import torch
+
+    dev = torch.device(device)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(SEED_BASE + 5 if seed is None else seed)
+    shape = (nz, ny, nx)
+    f64 = dict(dtype=torch.float64, device=dev)
+
+    def uniform(lo, hi):
+        return lo + (hi - lo) * torch.rand(shape, generator=gen, **f64)
+
+    tab1 = table10(Ru=1.0)
+    rho = 10.0 ** uniform(-1.0, 1.0)
+    p = 10.0 ** uniform(-1.0, 2.0)
+    Y = torch._standard_gamma(torch.full((10,) + shape, 0.5, **f64), generator=gen)   # Dirichlet = normalised Gamma
+    Y /= Y.sum(dim=0, keepdim=True)
+    Wt = torch.tensor(tab1.W, **f64).reshape(10, 1, 1, 1)
+    Wbar = 1.0 / (Y / Wt).sum(dim=0)
+    t_unit = p * Wbar / rho                                   # T * Ru
+    Ru = float(torch.median(t_unit.reshape(-1)).item() / 1000.0)
+    table = table10(Ru=Ru)
+    T = t_unit / Ru
+    del t_unit, p, Wbar
+    # forward evaluation of the table (input generation only): cp/R, h/R per species with the constant-cp continuation
+    a = torch.tensor(table.nasa7, **f64)
+    Rs = torch.tensor(table.Rs, **f64)
+    Tc = T.clamp(table.Tlo, table.Thi)
+    cp_mix = torch.zeros(shape, **f64)
+    h_mix = torch.zeros(shape, **f64)
+    R_mix = torch.zeros(shape, **f64)
+    for s_ in range(10):
+        cpR = a[s_, 0] + Tc * (a[s_, 1] + Tc * (a[s_, 2] + Tc * (a[s_, 3] + Tc * a[s_, 4])))
+        hR = Tc * (a[s_, 0] + Tc * (a[s_, 1] / 2 + Tc * (a[s_, 2] / 3 + Tc * (a[s_, 3] / 4 + Tc * a[s_, 4] / 5)))) + a[s_, 5]
+        hR = hR + cpR * (T - Tc)
+        cp_mix += Y[s_] * Rs[s_] * cpR
+        h_mix += Y[s_] * Rs[s_] * hR
+        R_mix += Y[s_] * Rs[s_]
+    del Tc, cpR, hR
+    c = torch.sqrt(cp_mix / (cp_mix - R_mix) * R_mix * T)
+    e = h_mix - R_mix * T
+    del cp_mix, h_mix, R_mix, T
+    U = torch.empty((14,) + shape, **f64)
+    U[0] = rho
+    k2 = torch.zeros(shape, **f64)
+    for q, n_ in enumerate((nx, ny, nz)):
+        vel = uniform(-2.0, 2.0) * c if n_ > 1 else torch.zeros(shape, **f64)
+        U[1 + q] = rho * vel
+        k2 += vel * vel
+    U[4] = rho * (e + 0.5 * k2)
+    for s_ in range(9):
+        U[5 + s_] = rho * Y[s_]
+    del Y, e, k2, vel, c, rho
+    for _ in range(3):
+        for k in range(14):
+            A = U[k]
+            for ax in (-1, -2, -3):
+                if A.shape[ax] > 1:
+                    A = (torch.roll(A, 1, dims=ax) + A + torch.roll(A, -1, dims=ax)) / 3.0
+            U[k] = A
+    gx, gy, gz = (NG if n_ > 1 else 0 for n_ in (nx, ny, nz))
+    Up = torch.zeros((14, nz + 2 * gz, ny + 2 * gy, nx + 2 * gx), **f64)
+    Up[:, gz:gz + nz, gy:gy + ny, gx:gx + nx] = U
+    del U
+    Tg = torch.full(Up.shape[1:], 1000.0, **f64) * (1.0 + 0.02 * (2.0 * torch.rand(Up.shape[1:], generator=gen, **f64) - 1.0))
+    d = 1.0 / 384.0
+    return Workload(name="config5_random_10sp_device", nx=nx, ny=ny, nz=nz, dx=d, dy=d if ny > 1 else 1.0,
+                    dz=d if nz > 1 else 1.0, table=table, bc=(BC_PERIODIC,) * 6, U=Up, T_guess=Tg, steps=1,
+                    notes={"Ru": Ru})
+
+
+def periodic_subblock_arrays(wl: Workload, Ui: np.ndarray, Ti: np.ndarray) -> Workload:
+    """A stand-alone transmissive workload from an already cut interior block Ui [Nv, n, n, n], Ti [n, n, n]."""
+    n = Ui.shape[-1]
+    return Workload(name=wl.name + "_subblock", nx=n, ny=n, nz=n, dx=wl.dx, dy=wl.dy, dz=wl.dz, table=wl.table,
+                    bc=(BC_TRANSMISSIVE,) * 6, U=_pad(np.ascontiguousarray(Ui), n, n, n),
+                    T_guess=_pad(np.ascontiguousarray(Ti), n, n, n), steps=1)
+
+
 def periodic_subblock(wl: Workload, origin: Tuple[int, int, int], size: int, margin: int) -> Workload:
     """Cut the (size + 2 margin)^3 block around ``origin`` (interior index of the inner block's first cell, x y z)
     out of a periodic workload, with periodic wrap, as a stand-alone workload with transmissive ends.  After one

@@ -77,3 +77,22 @@ for a_ in range(n):
     lines.append(f"row{a_}=" + ",".join(row))
 (Path(__file__).resolve().parent / "wenocu6_beta6_form.txt").write_text("\n".join(lines) + "\n")
 print("\n".join(lines))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# WENO-CU6: beta_6 of a smooth wave at 150 points per wavelength, exact (the case behind reading R16: in doubles the
+# value form above loses ~1e-12 of the cell-to-cell difference to cancellation there)
+# ---------------------------------------------------------------------------------------------------------------
+import math  # noqa: E402
+
+C = [[int(x) for x in ln.split("=")[1].split(",")] for ln in lines if ln.startswith("row")]
+out_lines = ["# six doubles v_{i-2}..v_{i+3} (hex) of v(x) = 2 + sin 2 pi x + 0.3 cos 6 pi x at 150 points per unit; beta_6",
+             "# (hex, rounded once) from the exact quadratic form of wenocu6_beta6_form.txt evaluated with",
+             "# fractions.Fraction on those very doubles; written by tests/golden/make_golden.py"]
+for j0 in range(0, 150, 19):
+    vs = [2.0 + math.sin(2 * math.pi * (j0 + m) / 150) + 0.3 * math.cos(6 * math.pi * (j0 + m) / 150) for m in range(6)]
+    f = [Fr(x) for x in vs]
+    b6 = sum(C[a_][k] * f[a_] * f[a_ + k] for a_ in range(6) for k in range(6 - a_)) / 120960
+    out_lines.append(",".join(x.hex() for x in vs) + ";" + float(b6).hex())
+(Path(__file__).resolve().parent / "wenocu6_beta6_smooth.txt").write_text("\n".join(out_lines) + "\n")
+print("\n".join(out_lines))

@@ -7,8 +7,6 @@ components share one scale so that an identically zero component does not divide
 """
 from __future__ import annotations
 
-import os
-
 import numpy as np
 import pytest
 
@@ -220,16 +218,18 @@ def _multi_step(oracle_mod, w, steps):
     return worst
 
 
+# SURVEY.md 8(d) table / BASELINE.md section 3: 200 steps at 512x256, 200 at 64^3, 100 at 128x64x64 (same generators, same
+# physical set-up as the full-size configs; about 35 s, 70 s and 70 s of the oracle on 16 cores)
 def test_config2_reduced_200_steps(oracle_mod):
-    assert _multi_step(oracle_mod, wl.config2_shock_bubble_2d(256, 128), 200) < STEPS_TOL
+    assert _multi_step(oracle_mod, wl.config2_shock_bubble_2d(512, 256), 200) < STEPS_TOL
 
 
-def test_config3_reduced_steps(oracle_mod):
-    assert _multi_step(oracle_mod, wl.config3_shock_bubble_3d(40), 40) < STEPS_TOL
+def test_config3_reduced_200_steps(oracle_mod):
+    assert _multi_step(oracle_mod, wl.config3_shock_bubble_3d(64), 200) < STEPS_TOL
 
 
-def test_config4_reduced_steps(oracle_mod):
-    assert _multi_step(oracle_mod, wl.config4_shock_bubble_3d_10sp(64, 32, 32), 20) < STEPS_TOL
+def test_config4_reduced_100_steps(oracle_mod):
+    assert _multi_step(oracle_mod, wl.config4_shock_bubble_3d_10sp(128, 64, 64), 100) < STEPS_TOL
 
 
 def test_config5_subblock_one_rk3_step(oracle_mod):
@@ -403,10 +403,6 @@ def test_full_size_rhs_on_sampled_cells(oracle_mod, name):
     orc.fill_ghosts(Uo)
     assert np.array_equal(Ug, Uo)                             # ghost fill: bit-exact at full size
     nv = w.nvars
-    scale = np.abs(w.interior(r)).reshape(nv, -1).max(axis=1)
-    scale[1:4] = scale[1:4].max()                             # momentum components share their scale (R14)
-    scale[5:] = np.maximum(scale[5:], scale[0])               # a trace species is measured against the density row:
-    #   its flux differences carry the round-off of the O(1) characteristic variables they are assembled from
     # samples: the cells with the largest |rhs| of the density equation (shock, bubble surface), a seeded uniform
     # draw, and the domain corners / block-boundary neighbourhoods of the sweeps (i around multiples of 32 and 128)
     rng = np.random.default_rng(wl.SEED_BASE + 99)
@@ -427,55 +423,70 @@ def test_full_size_rhs_on_sampled_cells(oracle_mod, name):
     ro = orc.rhs_cells(Uo, w.T_guess, idx)                    # [samples, Nv]
     assert orc.last_status == 0
     rg = r.reshape(nv, -1)[:, idx].T
+    # reading R14, strictly: every variable -- the trace species of config 4 (Y ~ 1e-8 .. 1e-4) included -- is measured
+    # against ITS OWN scale, taken from the oracle's values (the samples contain the cells with the largest residuals)
+    scale = np.abs(ro).max(axis=0)
+    scale[1:4] = scale[1:4].max()                             # momentum components share their scale (R14)
     err = np.abs(rg - ro).max(axis=0) / scale
+    print(f"{name}: per-variable error on own scale", err)
     assert err.max() < RHS_TOL, err
 
 
-@pytest.mark.skipif(os.environ.get("XF_FULL_CONFIG5") != "1",
-                    reason="3 min of host-side generation (94 M cells): set XF_FULL_CONFIG5=1; result in DESIGN.md section 8")
 def test_config5_full_size_subblock(oracle_mod):
-    """BASELINE.json configs[4] as stated: 640x384x384 periodic random states, 50 back-to-back RHS evaluations (status
-    only), then one RK3 step checked against the oracle on a seeded 64^3 sub-block (+9 cells of margin)."""
+    """BASELINE.json configs[4] as stated: 640x384x384 periodic random states (generated on the device, see
+    workloads.config5_random_states_device), 50 back-to-back RHS evaluations with the T guess restored (status only),
+    then one RK3 step checked against the oracle on a seeded 64^3 sub-block (+9 cells of margin = 3 stages x 3 cells)."""
     import torch
 
-    w = wl.config5_random_states()
-    g = _gpu(w)
-    out = torch.empty_like(g.U)
-    g.ctx.xf_convective_rhs(g.U, g.T, out, g.work)
-    Tconv = g.T.clone()
-    gen = torch.Generator(device="cuda")
-    gen.manual_seed(5)
-    Tg = Tconv * (1 + 0.02 * (2 * torch.rand(Tconv.shape, generator=gen, device="cuda", dtype=torch.float64) - 1))
+    from paper_2403_05910_b200 import xf
+
+    w = wl.config5_random_states_device()
+    ctx = xf.Context.from_workload(w)
+    U, Tg = w.U, w.T_guess
+    T = Tg.clone()
+    work = ctx.workspace()
+    out = torch.empty_like(U)
     for _ in range(50):
-        g.T.copy_(Tg)
-        g.ctx.xf_convective_rhs(g.U, g.T, out, g.work)
-    assert g.ctx.xf_status() == 0
-    g.T.copy_(Tg)
-    S = g.max_wavespeed()
+        T.copy_(Tg)
+        ctx.xf_convective_rhs(U, T, out, work)
+    assert ctx.xf_status() == 0
+    frac_out = float(((T < 200.0) | (T > 3000.0)).double().mean())
+    assert frac_out > 0.01                                    # the continuation branch (reading R3) is exercised
+    del out
+    S_dev = torch.zeros(1, dtype=torch.float64, device=U.device)
+    T.copy_(Tg)
+    ctx.xf_max_wavespeed(U, T, S_dev)
+    S = float(S_dev.item())
     dt = w.cfl / S
-    g.T.copy_(Tg)
-    g.step(dt)
-    assert g.ctx.xf_status() == 0
-    Ug = w.interior(g.host_U())
+    # the oracle's input: the (64 + 18)^3 block of U^n and of the T guess around a seeded origin, periodic wrap
     rng = np.random.default_rng(wl.SEED_BASE + 55)
     origin = (int(rng.integers(0, w.nx)), int(rng.integers(0, w.ny)), int(rng.integers(0, w.nz)))
     size, margin = 64, 9
-    w.T_guess = Tg.cpu().numpy()
-    sub = wl.periodic_subblock(w, origin, size, margin)
+    n = size + 2 * margin
+    dev = U.device
+    ix = ((torch.arange(n, device=dev) + origin[0] - margin) % w.nx) + 3
+    iy = ((torch.arange(n, device=dev) + origin[1] - margin) % w.ny) + 3
+    iz = ((torch.arange(n, device=dev) + origin[2] - margin) % w.nz) + 3
+    Ub = U.index_select(1, iz).index_select(2, iy).index_select(3, ix).cpu().numpy()
+    Tb = Tg.index_select(0, iz).index_select(1, iy).index_select(2, ix).cpu().numpy()
+    T.copy_(Tg)
+    ctx.xf_rk3_step(U, T, dt, work)
+    assert ctx.xf_status() == 0
+    sl = slice(margin, margin + size)
+    inner_g = U.index_select(1, iz[sl]).index_select(2, iy[sl]).index_select(3, ix[sl]).cpu().numpy()
+    ctx.close()
+    del U, T, Tg, work
+    torch.cuda.empty_cache()
+    sub = wl.periodic_subblock_arrays(w, Ub, Tb)
     orc = oracle_mod.Oracle.from_workload(sub)
     Uo, To = sub.U.copy(), sub.T_guess.copy()
-    orc.rk3_step(Uo, To, dt)
-    inner_o = sub.interior(Uo)[:, margin:margin + size, margin:margin + size, margin:margin + size]
-    ix = (np.arange(size) + origin[0]) % w.nx
-    iy = (np.arange(size) + origin[1]) % w.ny
-    iz = (np.arange(size) + origin[2]) % w.nz
-    inner_g = Ug[:, iz][:, :, iy][:, :, :, ix]
+    assert orc.rk3_step(Uo, To, dt) == 0
+    inner_o = sub.interior(Uo)[:, sl, sl, sl]
     nv = w.nvars
     num = np.abs(inner_g - inner_o).reshape(nv, -1).max(axis=1)
     den = np.abs(inner_o).reshape(nv, -1).max(axis=1)
     den[1:4] = np.abs(inner_o[0]).max() * S * w.dx
-    assert (num / den).max() < STEPS_TOL
-    g.close()
+    assert (num / den).max() < STEPS_TOL, num / den
 
 
 # ------------------------------------------------------------------------------------------------------------
