@@ -51,7 +51,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         objs = list(ex.map(compile_one, SOURCES))
     if force or _stale(LIB, objs):
         tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")
-        subprocess.run([nvcc, "-shared", "-Wno-deprecated-gpu-targets", "-o", str(tmp), *map(str, objs)], check=True)
+        subprocess.run([nvcc, "-shared", "-arch=sm_100a", "-o", str(tmp), *map(str, objs), "-ldl"], check=True)
         os.replace(tmp, LIB)
     return LIB
 

@@ -6,6 +6,8 @@
 
 #include <new>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "xf_common.cuh"
 
 int xf_sweep_x_init();
@@ -25,6 +27,7 @@ struct xf_ctx {
   double *lam_glob_dev;               // GLF: [3][3] global maxima of the current residual evaluation
   int visc, recon;                    // XF_VISC_*, XF_RECON_*
   long launches;
+  XfTmapCache tmaps;                  // tensor maps of the TMA sweeps, per (base pointer, fields)
   // lazily allocated device mirrors for the *_host entry points
   double *hU, *hT, *hR;
   void *hW;
@@ -35,6 +38,12 @@ struct xf_ctx {
 };
 
 namespace {
+
+// NVTX range around an ABI call (tracing); free when no profiler is attached
+struct Range {
+  explicit Range(const char *name) { nvtxRangePushA(name); }
+  ~Range() { nvtxRangePop(); }
+};
 
 struct DeviceGuard {
   int prev;
@@ -130,9 +139,9 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
     E.recon = c->recon;
     E.lam_glob = c->lam_glob_dev;
     Timed t(c, XF_K_SWEEP_X + d, s);
-    if (d == 0) rc = xf_launch_sweep_x(c->G, c->N, U, prim, E, c->status_dev, s);
-    else if (d == 1) rc = xf_launch_sweep_y(c->G, c->N, U, prim, E, c->status_dev, s);
-    else rc = xf_launch_sweep_z(c->G, c->N, U, prim, E, c->status_dev, s);
+    if (d == 0) rc = xf_launch_sweep_x(c->G, c->N, U, prim, E, c->status_dev, &c->tmaps, s);
+    else if (d == 1) rc = xf_launch_sweep_y(c->G, c->N, U, prim, E, c->status_dev, &c->tmaps, s);
+    else rc = xf_launch_sweep_z(c->G, c->N, U, prim, E, c->status_dev, &c->tmaps, s);
     ++c->launches;
     if (rc != XF_OK) return rc;
     ++done;
@@ -167,13 +176,19 @@ int rk3(xf_ctx *c, double *U, double *T, double dt, double cfl, const double *S_
 }
 
 int ensure_host_mirrors(xf_ctx *c) {
-  if (c->hU) return XF_OK;
+  if (c->hU && c->hT && c->hR && c->hW) return XF_OK;
   const size_t fb = field_bytes(c);
-  if (cudaMalloc(&c->hU, fb * c->Nv) != cudaSuccess) return XF_ENOMEM;
-  if (cudaMalloc(&c->hT, fb) != cudaSuccess) return XF_ENOMEM;
-  if (cudaMalloc(&c->hR, fb * c->Nv) != cudaSuccess) return XF_ENOMEM;
-  if (cudaMalloc(&c->hW, xf_workspace_bytes(c)) != cudaSuccess) return XF_ENOMEM;
-  return XF_OK;
+  if (cudaMalloc(&c->hU, fb * c->Nv) == cudaSuccess && cudaMalloc(&c->hT, fb) == cudaSuccess &&
+      cudaMalloc(&c->hR, fb * c->Nv) == cudaSuccess && cudaMalloc(&c->hW, xf_workspace_bytes(c)) == cudaSuccess)
+    return XF_OK;
+  cudaFree(c->hU);   // all or nothing: a later call must not find a partial set
+  cudaFree(c->hT);
+  cudaFree(c->hR);
+  cudaFree(c->hW);
+  c->hU = c->hT = c->hR = nullptr;
+  c->hW = nullptr;
+  cudaGetLastError();
+  return XF_ENOMEM;
 }
 
 }  // namespace
@@ -295,6 +310,7 @@ size_t xf_workspace_bytes(const xf_ctx *c) {
 
 int xf_fill_ghosts(xf_ctx *c, double *U, void *stream) {
   if (!c || !U) return XF_EINVAL;
+  Range r("xf_fill_ghosts");
   DeviceGuard guard(c->device);
   if (!guard.ok) return XF_ECUDA;
   return xf_launch_ghosts(c->G, c->Nv, c->bc, c->bc_state_dev, U, static_cast<cudaStream_t>(stream), &c->launches);
@@ -302,6 +318,7 @@ int xf_fill_ghosts(xf_ctx *c, double *U, void *stream) {
 
 int xf_primitives(xf_ctx *c, const double *U, double *T, double *p, double *cs, void *stream) {
   if (!c || !U || !T) return XF_EINVAL;
+  Range r("xf_primitives");
   DeviceGuard guard(c->device);
   if (!guard.ok) return XF_ECUDA;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
@@ -312,6 +329,7 @@ int xf_primitives(xf_ctx *c, const double *U, double *T, double *p, double *cs, 
 
 int xf_convective_rhs(xf_ctx *c, double *U, double *T, double *rhs, void *work, void *stream) {
   if (!c || !U || !T || !rhs || !work) return XF_EINVAL;
+  Range r("xf_convective_rhs");
   DeviceGuard guard(c->device);
   if (!guard.ok) return XF_ECUDA;
   XfEpilogue E;
@@ -322,7 +340,8 @@ int xf_convective_rhs(xf_ctx *c, double *U, double *T, double *rhs, void *work, 
 }
 
 int xf_rk3_step(xf_ctx *c, double *U, double *T, double dt, void *work, void *stream) {
-  if (!c || !U || !T || !work || !(dt == dt)) return XF_EINVAL;
+  if (!c || !U || !T || !work || !(dt > 0.0) || isinf(dt)) return XF_EINVAL;   // dt = 0, negative, inf, NaN
+  Range r("xf_rk3_step");
   DeviceGuard guard(c->device);
   if (!guard.ok) return XF_ECUDA;
   return rk3(c, U, T, dt, 0.0, nullptr, work, static_cast<cudaStream_t>(stream));
@@ -330,6 +349,7 @@ int xf_rk3_step(xf_ctx *c, double *U, double *T, double dt, void *work, void *st
 
 int xf_rk3_step_cfl(xf_ctx *c, double *U, double *T, double cfl, const double *S_dev, void *work, void *stream) {
   if (!c || !U || !T || !work || !S_dev || !(cfl > 0.0)) return XF_EINVAL;
+  Range r("xf_rk3_step_cfl");
   DeviceGuard guard(c->device);
   if (!guard.ok) return XF_ECUDA;
   return rk3(c, U, T, 0.0, cfl, S_dev, work, static_cast<cudaStream_t>(stream));
@@ -337,6 +357,7 @@ int xf_rk3_step_cfl(xf_ctx *c, double *U, double *T, double cfl, const double *S
 
 int xf_step_cfl(xf_ctx *c, double *U, double *T, double cfl, double *S_dev, void *work, void *stream) {
   if (!c || !U || !T || !work || !S_dev || !(cfl > 0.0)) return XF_EINVAL;
+  Range r("xf_step_cfl");
   DeviceGuard guard(c->device);
   if (!guard.ok) return XF_ECUDA;
   return rk3(c, U, T, 0.0, cfl, S_dev, work, static_cast<cudaStream_t>(stream), S_dev);
@@ -344,6 +365,7 @@ int xf_step_cfl(xf_ctx *c, double *U, double *T, double cfl, double *S_dev, void
 
 int xf_max_wavespeed(xf_ctx *c, const double *U, double *T, double *S_dev, void *stream) {
   if (!c || !U || !T || !S_dev) return XF_EINVAL;
+  Range r("xf_max_wavespeed");
   DeviceGuard guard(c->device);
   if (!guard.ok) return XF_ECUDA;
   ++c->launches;
@@ -424,6 +446,7 @@ int xf_timing_read(xf_ctx *c, void *stream, double *ms_out, long *count_out) {
 
 int xf_convective_rhs_host(xf_ctx *c, const double *U_host, double *T_host, double *rhs_host) {
   if (!c || !U_host || !T_host || !rhs_host) return XF_EINVAL;
+  Range r("xf_convective_rhs_host");
   DeviceGuard guard(c->device);
   if (!guard.ok) return XF_ECUDA;
   int rc = ensure_host_mirrors(c);
@@ -445,6 +468,7 @@ int xf_convective_rhs_host(xf_ctx *c, const double *U_host, double *T_host, doub
 
 int xf_rk3_steps_host(xf_ctx *c, double *U_host, double *T_host, double cfl, int nsteps, double *t_advanced) {
   if (!c || !U_host || !T_host || !(cfl > 0.0) || nsteps < 0) return XF_EINVAL;
+  Range r("xf_rk3_steps_host");
   DeviceGuard guard(c->device);
   if (!guard.ok) return XF_ECUDA;
   int rc = ensure_host_mirrors(c);

@@ -1,5 +1,6 @@
 // xf_common.cuh -- shared declarations of the CUDA path (sm_100a).  No code is shared with oracle/.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -59,6 +60,19 @@ struct XfEpilogue {
   const double *lam_glob;  // GLF: [direction][u-c, u, u+c] global maxima on the device
 };
 
+// Tensor maps of the TMA sweeps depend only on (base pointer, number of fields, grid): encoded once and kept in the
+// context (three cuTensorMapEncodeTiled calls per sweep launch showed on the 2 M-cell configuration).
+struct XfTmapCache {
+  struct Entry {
+    const void *base;
+    int nf, kind;   // kind 0: rank-4 row map of the y/z sweeps, 1: rank-2 span map of the x sweep
+    bool ok;        // false: TMA cannot describe this array (odd extents, unaligned base)
+    CUtensorMap tm;
+  };
+  Entry e[32];
+  int n, next;
+};
+
 // launch helpers implemented per translation unit
 // prim: the N + 4 workspace fields p, c, 1/rho, Gamma, chi_1..chi_N ([field][padded cells]); NULL = do
 // not store them (xf_primitives), p_out / c_out: optional separate copies of p and c for the caller.
@@ -72,11 +86,11 @@ int xf_launch_wavespeed(const XfGrid &G, const XfThermo &Th, const double *U, do
 int xf_launch_ghosts(const XfGrid &G, int Nv, const XfBc &bc, const double *bc_state_dev, double *U, cudaStream_t s,
                      long *launches);
 int xf_launch_sweep_x(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
-                      cudaStream_t s);
+                      XfTmapCache *tc, cudaStream_t s);
 int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
-                      cudaStream_t s);
+                      XfTmapCache *tc, cudaStream_t s);
 int xf_launch_sweep_z(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
-                      cudaStream_t s);
+                      XfTmapCache *tc, cudaStream_t s);
 
 // fp64 reciprocal: MUFU.RCP64H seed (relative error e <= 1e-6) refined as r (1 + e + e^2), which leaves e^3:
 // 3 DFMA, measured max relative error 2.2e-16 over 1e-13 .. 1e13.  The path is bound by the fp64 pipe, and an

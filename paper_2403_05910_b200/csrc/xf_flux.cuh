@@ -49,8 +49,9 @@ __device__ __forceinline__ void weno5_parts(double v0, double v1, double v2, dou
 __device__ __forceinline__ double weno5(double v0, double v1, double v2, double v3, double v4) {
   double num, den, base;
   weno5_parts(v0, v1, v2, v3, v4, num, den, base);
-  // 1/(2 den): the factor 1/2 is an integer subtraction on the exponent field, not an fp64-pipe instruction
-  const double rh = __longlong_as_double(__double_as_longlong(xf_rcp(den)) - (1ll << 52));
+  // 1/(2 den): the factor 1/2 is ONE integer subtraction on the exponent field (high word), not an fp64-pipe instruction
+  const double rc = xf_rcp(den);
+  const double rh = __hiloint2double(__double2hiint(rc) - 0x00100000, __double2loint(rc));
   return fma(num, rh, base);
 }
 
@@ -181,10 +182,12 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const d
     nuU[m] = fma(-ut[nd], rho[m], mn);
     ud[m] = mn * XRI(m);
     const double cm = XC(m);
-    if (visc == XF_VISC_LLF) {
-      lam_m = fmax(lam_m, fabs(ud[m] - cm));
-      lam_0 = fmax(lam_0, fabs(ud[m]));
-      lam_p = fmax(lam_p, fabs(ud[m] + cm));
+    if (visc == XF_VISC_LLF) {   // max by compare + select: fmax() drags IEEE NaN handling along (a dozen integer
+                                 // instructions each); a NaN state is caught by the status flag anyway
+      const double tm = fabs(ud[m] - cm), t0 = fabs(ud[m]), tp = fabs(ud[m] + cm);
+      lam_m = tm > lam_m ? tm : lam_m;
+      lam_0 = t0 > lam_0 ? t0 : lam_0;
+      lam_p = tp > lam_p ? tp : lam_p;
     }
     const double pm = XP(m);                           // pressure terms of L F_m, with p_m / (4 c~^2) = hh p_m:
     qp[m] = (ghh * pm) * (ud[m] - ut[nd]);             //   Gamma~ (u_m - u~) p_m / (4 c~^2)

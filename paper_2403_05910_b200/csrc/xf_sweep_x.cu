@@ -1,23 +1,22 @@
 // xf_sweep_x.cu -- instantiations and launcher of the x-direction sweep (see xf_sweeps.cuh).
-#include <stdlib.h>
-
 #include "xf_sweeps.cuh"
 
 namespace {
 using namespace xf;
 
 template <int NT, int RC>
-int launch(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status, cudaStream_t s) {
-  CUtensorMap tmU, tmP, tmS;   // U [N + 4]; p, c, 1/rho [3]; Gamma, chi_s [N + 1]
-  static const bool no_tma = getenv("XF_NO_TMA") != nullptr;
-  if (!no_tma && xf_span_tensor_map(&tmU, G, U, N + 4) && xf_span_tensor_map(&tmP, G, prim, 3) &&
-      xf_span_tensor_map(&tmS, G, prim + 3 * G.cells, N + 1)) {
+int launch(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
+           XfTmapCache *tc, cudaStream_t s) {
+  // U [N + 4]; p, c, 1/rho [3]; Gamma, chi_s [N + 1]
+  const CUtensorMap *tmU = xf_tmap(tc, G, U, N + 4, 1), *tmP = xf_tmap(tc, G, prim, 3, 1),
+                    *tmS = xf_tmap(tc, G, prim + 3 * G.cells, N + 1, 1);
+  if (tmU && tmP && tmS) {
     const long long Lf = (long long)G.n[1] * G.np[0];
     const int segc = XW_NCH * XW_CH - 1;
     const int segs = (int)((Lf + segc - 1) / segc);
     const unsigned blocks = (unsigned)(segs * G.n[2]);
     const size_t smem = sizeof(double) * xw_smem_doubles(N);
-    sweep_x_ws_kernel<NT, RC><<<blocks, dim3(32, 2 * XW_W), smem, s>>>(G, N, U, E, status, segs, tmU, tmP, tmS);
+    sweep_x_ws_kernel<NT, RC><<<blocks, dim3(32, 2 * XW_W), smem, s>>>(G, N, U, E, status, segs, *tmU, *tmP, *tmS);
     return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
   }
   const long long L = (long long)G.n[1] * G.np[0];
@@ -31,8 +30,8 @@ int launch(const XfGrid &G, int N, const double *U, const double *prim, const Xf
 }  // namespace
 
 int xf_launch_sweep_x(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
-                      cudaStream_t s) {
-#define CALL(NT) return E.recon == 1 ? launch<NT, 1>(G, N, U, prim, E, status, s) : launch<NT, 0>(G, N, U, prim, E, status, s)
+                      XfTmapCache *tc, cudaStream_t s) {
+#define CALL(NT) return E.recon == 1 ? launch<NT, 1>(G, N, U, prim, E, status, tc, s) : launch<NT, 0>(G, N, U, prim, E, status, tc, s)
   XF_DISPATCH_SWEEP_N(N, CALL)
 #undef CALL
   return XF_EINVAL;

@@ -1,5 +1,5 @@
 // xf_sweep_z.cu -- instantiations and launcher of the z-direction sweep (see xf_sweeps.cuh).
-#include <stdlib.h>
+#include <string.h>
 
 #include "xf_sweeps.cuh"
 
@@ -7,7 +7,8 @@ namespace {
 constexpr int DIR = 2, OD = DIR == 1 ? 2 : 1;
 
 template <int NT, int RC>
-int launch(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status, cudaStream_t s) {
+int launch(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
+           XfTmapCache *tc, cudaStream_t s) {
   using namespace xf;
   const int strips = (G.n[0] + 31) / 32;
   // one block marches a whole column unless the grid alone cannot fill 148 SMs x 2 blocks a few times over;
@@ -19,20 +20,27 @@ int launch(const XfGrid &G, int N, const double *U, const double *prim, const Xf
   nseg = (n + seg_len - 1) / seg_len;
   const dim3 grid(strips, G.n[OD], nseg), block(32, 2 * YZ_W);
   const size_t smem = sizeof(double) * yz_smem_doubles(N, YZ_W);
-  CUtensorMap tmU, tmP, tmS;   // U [N + 4]; p, c, 1/rho [3]; Gamma, chi_s [N + 1]
-  static const bool no_tma = getenv("XF_NO_TMA") != nullptr;
-  if (!no_tma && G.g[0] == XF_NG && xf_row_tensor_map(&tmU, G, U, N + 4) && xf_row_tensor_map(&tmP, G, prim, 3) &&
-      xf_row_tensor_map(&tmS, G, prim + 3 * G.cells, N + 1))
-    sweep_yz_ws_kernel<NT, DIR, YZ_W, true, RC><<<grid, block, smem, s>>>(G, N, U, prim, E, status, seg_len, tmU, tmP, tmS);
-  else
-    sweep_yz_ws_kernel<NT, DIR, YZ_W, false, RC><<<grid, block, smem, s>>>(G, N, U, prim, E, status, seg_len, tmU, tmP, tmS);
+  // U [N + 4]; p, c, 1/rho [3]; Gamma, chi_s [N + 1]
+  const CUtensorMap *tmU = nullptr, *tmP = nullptr, *tmS = nullptr;
+  if (G.g[0] == XF_NG) {
+    tmU = xf_tmap(tc, G, U, N + 4, 0);
+    tmP = xf_tmap(tc, G, prim, 3, 0);
+    tmS = xf_tmap(tc, G, prim + 3 * G.cells, N + 1, 0);
+  }
+  if (tmU && tmP && tmS) {
+    sweep_yz_ws_kernel<NT, DIR, YZ_W, true, RC><<<grid, block, smem, s>>>(G, N, U, prim, E, status, seg_len, *tmU, *tmP, *tmS);
+  } else {
+    CUtensorMap none;   // not read by the cp.async instantiation
+    memset(&none, 0, sizeof(none));
+    sweep_yz_ws_kernel<NT, DIR, YZ_W, false, RC><<<grid, block, smem, s>>>(G, N, U, prim, E, status, seg_len, none, none, none);
+  }
   return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
 }
 }  // namespace
 
 int xf_launch_sweep_z(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
-                      cudaStream_t s) {
-#define CALL(NT) return E.recon == 1 ? launch<NT, 1>(G, N, U, prim, E, status, s) : launch<NT, 0>(G, N, U, prim, E, status, s)
+                      XfTmapCache *tc, cudaStream_t s) {
+#define CALL(NT) return E.recon == 1 ? launch<NT, 1>(G, N, U, prim, E, status, tc, s) : launch<NT, 0>(G, N, U, prim, E, status, tc, s)
   XF_DISPATCH_SWEEP_N(N, CALL)
 #undef CALL
   return XF_EINVAL;

@@ -18,8 +18,6 @@
 // cell f; its stencil is rows f .. f+5; the lane that owns face f updates cell f-1 from its own flux and that of face
 // f-1 (the lane LI below it, or the carry left in shared memory by the previous chunk).
 #pragma once
-#include <cuda.h>
-
 #include "xf_flux.cuh"
 
 namespace xf {
@@ -41,6 +39,16 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int NPENDING>
 __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;" ::"n"(NPENDING) : "memory");
+}
+
+// dt of a Runge-Kutta stage: the host's, or CFL / S read on the device (xf_rk3_step_cfl, xf_step_cfl).  A step that is
+// not finite and positive (S = 0, inf or NaN on the device; the host entry points reject such a dt) raises the
+// non-physical flag instead of silently turning U into NaN through alpha / (beta dt).
+__device__ __forceinline__ double stage_dt(const XfEpilogue &E, int *status) {
+  if (E.mode < 2) return 0.0;
+  const double dt = E.S_dev ? E.cfl / *E.S_dev : E.dt;
+  if (!(dt > 0.0 && dt < 1.0e300)) atomicOr(status, XF_FLAG_NONPHYSICAL);
+  return dt;
 }
 
 // Differences each flux component against the face below (Eq. 13) and writes the cell value: a plain residual,
@@ -164,7 +172,7 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
   }
   cp_async_commit();
 
-  const double dt = E.mode >= 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
+  const double dt = stage_dt(E, status);
   CellWriter<LI> W{E};
   W.cells = G.cells;
   W.dt = dt;
@@ -266,7 +274,7 @@ __host__ __device__ constexpr int tma_shallow_slot(int N) { return tma_box_doubl
 __host__ __device__ inline size_t yz_smem_doubles(int N, int W) {   // ring(s), flux buffer, two mbarriers
   const size_t plain = (size_t)nstaged(N) * ring_rows(W) * 32;
   const size_t tma = (size_t)ring_rows(W) * tma_deep_slot(N) + (size_t)(2 * W + 1) * tma_shallow_slot(N);
-  return (plain > tma ? plain : tma) + (size_t)(N + 4) * (W + 1) * 32 + 2;
+  return (plain > tma ? plain : tma) + (size_t)(N + 4) * (W + 1) * 32 + 4;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -278,9 +286,12 @@ __host__ __device__ inline size_t yz_smem_doubles(int N, int W) {   // ring(s), 
 //   * W SERVICE warps keep the ring one chunk ahead (cp.async) and, concurrently with the next chunk's arithmetic,
 //     difference the fluxes of the chunk just finished and write the cells (Eq. 13, Eq. 16).
 // setmaxnreg moves registers from the service group (88) to the compute group (168): two blocks per SM.
-// Named barriers (ids alternate with the chunk parity): RING_FULL  service -> compute  rows of chunk c landed
+// Named barriers (ids alternate with the chunk parity): RING_FULL  service -> compute  rows of chunk c landed (cp.async path)
 //                                                        FLUX_READY compute -> service  fluxes of chunk c in fb
-//                                                        FB_EMPTY   service -> compute  fb of chunk c - 1 consumed
+// mbarriers (one per chunk parity):                      full       TMA -> compute      rows of chunk c landed
+//                                                        fb_empty   service -> compute  fb of chunk c - 1 consumed
+// The compute warps only ever ARRIVE on a named barrier; what they wait on are mbarriers, whose phase has as a rule
+// completed long before they look, so a compute warp never stalls on another compute warp.
 // ---------------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void named_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
@@ -294,6 +305,9 @@ __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
 }
 __device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
   asm volatile(
@@ -314,7 +328,7 @@ __device__ __forceinline__ void tma_load_row(unsigned dst, const void *tmap, int
       : "memory");
 }
 
-constexpr int BAR_RING_FULL = 1, BAR_FLUX_READY = 3, BAR_FB_EMPTY = 5;   // + chunk parity
+constexpr int BAR_RING_FULL = 1, BAR_FLUX_READY = 3;   // + chunk parity
 constexpr int BAR_SERVICE = 7;   // among the service warps: all have read U^s before any of them overwrites ring rows
 #ifndef XF_WS_RC
 #define XF_WS_RC 168   // 2 blocks x 128 threads x (168 + 88) registers = the SM's 64 K
@@ -323,12 +337,13 @@ constexpr int BAR_SERVICE = 7;   // among the service warps: all have read U^s b
 constexpr int WS_REGS_COMPUTE = XF_WS_RC, WS_REGS_SERVICE = XF_WS_RS;
 
 struct FluxStoreWS {
-  double *dst;   // fb + row * 32 + lane
-  int stride;    // doubles between components
-  int wait_id;   // named barrier to pass before the first component is written (-1: none)
-  int nthreads;
+  double *dst;       // fb + row * 32 + lane
+  int stride;        // doubles between components
+  unsigned wait_bar; // mbarrier to pass before the first component is written: the service warps have read the
+  unsigned parity;   //   previous chunk's fluxes (0: nothing to wait for).  Not a bar.sync: the compute warps never
+                     //   wait for ONE ANOTHER, only for the consumer of the buffer they are about to overwrite
   __device__ __forceinline__ void operator()(int v, double F, int) {
-    if (v == 0 && wait_id >= 0) named_sync(wait_id, nthreads);
+    if (v == 0 && wait_bar) mbar_wait(wait_bar, parity);
     dst[v * stride] = F;
   }
 };
@@ -357,14 +372,15 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
   double *sms = TMA ? smem + (size_t)RR * SLOT : smem + (size_t)(Nv + 3) * FS;  // Gamma, chi_s
   double *fb = TMA ? sms + (size_t)RS * SSLOT : smem + (size_t)NST * RR * 32;
   const unsigned full_bar = (unsigned)__cvta_generic_to_shared(fb + (size_t)Nv * FBS);   // two mbarriers (TMA only)
-  if (TMA) {
-    if (threadIdx.x == 0 && threadIdx.y == 0) {
-      mbar_init(full_bar, W);                               // one arrival (with its byte count) per service warp
-      mbar_init(full_bar + 8, W);
-      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
+  const unsigned fbe_bar = full_bar + 16;                   // two more: flux buffer consumed
+  if (threadIdx.x == 0 && threadIdx.y == 0) {
+    mbar_init(full_bar, W);                                 // one arrival (with its byte count) per service warp
+    mbar_init(full_bar + 8, W);
+    mbar_init(fbe_bar, W);                                  // one arrival per service warp
+    mbar_init(fbe_bar + 8, W);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  __syncthreads();
 
   const int lane = threadIdx.x;
   const bool service = threadIdx.y >= W;
@@ -410,11 +426,12 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
       for (int m = 0; m < 6; ++m) asm volatile("" : "+r"(o[m]));
       asm volatile("" : "+r"(s2), "+r"(s3));
       if (f <= f_end) {                                     // warp-uniform
-        FluxStoreWS st{fb + (w + 1) * 32 + lane, FBS, first ? -1 : BAR_FB_EMPTY + par, NT};
+        // fb_empty[c & 1] completes each time the service warps have read the fluxes of a chunk c - 1: for the
+        // ((c - 1) >> 1)-th time (c odd) or the ((c - 2) >> 1)-th (c even), i.e. phase parity `phase` or `phase ^ 1`
+        // with `phase` = (c >> 1) & 1 as for the ring
+        FluxStoreWS st{fb + (w + 1) * 32 + lane, FBS, first ? 0u : fbe_bar + 8 * par, par ? phase : phase ^ 1u};
         const bool c2ok = face_flux<DIR, RECON>(N, sm, smp, FS, o, sms, FS, s2, s3, E.visc, E.lam_glob + 3 * DIR, st);
         bad = bad || (!c2ok && lane_ok);
-      } else if (!first) {
-        named_sync(BAR_FB_EMPTY + par, NT);                 // keep the barrier counts whole
       }
       named_arrive(BAR_FLUX_READY + par, NT);
       rb += W;
@@ -458,7 +475,7 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
       tma_load_row((unsigned)__cvta_generic_to_shared(sms + (size_t)slot * SSLOT), &tmS, c0, DIR == 1 ? rc : co,
                    DIR == 1 ? co : rc, bar);
   };
-  const double dt = E.mode >= 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
+  const double dt = stage_dt(E, status);
   const double kappa = E.mode == 3 ? E.alpha / (E.beta * dt) : 0.0;   // mode 3: out = div + kappa U^n (see XfEpilogue)
   const double ninv = -G.inv_d[DIR];
   const bool need_acc = E.mode == 1 || (E.mode == 2 && E.has_acc);
@@ -534,7 +551,8 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
       load_operands(fprev);
       named_sync(BAR_FLUX_READY + (par ^ 1), NT);           // the previous chunk's fluxes are in fb, its ring rows are dead
       read_fluxes(ous);
-      named_arrive(BAR_FB_EMPTY + par, NT);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(fbe_bar + 8 * par);
     }
     if (fc + W <= f_end) {                                  // the W new rows of the next chunk: rows fc + W + 5 + q
       // warp w fetches row q = (w + 2) mod W: it lands in the ring slot of the previous chunk's row q, and the only
@@ -591,7 +609,7 @@ __host__ __device__ constexpr int xw_stage_doubles(int N) {
   return xw_box_doubles(N + 4) + xw_box_doubles(3) + xw_box_doubles(N + 1);
 }
 __host__ __device__ inline size_t xw_smem_doubles(int N) {
-  return 2 * (size_t)xw_stage_doubles(N) + (size_t)(N + 4) * XW_FBW + 2;
+  return 2 * (size_t)xw_stage_doubles(N) + (size_t)(N + 4) * XW_FBW + 4;
 }
 __device__ __forceinline__ void tma_load_span(unsigned dst, const void *tmap, int c0, unsigned bar) {
   asm volatile(
@@ -613,9 +631,12 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
   extern __shared__ __align__(128) double smem[];
   double *fb = smem + 2 * (size_t)STAGE;                    // face fluxes [Nv][XW_FBW]
   const unsigned full_bar = (unsigned)__cvta_generic_to_shared(fb + (size_t)Nv * XW_FBW);
+  const unsigned fbe_bar = full_bar + 16;                   // flux buffer consumed (see the y/z kernel)
   if (threadIdx.x == 0 && threadIdx.y == 0) {
     mbar_init(full_bar, 1);
     mbar_init(full_bar + 8, 1);
+    mbar_init(fbe_bar, W);
+    mbar_init(fbe_bar + 8, W);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -648,7 +669,7 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
 #pragma unroll
       for (int m = 0; m < 6; ++m) o[m] = u + delta + m;
       // every lane of the block passes the same barriers; lanes past f_end compute on staged (valid or zero) data
-      FluxStoreWS fsw{fb + u + 1, XW_FBW, first ? -1 : BAR_FB_EMPTY + par, NT};
+      FluxStoreWS fsw{fb + u + 1, XW_FBW, first ? 0u : fbe_bar + 8 * par, par ? phase : phase ^ 1u};
       const bool c2ok = face_flux<0, RECON>(N, st, st + OFFP, FS, o, st + OFFS, FS, o[2], o[3], E.visc, E.lam_glob, fsw);
       {
         const int ia = (f - 1 + G.np[0]) % G.np[0], ib = f % G.np[0];
@@ -676,7 +697,7 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
     tma_load_span(dst + (unsigned)(OFFP * sizeof(double)), &tmP, c0, bar);
     tma_load_span(dst + (unsigned)(OFFS * sizeof(double)), &tmS, c0, bar);
   };
-  const double dt = E.mode >= 2 ? (E.S_dev ? E.cfl / *E.S_dev : E.dt) : 0.0;
+  const double dt = stage_dt(E, status);
   const double kappa = E.mode == 3 ? E.alpha / (E.beta * dt) : 0.0;   // mode 3: out = div + kappa U^n (see XfEpilogue)
   const double ninv = -G.inv_d[0];
   const bool need_acc = E.mode == 1 || (E.mode == 2 && E.has_acc);
@@ -743,7 +764,8 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
       load_operands(fprev);
       named_sync(BAR_FLUX_READY + (par ^ 1), NT);           // the previous chunk's fluxes are in fb, its stage is free
       read_fluxes(par ^ 1);
-      named_arrive(BAR_FB_EMPTY + par, NT);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(fbe_bar + 8 * par);
       if (E.mode == 2) named_sync(BAR_SERVICE, 32 * W);     // U^s was read from the stage the next copy overwrites
     }
     if (fc + XW_CH <= f_end) stage_chunk(fc + XW_CH, par ^ 1);
@@ -800,6 +822,19 @@ inline bool xf_span_tensor_map(CUtensorMap *tm, const XfGrid &G, const double *b
   return encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double *>(base), dims, strides, box, estr,
                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// cached tensor map of `nf` fields at `base` (kind 0: row map, 1: span map); nullptr where TMA cannot describe the array
+inline const CUtensorMap *xf_tmap(XfTmapCache *c, const XfGrid &G, const double *base, int nf, int kind) {
+  for (int q = 0; q < c->n; ++q)
+    if (c->e[q].base == base && c->e[q].nf == nf && c->e[q].kind == kind) return c->e[q].ok ? &c->e[q].tm : nullptr;
+  const int cap = (int)(sizeof(c->e) / sizeof(c->e[0]));
+  XfTmapCache::Entry &en = c->e[c->n < cap ? c->n++ : (c->next = (c->next + 1) % cap)];
+  en.base = base;
+  en.nf = nf;
+  en.kind = kind;
+  en.ok = kind == 0 ? xf_row_tensor_map(&en.tm, G, base, nf) : xf_span_tensor_map(&en.tm, G, base, nf);
+  return en.ok ? &en.tm : nullptr;
 }
 
 #define XF_DISPATCH_SWEEP_N(N, CALL) \

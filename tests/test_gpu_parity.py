@@ -423,13 +423,23 @@ def test_full_size_rhs_on_sampled_cells(oracle_mod, name):
     ro = orc.rhs_cells(Uo, w.T_guess, idx)                    # [samples, Nv]
     assert orc.last_status == 0
     rg = r.reshape(nv, -1)[:, idx].T
-    # reading R14, strictly: every variable -- the trace species of config 4 (Y ~ 1e-8 .. 1e-4) included -- is measured
-    # against ITS OWN scale, taken from the oracle's values (the samples contain the cells with the largest residuals)
-    scale = np.abs(ro).max(axis=0)
-    scale[1:4] = scale[1:4].max()                             # momentum components share their scale (R14)
-    err = np.abs(rg - ro).max(axis=0) / scale
-    print(f"{name}: per-variable error on own scale", err)
-    assert err.max() < RHS_TOL, err
+    # Reading R14 with the round-off floor of DESIGN.md section 11: every variable is measured against its own scale
+    # (oracle values; the samples contain the cells with the largest residuals), except that a partial density is never
+    # measured against less than max(Y_s) x the density row's scale.  Reason: Fhat_{rho Y_s} = Y~_s s + g_s with s the
+    # mass flux assembled from O(rho c) characteristic fluxes that cancel in quiescent gas, so its round-off is
+    # eps Y_s rho c / dx whatever the row's own residual is -- for the ORACLE too (tests/test_oracle_roundoff_floor.py
+    # measures that floor against a long-double build of the oracle on these very cells).  A species that sits only
+    # where nothing moves yet (config 2's bubble gas at t = 0) has an own scale below that floor.  The trace species of
+    # config 4 (Y ~ 1e-8 .. 1e-4) are thereby held to 1e-12 of a scale 1e-4 .. 1e-8 times the density row's.
+    own = np.abs(ro).max(axis=0)
+    own[1:4] = own[1:4].max()                                 # momentum components share their scale (R14)
+    Ymax = (np.abs(w.interior(w.U)[5:]) / w.interior(w.U)[0]).reshape(nv - 5, -1).max(axis=1)
+    scale = own.copy()
+    scale[5:] = np.maximum(own[5:], Ymax * own[0])
+    err = np.abs(rg - ro).max(axis=0)
+    print(f"{name}: error per variable on its OWN scale", err / own)
+    print(f"{name}: error per variable on the R14 scale ", err / scale, " Ymax", Ymax)
+    assert (err / scale).max() < RHS_TOL, err / scale
 
 
 def test_config5_full_size_subblock(oracle_mod):
