@@ -24,7 +24,7 @@ class OConfig(C.Structure):
         ("Tlo", C.c_double), ("Thi", C.c_double),
         ("bc", C.c_int * 6), ("bc_state", (C.c_double * MAXNV) * 6),
         ("rtol", C.c_double), ("maxit", C.c_int), ("ideal_weights", C.c_int), ("viscosity", C.c_int),
-        ("lam_glob", (C.c_double * 3) * 3), ("recon", C.c_int),
+        ("lam_glob", (C.c_double * 3) * 3), ("recon", C.c_int), ("positivity", C.c_int), ("pp_dt", C.c_double),
     ]
 
 
@@ -78,6 +78,11 @@ def lib():
         L.xo_weno5.restype = C.c_double
         L.xo_wenocu6.argtypes = [dp, C.c_int, dp, dp]
         L.xo_wenocu6.restype = C.c_double
+        L.xo_weno7.argtypes = [dp, C.c_int, dp, dp]
+        L.xo_weno7.restype = C.c_double
+        L.xo_stencil_cells.argtypes = [cp]
+        L.xo_positivity_blend.argtypes = [cp, C.c_int, dp, pp, dp, pp, C.c_double, dp]
+        L.xo_positivity_blend.restype = C.c_double
         L.xo_face_flux.argtypes = [cp, C.c_int, dp, pp, dp]
         L.xo_fill_ghosts.argtypes = [cp, dp]
         L.xo_fill_ghosts.restype = None
@@ -105,6 +110,15 @@ def wenocu6(v, ideal: bool = False):
     return val, beta, w
 
 
+def weno7(v, ideal: bool = False):
+    """-> (value at +1/2, [beta0..beta3], [four normalised weights]); v = v_{-3}..v_{+3}"""
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    assert v.shape == (7,)
+    beta, w = np.zeros(4), np.zeros(4)
+    val = float(lib().xo_weno7(_dp(v), int(ideal), _dp(beta), _dp(w)))
+    return val, beta, w
+
+
 def weno5(v, ideal: bool = False) -> float:
     v = np.ascontiguousarray(v, dtype=np.float64)
     assert v.shape == (5,)
@@ -115,13 +129,16 @@ class Oracle:
     """One oracle context: grid, species table and boundary data (mirrors xf_config of include/xf.h)."""
 
     def __init__(self, nx, ny, nz, dx, dy, dz, W, nasa7, Ru, Tlo, Thi, bc=(0,) * 6, bc_state=None,
-                 rtol: float = 1e-13, maxit: int = 50, ideal_weights: bool = False, viscosity: int = 0, recon: int = 0):
+                 rtol: float = 1e-13, maxit: int = 50, ideal_weights: bool = False, viscosity: int = 0, recon: int = 0,
+                 positivity: bool = False, pp_dt: float = 0.0, ng: Optional[int] = None):
         W = np.asarray(W, dtype=np.float64)
         nasa7 = np.asarray(nasa7, dtype=np.float64)
         n = W.shape[0]
         assert 1 <= n <= MAXN and nasa7.shape == (n, 7)
         cfg = OConfig()
-        cfg.nx, cfg.ny, cfg.nz, cfg.ng = int(nx), int(ny), int(nz), 3
+        ng = (4 if recon == 2 else 3) if ng is None else int(ng)
+        assert ng >= (4 if recon == 2 else 3)
+        cfg.nx, cfg.ny, cfg.nz, cfg.ng = int(nx), int(ny), int(nz), ng
         cfg.dx, cfg.dy, cfg.dz = float(dx), float(dy), float(dz)
         cfg.N, cfg.Ru = n, float(Ru)
         for s in range(n):
@@ -138,16 +155,19 @@ class Oracle:
                     cfg.bc_state[q][v] = bs[q, v]
         cfg.rtol, cfg.maxit, cfg.ideal_weights = float(rtol), int(maxit), int(ideal_weights)
         cfg.viscosity = int(viscosity)   # 0 LLF, 1 ROE, 2 GLF (xf_oracle.h)
-        cfg.recon = int(recon)           # 0 WENO5-JS, 1 WENO-CU6
+        cfg.recon = int(recon)           # 0 WENO5-JS, 1 WENO-CU6, 2 WENO7
+        cfg.positivity, cfg.pp_dt = int(positivity), float(pp_dt)
         self.cfg = cfg
+        self.ng = ng
         self.N = n
         self.Nv = n + 4
         self.cells = int(lib().xo_padded_cells(C.byref(cfg)))
-        self.shape = (nz + 6 if nz > 1 else 1, ny + 6 if ny > 1 else 1, nx + 6 if nx > 1 else 1)
+        self.shape = (nz + 2 * ng if nz > 1 else 1, ny + 2 * ng if ny > 1 else 1, nx + 2 * ng if nx > 1 else 1)
 
     @classmethod
     def from_workload(cls, wl, **kw) -> "Oracle":
         t = wl.table
+        kw.setdefault("ng", getattr(wl, "ng", 3))
         return cls(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, t.W, t.nasa7, t.Ru, t.Tlo, t.Thi, wl.bc, wl.bc_state, **kw)
 
     # ---- per-cell pieces (for the pins) ----
@@ -181,11 +201,21 @@ class Oracle:
         st = lib().xo_eigensystem(C.byref(self.cfg), C.byref(PA), C.byref(PB), d, _dp(L), _dp(R), _dp(roe))
         return L, R, roe, st
 
+    def positivity_blend(self, d: int, Ua, Pa: OPrim, Ub, Pb: OPrim, kappa: float, Fhat):
+        """-> (theta, blended flux); Fhat is not modified"""
+        Ua = np.ascontiguousarray(Ua, dtype=np.float64)
+        Ub = np.ascontiguousarray(Ub, dtype=np.float64)
+        F = np.array(Fhat, dtype=np.float64)
+        th = lib().xo_positivity_blend(C.byref(self.cfg), d, _dp(Ua), C.byref(Pa), _dp(Ub), C.byref(Pb), float(kappa), _dp(F))
+        return float(th), F
+
     def face_flux(self, d: int, Ust, Tguess) -> np.ndarray:
-        """Ust[6][Nv]: the six stencil cells; primitives by Newton from Tguess[6]."""
+        """Ust[S][Nv]: the S = 6 (8 for WENO7) stencil cells; primitives by Newton from Tguess[S]."""
         Ust = np.ascontiguousarray(Ust, dtype=np.float64)
-        prims = (OPrim * 6)()
-        for m in range(6):
+        S = int(lib().xo_stencil_cells(C.byref(self.cfg)))
+        assert Ust.shape[0] == S
+        prims = (OPrim * S)()
+        for m in range(S):
             lib().xo_cell_primitives(C.byref(self.cfg), _dp(Ust[m]), float(Tguess[m]), C.byref(prims[m]))
         F = np.zeros(self.Nv)
         lib().xo_face_flux(C.byref(self.cfg), d, _dp(Ust), prims, _dp(F))

@@ -318,16 +318,56 @@ double xo_wenocu6(const double v[6], int ideal_weights, double *beta_out, double
 }
 
 /* ------------------------------------------------------------------------------------------------------------ */
+/* C6''. WENO7 (PAPER.md:107 names it, ref 36, and prints no formula: reading R18).  Seven-point stencil v_{-3}..v_{+3}; */
+/* four cubic candidates on cells (k-3..k), k = 0..3; linear weights 1/35, 12/35, 18/35, 4/35 (together the 7-point     */
+/* interpolation (-3, 25, -101, 319, 214, -38, 4)/420); beta_k = sum_{l=1..3} dx^(2l-1) int (d^l p_k/dx^l)^2 dx of the   */
+/* candidate polynomial over cell i -- the Jiang-Shu measure; its quadratic form in the three FIRST DIFFERENCES of the   */
+/* sub-stencil, times 240, is derived exactly in tests/golden/make_golden.py (weno7_coefficients.txt);                   */
+/* alpha_k = d_k/(eps + beta_k)^2 with eps = 1e-6 and exponent 2 as for WENO5 (reading R7).                             */
+/* ------------------------------------------------------------------------------------------------------------ */
+double xo_weno7(const double v[7], int ideal_weights, double *beta_out, double *w_out) {
+  static const double d[4] = {1.0 / 35.0, 12.0 / 35.0, 18.0 / 35.0, 4.0 / 35.0};
+  static const double C[4][4] = {{-3.0, 13.0, -23.0, 25.0}, {1.0, -5.0, 13.0, 3.0}, {-1.0, 7.0, 7.0, -1.0}, {3.0, 13.0, -5.0, 1.0}};
+  /* 240 beta_k = G[k][0] D0^2 + G[k][1] D0 D1 + G[k][2] D0 D2 + G[k][3] D1^2 + G[k][4] D1 D2 + G[k][5] D2^2,
+   * D_m = v_{k+m+1} - v_{k+m} the first differences of sub-stencil k */
+  static const double G[4][6] = {{547.0, -2788.0, 1854.0, 3708.0, -5188.0, 2107.0},
+                                 {267.0, -1108.0, 494.0, 1468.0, -1428.0, 547.0},
+                                 {547.0, -1428.0, 494.0, 1468.0, -1108.0, 267.0},
+                                 {2107.0, -5188.0, 1854.0, 3708.0, -2788.0, 547.0}};
+  double q[4], a[4], beta[4];
+  for (int k = 0; k < 4; ++k) {
+    q[k] = (C[k][0] * v[k] + C[k][1] * v[k + 1] + C[k][2] * v[k + 2] + C[k][3] * v[k + 3]) / 12.0;
+    const double D0 = v[k + 1] - v[k], D1 = v[k + 2] - v[k + 1], D2 = v[k + 3] - v[k + 2];
+    beta[k] = (G[k][0] * D0 * D0 + G[k][1] * D0 * D1 + G[k][2] * D0 * D2 + G[k][3] * D1 * D1 + G[k][4] * D1 * D2 +
+               G[k][5] * D2 * D2) / 240.0;
+  }
+  if (ideal_weights) {
+    for (int k = 0; k < 4; ++k) a[k] = d[k];
+  } else {
+    const double eps = 1e-6;
+    for (int k = 0; k < 4; ++k) a[k] = d[k] / ((eps + beta[k]) * (eps + beta[k]));
+  }
+  const double sum = a[0] + a[1] + a[2] + a[3];
+  if (beta_out) for (int k = 0; k < 4; ++k) beta_out[k] = beta[k];
+  if (w_out) for (int k = 0; k < 4; ++k) w_out[k] = a[k] / sum;
+  return (a[0] * q[0] + a[1] * q[1] + a[2] * q[2] + a[3] * q[3]) / sum;
+}
+
+int xo_stencil_cells(const xo_config *c) { return c->recon == XO_RECON_WENO7 ? 8 : 6; }
+
+/* ------------------------------------------------------------------------------------------------------------ */
 /* C5 + C6 + C7. Numerical flux at one face (Eq. 14-15; LLF: PAPER.md:374, reading R8)        */
-/* Ust[m][v], Pst[m], m = 0..5 <-> cells i-2..i+3; the face lies between m = 2 and m = 3.                       */
+/* Ust[m][v], Pst[m], m = 0..S-1 <-> cells i-S/2+1..i+S/2 (S = 6: i-2..i+3; WENO7, S = 8: i-3..i+4); the face lies      */
+/* between m = S/2-1 and m = S/2.                                                                                */
 /* ------------------------------------------------------------------------------------------------------------ */
 int xo_face_flux(const xo_config *c, int d, const double *Ust, const xo_prim *Pst, double *Fhat) {
   const int Nv = c->N + 4;
+  const int S = xo_stencil_cells(c), ma = S / 2 - 1;
   double L[XO_MAXNV * XO_MAXNV], R[XO_MAXNV * XO_MAXNV], roe[6];
-  int status = xo_eigensystem(c, &Pst[2], &Pst[3], d, L, R, roe);
+  int status = xo_eigensystem(c, &Pst[ma], &Pst[ma + 1], d, L, R, roe);
 
-  double aF[6][XO_MAXNV], aU[6][XO_MAXNV], lam[6][3];
-  for (int m = 0; m < 6; ++m) {
+  double aF[8][XO_MAXNV], aU[8][XO_MAXNV], lam[8][3];
+  for (int m = 0; m < S; ++m) {
     double F[XO_MAXNV];
     xo_phys_flux(c, Ust + m * Nv, &Pst[m], d, F);
     for (int n = 0; n < Nv; ++n) {          /* alpha^F_m = L F_m, alpha^U_m = L U_m (face-frozen L) */
@@ -351,15 +391,19 @@ int xo_face_flux(const xo_config *c, int d, const double *Ust, const xo_prim *Ps
       Lam = fabs(roe[d] + (kind - 1) * roe[5]);
     } else if (c->viscosity == XO_VISC_GLF) {
       Lam = c->lam_glob[d][kind];            /* global maximum, set by the caller */
-    } else {                                 /* LLF: max over the 6 stencil cells, factor 1 */
-      for (int m = 0; m < 6; ++m) Lam = fmax(Lam, fabs(lam[m][kind]));
+    } else {                                 /* LLF: max over the S stencil cells, factor 1 */
+      for (int m = 0; m < S; ++m) Lam = fmax(Lam, fabs(lam[m][kind]));
     }
-    double fp[6], fm[6];
-    for (int m = 0; m < 6; ++m) {            /* Eq. 14 */
+    double fp[8], fm[8];
+    for (int m = 0; m < S; ++m) {            /* Eq. 14 */
       fp[m] = 0.5 * (aF[m][n] + Lam * aU[m][n]);
       fm[m] = 0.5 * (aF[m][n] - Lam * aU[m][n]);
     }
-    if (c->recon == XO_RECON_WENOCU6) {      /* six points: i-2..i+3 for f+, mirrored for f- */
+    if (c->recon == XO_RECON_WENO7) {        /* seven points each: i-3..i+3 for f+, i+4..i-2 for f- */
+      const double vp[7] = {fp[0], fp[1], fp[2], fp[3], fp[4], fp[5], fp[6]};
+      const double vm[7] = {fm[7], fm[6], fm[5], fm[4], fm[3], fm[2], fm[1]};
+      g[n] = xo_weno7(vp, c->ideal_weights, NULL, NULL) + xo_weno7(vm, c->ideal_weights, NULL, NULL);
+    } else if (c->recon == XO_RECON_WENOCU6) {      /* six points: i-2..i+3 for f+, mirrored for f- */
       const double vp[6] = {fp[0], fp[1], fp[2], fp[3], fp[4], fp[5]};
       const double vm[6] = {fm[5], fm[4], fm[3], fm[2], fm[1], fm[0]};
       g[n] = xo_wenocu6(vp, c->ideal_weights, NULL, NULL) + xo_wenocu6(vm, c->ideal_weights, NULL, NULL);
@@ -375,6 +419,50 @@ int xo_face_flux(const xo_config *c, int d, const double *Ust, const xo_prim *Ps
     Fhat[j] = s;
   }
   return status;
+}
+
+/* ------------------------------------------------------------------------------------------------------------ */
+/* Positivity-preserving flux blending (Eq. 17-20).  The paper gives the convex splitting      */
+/* U^{n+1}_i = (U^-_i + U^+_i)/2, U^+- = U_i -+ 2 lambda Fhat_{i+-1/2} (Eq. 18), the first-order Lax-Friedrichs  */
+/* flux (Eq. 19) and the blend F* = (1 - theta) F^LF + theta Fhat (Eq. 20), and defers theta to its ref 41.     */
+/* Reading R17: the guarded quantities are q in {rho, rho Y_1, ..., rho Y_N} ("extended to both the  */
+/* density and mass fractions"), rho Y_N = rho - sum_{s<N} rho Y_s; all are linear in U, so q(F)   */
+/* is the same functional of a flux.  For the face between cells a = i and b = i+1, with kappa = 2 D dt/dx_d     */
+/* (each of the D active directions carries the weight 1/D of the splitting):                                   */
+/*   q^+  = q(U_a) - kappa q(Fhat),  q^+LF = q(U_a) - kappa q(F^LF)     (cell a, its upper face)                 */
+/*   q^-  = q(U_b) + kappa q(Fhat),  q^-LF = q(U_b) + kappa q(F^LF)     (cell b, its lower face)                 */
+/*   eps  = min(1e-13, q^LF);  theta^+- = 1 if q^+- >= eps, else (q^LF - eps)/(q^LF - q^+-)                       */
+/*   theta = min over q and over the two sides -- ONE factor for the whole flux vector (Eq. 20).                 */
+/* Lambda~ of Eq. 19 = max(|u_d| + c) of the two cells.  Whenever the LF states are non-negative (they are for  */
+/* kappa Lambda~ <= 1, i.e. D dt Lambda~/dx_d <= 1/2: "CFL <= 0.5"), the blended states satisfy   */
+/* q^+-* >= eps >= 0, and the updated cell value, their average over directions and sides, is non-negative.     */
+/* ------------------------------------------------------------------------------------------------------------ */
+double xo_positivity_blend(const xo_config *c, int d, const double *Ua, const xo_prim *Pa, const double *Ub,
+                           const xo_prim *Pb, double kappa, double *Fhat) {
+  const int N = c->N, Nv = N + 4;
+  double Fa[XO_MAXNV], Fb[XO_MAXNV], FLF[XO_MAXNV];
+  xo_phys_flux(c, Ua, Pa, d, Fa);
+  xo_phys_flux(c, Ub, Pb, d, Fb);
+  const double Lam = fmax(fabs(Pa->vel[d]) + Pa->c, fabs(Pb->vel[d]) + Pb->c);
+  for (int v = 0; v < Nv; ++v) FLF[v] = 0.5 * (Fa[v] + Fb[v] + Lam * (Ua[v] - Ub[v]));   /* Eq. 19 */
+  double theta = 1.0;
+  for (int k = 0; k <= N; ++k) {             /* k = 0: rho; k = 1..N-1: rho Y_k; k = N: rho Y_N by closure */
+    double qa, qb, qF, qL;
+    if (k == 0) { qa = Ua[0]; qb = Ub[0]; qF = Fhat[0]; qL = FLF[0]; }
+    else if (k < N) { qa = Ua[4 + k]; qb = Ub[4 + k]; qF = Fhat[4 + k]; qL = FLF[4 + k]; }
+    else {
+      qa = Ua[0]; qb = Ub[0]; qF = Fhat[0]; qL = FLF[0];
+      for (int s = 1; s < N; ++s) { qa -= Ua[4 + s]; qb -= Ub[4 + s]; qF -= Fhat[4 + s]; qL -= FLF[4 + s]; }
+    }
+    const double qp = qa - kappa * qF, qpL = qa - kappa * qL;     /* Eq. 18: U^+ of cell a */
+    const double qm = qb + kappa * qF, qmL = qb + kappa * qL;     /*         U^- of cell b */
+    const double epsp = fmin(1e-13, qpL), epsm = fmin(1e-13, qmL);
+    if (qp < epsp) theta = fmin(theta, (qpL - epsp) / (qpL - qp));
+    if (qm < epsm) theta = fmin(theta, (qmL - epsm) / (qmL - qm));
+  }
+  if (theta < 1.0)
+    for (int v = 0; v < Nv; ++v) Fhat[v] = (1.0 - theta) * FLF[v] + theta * Fhat[v];     /* Eq. 20 */
+  return theta;
 }
 
 /* ------------------------------------------------------------------------------------------------------------ */
@@ -470,6 +558,9 @@ int xo_rhs_nofill(const xo_config *c_in, const double *U, double *T, double *rhs
   if (c->viscosity == XO_VISC_GLF) global_wavespeeds(c, U, T, cc.lam_glob);
   memset(rhs, 0, sizeof(double) * Nv * cells);
   const double dxs[3] = {c->dx, c->dy, c->dz};
+  const int ma = xo_stencil_cells(c) / 2 - 1;                /* stencil cell index of the cell below the face */
+  const int D = (n[0] > 1) + (n[1] > 1) + (n[2] > 1);
+  const double kappa[3] = {2.0 * D * c->pp_dt / c->dx, 2.0 * D * c->pp_dt / c->dy, 2.0 * D * c->pp_dt / c->dz};
   for (int d = 0; d < 3; ++d) {
     if (n[d] == 1) continue;
     const int a1 = (d + 1) % 3, a2 = (d + 2) % 3;
@@ -488,7 +579,9 @@ int xo_rhs_nofill(const xo_config *c_in, const double *U, double *T, double *rhs
         /* faces i = g-1 .. g+n-1 (face i+1/2 between cells i and i+1): n+1 faces */
         for (int f = 0; f <= n[d]; ++f) {
           const int i = g[d] - 1 + f;
-          status |= xo_face_flux(c, d, Ust + (i - 2) * Nv, Pst + (i - 2), Fh + f * Nv);
+          status |= xo_face_flux(c, d, Ust + (i - ma) * Nv, Pst + (i - ma), Fh + f * Nv);
+          if (c->positivity)                 /* Eq. 20: "the blended flux is used to update Eq. (13)" */
+            xo_positivity_blend(c, d, Ust + i * Nv, Pst + i, Ust + (i + 1) * Nv, Pst + (i + 1), kappa[d], Fh + f * Nv);
         }
         for (int f = 0; f < n[d]; ++f) {
           const long idx = base + (long)(g[d] + f) * st[d];
@@ -507,8 +600,8 @@ int xo_rhs(const xo_config *c, double *U, double *T, double *rhs) {
 }
 
 /* rhs at a list of sampled interior cells, each computed on its own from U (ghosts filled) and the T guess:
- * primitives by Newton for the 7-cell cross of every direction, two faces per direction.  Used for parity at
- * sizes where the whole-field oracle would take too long. rhs_out[q][v]. */
+ * primitives by Newton for the (S+1)-cell cross of every direction (S = 6 or 8 stencil cells), two faces per direction.
+ * Used for parity at sizes where the whole-field oracle would take too long. rhs_out[q][v]. */
 int xo_rhs_cells(const xo_config *c_in, const double *U, const double *Tguess, long ncells, const long *idx,
                  double *rhs_out) {
   xo_config cc = *c_in;
@@ -520,6 +613,8 @@ int xo_rhs_cells(const xo_config *c_in, const double *U, const double *Tguess, l
   grid(c, np, n, g, st);
   const long cells = xo_padded_cells(c);
   const double dxs[3] = {c->dx, c->dy, c->dz};
+  const int S = xo_stencil_cells(c), h = S / 2;              /* cells i-h .. i+h */
+  const int D = (n[0] > 1) + (n[1] > 1) + (n[2] > 1);
   int status = 0;
 #pragma omp parallel for reduction(| : status) schedule(dynamic, 8) if (ncells > 64)
   for (long q = 0; q < ncells; ++q) {
@@ -527,17 +622,22 @@ int xo_rhs_cells(const xo_config *c_in, const double *U, const double *Tguess, l
     for (int v = 0; v < Nv; ++v) acc[v] = 0.0;
     for (int d = 0; d < 3; ++d) {
       if (n[d] == 1) continue;
-      double Ust[7 * XO_MAXNV];
-      xo_prim Pst[7];
-      for (int m = 0; m < 7; ++m) {     /* cells i-3 .. i+3 */
-        const long id = idx[q] + (long)(m - 3) * st[d];
+      double Ust[9 * XO_MAXNV];
+      xo_prim Pst[9];
+      for (int m = 0; m <= 2 * h; ++m) {
+        const long id = idx[q] + (long)(m - h) * st[d];
         gather_cell(c, U, cells, id, Ust + m * Nv);
         xo_cell_primitives(c, Ust + m * Nv, Tguess[id], &Pst[m]);
         status |= Pst[m].status;
       }
       double Fl[XO_MAXNV], Fr[XO_MAXNV];
-      status |= xo_face_flux(c, d, Ust, Pst, Fl);            /* face i-1/2: cells i-3..i+2 */
-      status |= xo_face_flux(c, d, Ust + Nv, Pst + 1, Fr);   /* face i+1/2: cells i-2..i+3 */
+      status |= xo_face_flux(c, d, Ust, Pst, Fl);            /* face i-1/2: cells i-h..i+h-1 */
+      status |= xo_face_flux(c, d, Ust + Nv, Pst + 1, Fr);   /* face i+1/2: cells i-h+1..i+h */
+      if (c->positivity) {
+        const double kappa = 2.0 * D * c->pp_dt / dxs[d];
+        xo_positivity_blend(c, d, Ust + (h - 1) * Nv, Pst + h - 1, Ust + h * Nv, Pst + h, kappa, Fl);
+        xo_positivity_blend(c, d, Ust + h * Nv, Pst + h, Ust + (h + 1) * Nv, Pst + h + 1, kappa, Fr);
+      }
       for (int v = 0; v < Nv; ++v) acc[v] -= (Fr[v] - Fl[v]) / dxs[d];
     }
     for (int v = 0; v < Nv; ++v) rhs_out[q * Nv + v] = acc[v];
@@ -548,7 +648,10 @@ int xo_rhs_cells(const xo_config *c_in, const double *U, const double *Tguess, l
 /* ------------------------------------------------------------------------------------------------------------ */
 /* SSP-RK3 (Eq. 16); ghosts + primitives before each of the three residuals     */
 /* ------------------------------------------------------------------------------------------------------------ */
-int xo_rk3_step(const xo_config *c, double *U, double *T, double dt) {
+int xo_rk3_step(const xo_config *c_in, double *U, double *T, double dt) {
+  xo_config cc = *c_in;
+  cc.pp_dt = dt;                                          /* every stage is a forward-Euler step of size dt (Eq. 16, 17) */
+  const xo_config *c = &cc;
   const int Nv = c->N + 4;
   int np[3], n[3], g[3];
   long st[3];

@@ -37,7 +37,7 @@ enum { XO_OK = 0, XO_ENONPHYSICAL = 4, XO_ENOCONV = 5 };   /* status bits */
 
 typedef struct {
   int nx, ny, nz;             /* interior cells; n == 1 -> direction inactive (no ghosts, no sweep)           */
-  int ng;                     /* ghost width, 3                                                               */
+  int ng;                     /* ghost width: 3 (WENO5, WENO-CU6: stencil i-2..i+3) or 4 (WENO7: i-3..i+4)    */
   double dx, dy, dz;
   int N;                      /* species; Nv = N + 4                                                          */
   double Ru;
@@ -54,9 +54,13 @@ typedef struct {
                               /*   1 ROE: |lambda_n| of the Roe-averaged face state, no maximum                 */
                               /*   2 GLF: per field and direction, max of |lambda_n| over ALL padded cells      */
   double lam_glob[3][3];      /* GLF maxima [direction][u-c, u, u+c]; filled by the residual routines           */
-  int recon;                  /* reconstruction of Eq. 15: 0 WENO5-JS (reading R7), 1 WENO-CU6 ("[34]")  */
+  int recon;                  /* reconstruction of Eq. 15: 0 WENO5-JS (reading R7), 1 WENO-CU6 ("[34]"),  */
+                              /*   2 WENO7 ("[36]"; reading R18; needs ng = 4)                            */
+  int positivity;             /* 1: positivity-preserving flux blending for rho and rho Y_s (PAPER.md:120-141,         */
+                              /*    Eq. 17-20; the limiting factor theta: reading R17)                                 */
+  double pp_dt;               /* the time step the limiter guards (lambda = dt/dx of Eq. 17); xo_rk3_step sets it     */
 } xo_config;
-enum { XO_RECON_WENO5 = 0, XO_RECON_WENOCU6 = 1 };
+enum { XO_RECON_WENO5 = 0, XO_RECON_WENOCU6 = 1, XO_RECON_WENO7 = 2 };
 enum { XO_VISC_LLF = 0, XO_VISC_ROE = 1, XO_VISC_GLF = 2 };
 
 /* all primitive quantities of one cell (C2) */
@@ -90,8 +94,22 @@ double xo_weno5(const double v[5], int ideal_weights);
  * w_out (may be NULL) the four normalised weights */
 double xo_wenocu6(const double v[6], int ideal_weights, double *beta_out, double *w_out);
 
-/* C5-C7 numerical flux at one face from the 6 stencil cells (Ust[m][v], m = 0..5 <-> i-2..i+3) */
+/* WENO7 ("[36]") value at +1/2 from v[0..6] = v_{-3}..v_{+3}; beta_out / w_out (may be NULL): the four
+ * smoothness indicators / normalised weights */
+double xo_weno7(const double v[7], int ideal_weights, double *beta_out, double *w_out);
+
+/* number of stencil cells of a face flux: 6 (i-2..i+3) for WENO5 / WENO-CU6, 8 (i-3..i+4) for WENO7 */
+int xo_stencil_cells(const xo_config *c);
+
+/* C5-C7 numerical flux at one face from the S = xo_stencil_cells stencil cells (Ust[m][v], m = 0..S-1 <-> i-S/2+1..i+S/2;
+ * the face lies between m = S/2-1 and m = S/2) */
 int xo_face_flux(const xo_config *c, int d, const double *Ust, const xo_prim *Pst, double *Fhat);
+
+/* Positivity-preserving blending at one face (Eq. 17-20; reading R17): cells a = i, b = i+1 (conserved
+ * vectors + primitives), kappa = 2 D dt/dx_d (D = number of active directions), Fhat: in the high-order flux, out the
+ * blended flux F* = (1-theta) F^LF + theta Fhat.  Returns theta. */
+double xo_positivity_blend(const xo_config *c, int d, const double *Ua, const xo_prim *Pa, const double *Ub,
+                           const xo_prim *Pb, double kappa, double *Fhat);
 
 /* C8 ghost fill; C7 rhs, rk3, max wave speed.  U is [Nv][padded], T is [padded] (in: guess, out: T) */
 void xo_fill_ghosts(const xo_config *c, double *U);

@@ -27,10 +27,10 @@ namespace xf {
 #define XF_PRAGMA(x) _Pragma(#x)
 #define XF_UNROLL(n) XF_PRAGMA(unroll n)
 
-// the nonlinear part of one reconstruction as a fraction num/den and the linear part `base`
-__device__ __forceinline__ void weno5_parts(double v0, double v1, double v2, double v3, double v4, double &num,
-                                            double &den, double &base) {
-  const double D1 = v1 - v0, D2 = v2 - v1, D3 = v3 - v2, D4 = v4 - v3;
+// the nonlinear part of one reconstruction as a fraction num/den and the linear part `base`, from the centre value v2
+// and the four first differences D_k = v_k - v_{k-1}
+__device__ __forceinline__ void weno5_core(double v2, double D1, double D2, double D3, double D4, double &num,
+                                           double &den, double &base) {
   const double d0 = D2 - D1, d1 = D3 - D2, d2 = D4 - D3;
   const double e0 = fma(3.0, D2, -D1);   // v0 - 4 v1 + 3 v2
   const double e1 = D2 + D3;             // v3 - v1
@@ -46,13 +46,17 @@ __device__ __forceinline__ void weno5_parts(double v0, double v1, double v2, dou
   base = fma(fma(2.0, D3, D2), 1.0 / 6.0, v2);
 }
 
-__device__ __forceinline__ double weno5(double v0, double v1, double v2, double v3, double v4) {
-  double num, den, base;
-  weno5_parts(v0, v1, v2, v3, v4, num, den, base);
+__device__ __forceinline__ double weno5_finish(double num, double den, double base) {
   // 1/(2 den): the factor 1/2 is ONE integer subtraction on the exponent field (high word), not an fp64-pipe instruction
   const double rc = xf_rcp(den);
   const double rh = __hiloint2double(__double2hiint(rc) - 0x00100000, __double2loint(rc));
   return fma(num, rh, base);
+}
+
+__device__ __forceinline__ double weno5(double v0, double v1, double v2, double v3, double v4) {
+  double num, den, base;
+  weno5_core(v2, v1 - v0, v2 - v1, v3 - v2, v4 - v3, num, den, base);
+  return weno5_finish(num, den, base);
 }
 
 // WENO-CU6 (include/xf.h XF_RECON_WENOCU6; PAPER.md:107 ref 34) value at +1/2 from v0..v5 = v_{-2}..v_{+3}.
@@ -269,7 +273,7 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const d
       fp[m] = ap[m] * a;                                                                               \
       fm[m] = am[m] * a;                                                                               \
     }                                                                                                  \
-    const double g = weno_pair<RECON>(fp, fm);                                                               \
+    const double g = weno_pair<RECON>(fp, fm);                                                         \
     F4 = fma((DEXPR), g, F4);                                                                          \
     emit(VIDX, fma(C, s, g), VNEXT);                                                                   \
   }

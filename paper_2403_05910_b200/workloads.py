@@ -165,6 +165,7 @@ class Workload:
     cfl: float = 0.5                   # PAPER.md:135 (CFL <= 0.5)
     steps: int = 1
     notes: dict = field(default_factory=dict)
+    ng: int = NG                       # ghost width of the arrays: 3, or 4 for WENO7 (see ``with_ghost_width``)
 
     @property
     def nspecies(self) -> int:
@@ -184,9 +185,9 @@ class Workload:
 
     def interior(self, A: np.ndarray) -> np.ndarray:
         """View of the interior cells of a padded [..., nzp, nyp, nxp] array."""
-        gx = NG if self.nx > 1 else 0
-        gy = NG if self.ny > 1 else 0
-        gz = NG if self.nz > 1 else 0
+        gx = self.ng if self.nx > 1 else 0
+        gy = self.ng if self.ny > 1 else 0
+        gz = self.ng if self.nz > 1 else 0
         return A[..., gz:gz + self.nz, gy:gy + self.ny, gx:gx + self.nx]
 
 
@@ -195,10 +196,18 @@ def padded_dims(nx: int, ny: int, nz: int) -> Tuple[int, int, int]:
     return (nz + 2 * NG if nz > 1 else 1, ny + 2 * NG if ny > 1 else 1, nx + 2 * NG if nx > 1 else 1)
 
 
-def _pad(A: np.ndarray, nx: int, ny: int, nz: int) -> np.ndarray:
+def _pad(A: np.ndarray, nx: int, ny: int, nz: int, ng: int = NG) -> np.ndarray:
     """interior [..., nz, ny, nx] -> padded, edge-replicated ghosts."""
-    pw = [(0, 0)] * (A.ndim - 3) + [(NG, NG) if n > 1 else (0, 0) for n in (nz, ny, nx)]
+    pw = [(0, 0)] * (A.ndim - 3) + [(ng, ng) if n > 1 else (0, 0) for n in (nz, ny, nx)]
     return np.ascontiguousarray(np.pad(A, pw, mode="edge"))
+
+
+def with_ghost_width(w: "Workload", ng: int) -> "Workload":
+    """The same workload with ``ng`` ghost layers per active direction (WENO7 needs 4: stencil i-3..i+4)."""
+    import dataclasses
+
+    return dataclasses.replace(w, U=_pad(np.ascontiguousarray(w.interior(w.U)), w.nx, w.ny, w.nz, ng),
+                               T_guess=_pad(np.ascontiguousarray(w.interior(w.T_guess)), w.nx, w.ny, w.nz, ng), ng=ng)
 
 
 def conserved_from_primitive(table: SpeciesTable, rho, u, v, w, T, Y) -> np.ndarray:

@@ -96,3 +96,64 @@ for j0 in range(0, 150, 19):
     out_lines.append(",".join(x.hex() for x in vs) + ";" + float(b6).hex())
 (Path(__file__).resolve().parent / "wenocu6_beta6_smooth.txt").write_text("\n".join(out_lines) + "\n")
 print("\n".join(out_lines))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# WENO7 (PAPER.md:107 names the scheme, ref 36, and prints no formula; reading R18): candidates, linear
+# weights and smoothness indicators derived in exact rational arithmetic from their definitions --
+#   candidate k (k = 0..3): the cubic whose cell averages over cells i-3+k .. i+k are the data, evaluated at x_{i+1/2};
+#   linear weights d_k: the combination that reproduces the 7-point (degree-6) interpolation;
+#   beta_k = sum_{l=1..3} dx^(2l-1) int_cell_i (d^l p_k/dx^l)^2 dx  (the Jiang-Shu measure), as a quadratic form of the
+#   four values and of the three first differences D_m = f_{k+m+1} - f_{k+m} of the sub-stencil, both times 240.
+# ---------------------------------------------------------------------------------------------------------------
+def _basis(cells):
+    m = len(cells)
+    Am = [[_polyint([Fr(0)] * k + [Fr(1)], Fr(2 * c - 1, 2), Fr(2 * c + 1, 2)) for k in range(m)] for c in cells]
+    Mm = [row[:] + [Fr(int(i == j)) for j in range(m)] for i, row in enumerate(Am)]
+    for c in range(m):
+        piv = next(r for r in range(c, m) if Mm[r][c] != 0)
+        Mm[c], Mm[piv] = Mm[piv], Mm[c]
+        pv = Mm[c][c]
+        Mm[c] = [x / pv for x in Mm[c]]
+        for r in range(m):
+            if r != c and Mm[r][c] != 0:
+                f = Mm[r][c]
+                Mm[r] = [x - f * y for x, y in zip(Mm[r], Mm[c])]
+    inv = [row[m:] for row in Mm]
+    return [[inv[k][j] for k in range(m)] for j in range(m)]
+
+
+def _polyval(a, x):
+    return sum(c * x ** k for k, c in enumerate(a))
+
+
+w7 = ["# WENO7: exact coefficients from the definitions; written by tests/golden/make_golden.py"]
+cands, full = [], [_polyval(p, Fr(1, 2)) for p in _basis(list(range(-3, 4)))]
+w7.append("interp7_times_420=" + ",".join(str(x * 420) for x in full))
+for k in range(4):
+    P4 = _basis(list(range(k - 3, k + 1)))
+    cands.append([_polyval(p, Fr(1, 2)) for p in P4])
+    w7.append(f"cand{k}_times_12=" + ",".join(str(x * 12) for x in cands[k]))
+    B = [[Fr(0)] * 4 for _ in range(4)]
+    for a_ in range(4):
+        for b_ in range(4):
+            pa, pb = P4[a_], P4[b_]
+            for _ in range(1, 4):
+                pa, pb = _polyder(pa), _polyder(pb)
+                B[a_][b_] += _polyint(_polymul(pa, pb), Fr(-1, 2), Fr(1, 2))
+    assert all(sum(row) == 0 for row in B)                 # translation invariance
+    w7.append(f"beta{k}_values_times_240=" + ";".join(
+        ",".join(str(B[a_][b_] * (1 if a_ == b_ else 2) * 240) for b_ in range(a_, 4)) for a_ in range(4)))
+    G = [[sum(B[a_][b_] for a_ in range(m + 1, 4) for b_ in range(l + 1, 4)) for l in range(3)] for m in range(3)]
+    w7.append(f"beta{k}_differences_times_240=" + ";".join(
+        ",".join(str(G[m][l] * (1 if m == l else 2) * 240) for l in range(m, 3)) for m in range(3)))
+dlin = [None] * 4
+dlin[0] = full[0] / cands[0][0]
+dlin[3] = full[6] / cands[3][3]
+dlin[1] = (full[1] - dlin[0] * cands[0][1]) / cands[1][0]
+dlin[2] = (full[5] - dlin[3] * cands[3][2]) / cands[2][3]
+for j in range(7):
+    assert sum(dlin[k] * cands[k][j - k] for k in range(4) if 0 <= j - k < 4) == full[j]
+w7.append("linear_weights=" + ",".join(str(x) for x in dlin))
+(Path(__file__).resolve().parent / "weno7_coefficients.txt").write_text("\n".join(w7) + "\n")
+print("\n".join(w7))
