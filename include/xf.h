@@ -7,9 +7,9 @@
  * Conventions
  *   Variables   Nv = N + 4 per cell: v = 0 rho, 1..3 rho u, rho v, rho w, 4 E, 5.. rho Y_1 .. rho Y_{N-1}
  *               (Eq. 2; "s = 1..N-1"); Y_N = 1 - sum of the others.
- *   Layout      SoA, fp64, U[v][k][j][i], i fastest.  Every ACTIVE direction (n_d > 1) carries ng = 3 ghost cells
- *               on both sides (WENO5 stencil i-2..i+3); an inactive direction (n_d == 1) has none.
- *               padded extent np_d = n_d + 6 (active) or 1; padded cells = npx*npy*npz; field v starts at
+ *   Layout      SoA, fp64, U[v][k][j][i], i fastest.  Every ACTIVE direction (n_d > 1) carries ng ghost cells on both
+ *               sides (ng = 3: WENO5 stencil i-2..i+3; ng = 4 for WENO7); an inactive direction
+ *               (n_d == 1) has none.  padded extent np_d = n_d + 2 ng (active) or 1; padded cells = npx*npy*npz; field v starts at
  *               U + v*padded_cells.  Scalar fields (T, p, c) are [k][j][i] over the same padded box.
  *   Memory      All field pointers are CALLER-OWNED DEVICE memory (8-byte aligned) unless the name ends in
  *               _host.  The library allocates nothing per call; the context owns the species table, boundary
@@ -49,7 +49,7 @@ enum { XF_BC_PERIODIC = 0, XF_BC_TRANSMISSIVE = 1, XF_BC_REFLECTIVE = 2, XF_BC_D
 
 typedef struct {
   int nx, ny, nz;          /* interior cells; == 1 -> direction inactive (no ghosts, no sweep)                  */
-  int ng;                  /* ghost width; must be 3 (WENO5)                                                    */
+  int ng;                  /* ghost width = half the stencil: 3 (WENO5, WENO-CU6), 4 for XF_RECON_WENO7         */
   double dx, dy, dz;
   int nspecies;            /* N in 1..XF_MAX_SPECIES; Nv = N + 4                                                */
   double Ru;               /* universal gas constant in the caller's units (Eq. 7)                  */
@@ -63,14 +63,30 @@ typedef struct {
   int device;              /* CUDA ordinal                                                                      */
   int viscosity;           /* XF_VISC_*: the artificial viscosity Lambda~ of Eq. 14 (options 374)  */
   int reconstruction;      /* XF_RECON_*: the reconstruction of Eq. 15                            */
+  int positivity;          /* != 0: positivity-preserving flux blending of Eq. 17-20, see below */
 } xf_config;
+
+/* Positivity-preserving flux blending (theta is deferred by the paper to its ref 41 -> DESIGN.md
+ * reading R17).  Every face flux of every sweep becomes F* = (1 - theta) F^LF + theta Fhat (Eq. 20) with the first-order
+ * Lax-Friedrichs flux F^LF = (F_a + F_b + Lambda~ (U_a - U_b))/2 of the two adjacent cells (Eq. 19, Lambda~ = max(|u_d| +
+ * c)).  Guarded: q in {rho, rho Y_1, .., rho Y_N (by closure)}; with kappa = 2 D dt/dx_d (Eq. 18, D active directions)
+ * the half-states q(U_a) - kappa q(F), q(U_b) + kappa q(F) must stay >= eps = min(1e-13, the same half-state under
+ * F^LF); theta in [0, 1] is the largest factor for which all 2 (N + 1) of them do; one factor for the whole flux vector.
+ * theta = 1 (flux untouched, bit-identical residual) wherever nothing is violated.  dt is the forward-Euler step the
+ * limiter guards: the step of xf_rk3_step / xf_rk3_step_cfl / xf_step_cfl in each of their three stages, and for a bare
+ * xf_convective_rhs the value set by xf_set_rhs_dt (initially 0: every guard passes when U itself is non-negative).
+ * Non-negativity of rho and Y_s after a stage holds if D dt Lambda~/dx_d <= 1/2 in every direction ("CFL <= 0.5",
+ * PAPER.md:135). */
 
 /* Reconstruction of the split characteristic fluxes at a face:
  *   WENO5   Jiang-Shu, eps = 1e-6, exponent 2 (reading R7; the default), points i-2..i+2 / mirrored
  *   WENOCU6 the six-point central-upwind scheme of the paper's ref 34 (reading R16: linear weights 1/20, 9/20, 9/20,
  *           1/20; fourth indicator = the six-point Jiang-Shu measure beta_6; tau_6 = beta_6 - (beta_0 + 4 beta_1 +
- *           beta_2)/6; alpha_k = d_k (20 + tau_6/(beta_k + 1e-40))), points i-2..i+3 / mirrored: same ghost width */
-enum { XF_RECON_WENO5 = 0, XF_RECON_WENOCU6 = 1 };
+ *           beta_2)/6; alpha_k = d_k (20 + tau_6/(beta_k + 1e-40))), points i-2..i+3 / mirrored: same ghost width
+ *   WENO7   the seventh-order scheme of the paper's ref 36 (reading R18: four cubic candidates, linear weights 1/35,
+ *           12/35, 18/35, 4/35, Jiang-Shu indicators of the cubics, alpha_k = d_k/(1e-6 + beta_k)^2), points i-3..i+3 /
+ *           mirrored: stencil i-3..i+4, so the context must be created with ng = 4 */
+enum { XF_RECON_WENO5 = 0, XF_RECON_WENOCU6 = 1, XF_RECON_WENO7 = 2 };
 
 /* Lambda~_n of the flux splitting f+- = (L F +- Lambda~ L U)/2, per characteristic field n:
  *   LLF  max over the six stencil cells of |lambda_n| of each cell's own state (reading R8; the default)
@@ -90,7 +106,7 @@ size_t xf_workspace_bytes(const xf_ctx *ctx);     /* scratch for xf_rk3_step: th
 
 /* Ghost-cell fill ("specific boundary conditions"; reading R10): periodic wrap,
  * transmissive copy of the nearest interior cell, reflective mirror with the wall-normal momentum negated, or the
- * stored Dirichlet state; 3 layers; x, then y, then z, so that edges and corners are defined.  U in place. */
+ * stored Dirichlet state; ng layers; x, then y, then z, so that edges and corners are defined.  U in place. */
 int xf_fill_ghosts(xf_ctx *ctx, double *U, void *stream);
 
 /* Primitive recovery for every padded cell (Eq. 21): T by Newton iteration on
@@ -104,6 +120,9 @@ int xf_primitives(xf_ctx *ctx, const double *U, double *T, double *p, double *c,
  * overwritten, interior read-only), primitives (T in/out), the x, y, z sweeps.  rhs is [Nv][padded]; only interior
  * entries are written.  work: xf_rhs_workspace_bytes. */
 int xf_convective_rhs(xf_ctx *ctx, double *U, double *T, double *rhs, void *work, void *stream);
+
+/* The time step assumed by the positivity limiter of a bare xf_convective_rhs (see xf_config.positivity); dt >= 0. */
+int xf_set_rhs_dt(xf_ctx *ctx, double dt);
 
 /* One SSP-RK3 step with fixed dt (Eq. 16): three times (ghost fill, primitives, residual,
  * stage combination).  U: in U^n, out U^{n+1} (interior; ghosts are left as filled for the last stage).

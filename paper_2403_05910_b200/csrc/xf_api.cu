@@ -26,6 +26,8 @@ struct xf_ctx {
   double *S_dev;                      // max wave speed scalar used by the host-buffer entry points
   double *lam_glob_dev;               // GLF: [3][3] global maxima of the current residual evaluation
   int visc, recon;                    // XF_VISC_*, XF_RECON_*
+  int positivity;                     // positivity-preserving flux blending on (Eq. 17-20)
+  double rhs_dt;                      // the step the limiter of a bare xf_convective_rhs guards (xf_set_rhs_dt)
   long launches;
   XfTmapCache tmaps;                  // tensor maps of the TMA sweeps, per (base pointer, fields)
   // lazily allocated device mirrors for the *_host entry points
@@ -138,6 +140,10 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
     E.visc = c->visc;
     E.recon = c->recon;
     E.lam_glob = c->lam_glob_dev;
+    E.pp = c->positivity;       // the limiter guards the forward-Euler step of this stage (or of xf_set_rhs_dt)
+    E.pp_dt = E_last.mode == 2 ? E_last.dt : c->rhs_dt;
+    E.pp_cfl = E_last.cfl;
+    E.pp_S = E_last.mode == 2 ? E_last.S_dev : nullptr;
     Timed t(c, XF_K_SWEEP_X + d, s);
     if (d == 0) rc = xf_launch_sweep_x(c->G, c->N, U, prim, E, c->status_dev, &c->tmaps, s);
     else if (d == 1) rc = xf_launch_sweep_y(c->G, c->N, U, prim, E, c->status_dev, &c->tmaps, s);
@@ -199,14 +205,16 @@ int xf_create(xf_ctx **out, const xf_config *cfg) {
   if (!out || !cfg) return XF_EINVAL;
   *out = nullptr;
   const int N = cfg->nspecies;
-  if (cfg->ng != XF_NG || N < 1 || N > XF_MAXN || cfg->nx < 1 || cfg->ny < 1 || cfg->nz < 1) return XF_EINVAL;
+  if (cfg->reconstruction < XF_RECON_WENO5 || cfg->reconstruction > XF_RECON_WENO7) return XF_EINVAL;
+  const int ng = cfg->reconstruction == XF_RECON_WENO7 ? 4 : 3;   // half the stencil: i-2..i+3, or i-3..i+4
+  if (cfg->ng != ng || N < 1 || N > XF_MAXN || cfg->nx < 1 || cfg->ny < 1 || cfg->nz < 1) return XF_EINVAL;
   if (!cfg->W || !cfg->nasa7 || !(cfg->Ru > 0.0) || !(cfg->Thi > cfg->Tlo)) return XF_EINVAL;
   const int n[3] = {cfg->nx, cfg->ny, cfg->nz};
   const double dxs[3] = {cfg->dx, cfg->dy, cfg->dz};
   for (int d = 0; d < 3; ++d) {
     if (n[d] == 1) continue;
     if (!(dxs[d] > 0.0)) return XF_EINVAL;
-    if (n[d] < XF_NG) return XF_EINVAL;  // ghost layers are copies of interior layers: need >= 3 of them
+    if (n[d] < ng) return XF_EINVAL;  // ghost layers are copies of interior layers: need >= ng of them
     for (int side = 0; side < 2; ++side) {
       const int b = cfg->bc[2 * d + side];
       if (b < XF_BC_PERIODIC || b > XF_BC_DIRICHLET) return XF_EINVAL;
@@ -218,7 +226,6 @@ int xf_create(xf_ctx **out, const xf_config *cfg) {
     if (!(cfg->W[s] > 0.0)) return XF_EINVAL;
   if (n[0] == 1 && n[1] == 1 && n[2] == 1) return XF_EINVAL;
   if (cfg->viscosity < XF_VISC_LLF || cfg->viscosity > XF_VISC_GLF) return XF_EINVAL;
-  if (cfg->reconstruction < XF_RECON_WENO5 || cfg->reconstruction > XF_RECON_WENOCU6) return XF_EINVAL;
   if (n[1] > 65535 || n[2] > 65535) return XF_EINVAL;  // they index the y dimension of the y/z sweep grids
 
   int ndev = 0;
@@ -234,10 +241,11 @@ int xf_create(xf_ctx **out, const xf_config *cfg) {
   c->device = cfg->device;
   c->visc = cfg->viscosity;
   c->recon = cfg->reconstruction;
+  c->positivity = cfg->positivity != 0;
   XfGrid &G = c->G;
   for (int d = 0; d < 3; ++d) {
     G.n[d] = n[d];
-    G.g[d] = n[d] > 1 ? XF_NG : 0;
+    G.g[d] = n[d] > 1 ? ng : 0;
     G.np[d] = n[d] + 2 * G.g[d];
     G.inv_d[d] = n[d] > 1 ? 1.0 / dxs[d] : 0.0;
   }
@@ -337,6 +345,12 @@ int xf_convective_rhs(xf_ctx *c, double *U, double *T, double *rhs, void *work, 
   E.mode = 0;
   E.out = rhs;
   return residual(c, U, T, work, rhs, E, static_cast<cudaStream_t>(stream));
+}
+
+int xf_set_rhs_dt(xf_ctx *c, double dt) {
+  if (!c || !(dt >= 0.0) || isinf(dt)) return XF_EINVAL;
+  c->rhs_dt = dt;
+  return XF_OK;
 }
 
 int xf_rk3_step(xf_ctx *c, double *U, double *T, double dt, void *work, void *stream) {

@@ -6,7 +6,6 @@
 
 #include "../../include/xf.h"
 
-#define XF_NG 3
 #define XF_MAXN XF_MAX_SPECIES
 #define XF_MAXNV (XF_MAXN + 4)
 
@@ -58,6 +57,11 @@ struct XfEpilogue {
   int visc;           // XF_VISC_*: Lambda~ of Eq. 14
   int recon;          // XF_RECON_*: reconstruction of Eq. 15 (host-side dispatch of the kernel instantiation)
   const double *lam_glob;  // GLF: [direction][u-c, u, u+c] global maxima on the device
+  // positivity-preserving flux blending (Eq. 17-20; reading R17), set for EVERY sweep of a
+  // residual: the limiter guards a forward-Euler step of size dt, dt = pp_cfl / *pp_S if pp_S else pp_dt
+  int pp;
+  double pp_dt, pp_cfl;
+  const double *pp_S;
 };
 
 // Tensor maps of the TMA sweeps depend only on (base pointer, number of fields, grid): encoded once and kept in the

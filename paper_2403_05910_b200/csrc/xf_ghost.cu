@@ -5,7 +5,7 @@
 namespace {
 
 // thread <-> (transverse cell, layer l, side); loops over the Nv variables (stride = cells keeps every access of a
-// warp on consecutive i for the y and z fills; the x fill touches 3-cell runs and is tiny).
+// warp on consecutive i for the y and z fills; the x fill touches 3- or 4-cell runs and is tiny).
 __global__ void __launch_bounds__(256)
 ghost_kernel(const XfGrid G, int Nv, int d, int bc_lo, int bc_hi, const double *__restrict__ bc_state,
              double *__restrict__ U) {
@@ -19,20 +19,21 @@ ghost_kernel(const XfGrid G, int Nv, int d, int bc_lo, int bc_hi, const double *
   const int a1 = d == 0 ? 1 : 0;          // faster transverse axis
   const int a2 = d == 2 ? 1 : 2;          // slower transverse axis
   const long long ntrans = (long long)ext[a1] * ext[a2];
-  const long long total = ntrans * XF_NG * 2;
+  const int ng = G.g[d];                  // ghost layers per side: 3, or 4 for WENO7
+  const long long total = ntrans * ng * 2;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= total) return;
   long long tr;
   int l, side;
-  if (d == 0) {  // x fill: the 3 layers of one row end are neighbours in memory -> make them neighbours in the warp
-    l = (int)(t % XF_NG);
-    side = (int)((t / XF_NG) & 1);
-    tr = t / (2 * XF_NG);
+  if (d == 0) {  // x fill: the ng layers of one row end are neighbours in memory -> make them neighbours in the warp
+    l = (int)(t % ng);
+    side = (int)((t / ng) & 1);
+    tr = t / (2 * ng);
   } else {       // y / z fill: consecutive threads on consecutive i
     tr = t % ntrans;
     const int ls = (int)(t / ntrans);
-    l = ls % XF_NG;
-    side = ls / XF_NG;
+    l = ls % ng;
+    side = ls / ng;
   }
   const int p1 = lo[a1] + (int)(tr % ext[a1]);
   const int p2 = lo[a2] + (int)(tr / ext[a1]);
@@ -80,7 +81,7 @@ int xf_launch_ghosts(const XfGrid &G, int Nv, const XfBc &bc, const double *bc_s
     long long ntrans = 1;
     for (int q = 0; q < 3; ++q)
       if (q != d) ntrans *= (q < d ? G.np[q] : G.n[q]);
-    const long long total = ntrans * XF_NG * 2;
+    const long long total = ntrans * G.g[d] * 2;
     const int threads = 256;
     const unsigned blocks = (unsigned)((total + threads - 1) / threads);
     ghost_kernel<<<blocks, threads, 0, s>>>(G, Nv, d, bc.kind[2 * d], bc.kind[2 * d + 1], bc_state_dev, U);

@@ -19,10 +19,10 @@ int launch(const XfGrid &G, int N, const double *U, const double *prim, const Xf
   const int seg_len = (n + nseg - 1) / nseg;
   nseg = (n + seg_len - 1) / seg_len;
   const dim3 grid(strips, G.n[OD], nseg), block(32, 2 * YZ_W);
-  const size_t smem = sizeof(double) * yz_smem_doubles(N, YZ_W);
+  const size_t smem = sizeof(double) * yz_smem_doubles(N, YZ_W, stencil_cells(RC));
   // U [N + 4]; p, c, 1/rho [3]; Gamma, chi_s [N + 1]
   const CUtensorMap *tmU = nullptr, *tmP = nullptr, *tmS = nullptr;
-  if (G.g[0] == XF_NG) {
+  if (G.g[0] > 0) {
     tmU = xf_tmap(tc, G, U, N + 4, 0);
     tmP = xf_tmap(tc, G, prim, 3, 0);
     tmS = xf_tmap(tc, G, prim + 3 * G.cells, N + 1, 0);
@@ -40,7 +40,15 @@ int launch(const XfGrid &G, int N, const double *U, const double *prim, const Xf
 
 int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
                       XfTmapCache *tc, cudaStream_t s) {
-#define CALL(NT) return E.recon == 1 ? launch<NT, 1>(G, N, U, prim, E, status, tc, s) : launch<NT, 0>(G, N, U, prim, E, status, tc, s)
+  // kernel instantiation: the reconstruction, with WENO5 in its relative-accuracy form when the limiter is on
+  const int rc = E.recon == XF_RECON_WENO5 && E.pp ? 3 : E.recon;
+#define CALL(NT)                                                            \
+  switch (rc) {                                                             \
+    case 1: return launch<NT, 1>(G, N, U, prim, E, status, tc, s);          \
+    case 2: return launch<NT, 2>(G, N, U, prim, E, status, tc, s);          \
+    case 3: return launch<NT, 3>(G, N, U, prim, E, status, tc, s);          \
+    default: return launch<NT, 0>(G, N, U, prim, E, status, tc, s);         \
+  }
   XF_DISPATCH_SWEEP_N(N, CALL)
 #undef CALL
   return XF_EINVAL;
@@ -51,9 +59,10 @@ int xf_sweep_y_init() {
   cudaError_t e = cudaSuccess;
 #define CALL2(NT, TM, RC)                                                                                        \
   e = cudaFuncSetAttribute(sweep_yz_ws_kernel<NT, DIR, YZ_W, TM, RC>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
-                           (int)(sizeof(double) * yz_smem_doubles(NT > 0 ? NT : XF_MAXN, YZ_W)));                    \
+                           (int)(sizeof(double) * yz_smem_doubles(NT > 0 ? NT : XF_MAXN, YZ_W, stencil_cells(RC))));                    \
   if (e != cudaSuccess) return XF_ECUDA;
-#define CALL(NT) CALL2(NT, true, 0) CALL2(NT, false, 0) CALL2(NT, true, 1) CALL2(NT, false, 1)
+#define CALL(NT) CALL2(NT, true, 0) CALL2(NT, false, 0) CALL2(NT, true, 1) CALL2(NT, false, 1) \
+  CALL2(NT, true, 2) CALL2(NT, false, 2) CALL2(NT, true, 3) CALL2(NT, false, 3)
   CALL(0) CALL(1) CALL(2) CALL(3) CALL(4) CALL(10)
 #undef CALL
 #undef CALL2

@@ -13,22 +13,22 @@
 //   x sweep: LI = 1, LJ = 32.  All interior rows of one k-plane are contiguous in memory (row pitch = padded nx),
 //     so a plane is swept as ONE long flat pencil; the few faces whose stencil straddles a row end are computed
 //     on valid (ghost) data and never used (5 of every nx+6).
-// A chunk of LJ face rows needs LJ + 5 stencil rows; the ring holds RR rows (LJ + 5 .. 2 LJ + 5: the rows beyond LJ + 5
-// let part of the next chunk land while the current one is computed).  Face row f of a segment is the lower face of
-// cell f; its stencil is rows f .. f+5; the lane that owns face f updates cell f-1 from its own flux and that of face
-// f-1 (the lane LI below it, or the carry left in shared memory by the previous chunk).
+// With S stencil cells per face (6; 8 for WENO7; ghost width S/2) a chunk of LJ face rows needs LJ + S - 1 stencil rows;
+// the ring holds RR rows (LJ + S - 1 .. 2 LJ + S - 1: the rows beyond the first count let part of the next chunk land while
+// the current one is computed).  Face row f of a segment is the lower face of cell f; its stencil is rows f .. f+S-1; the
+// lane that owns face f updates cell f-1 (stencil row f + S/2 - 1) from its own flux and that of face f-1 (the lane LI below it, or the carry left in shared memory by the previous chunk).
 #pragma once
 #include "xf_flux.cuh"
 
 namespace xf {
 
 constexpr int X_LI = 1, X_LJ = 32, X_NCH = 16;   // x sweep: segment = X_NCH chunks = 32*X_NCH faces, 32*X_NCH - 1 cells
-constexpr int X_RR = X_LJ + 5, X_MINB = 12;       // ring of exactly one chunk, 12 warps per SM (measured best, profiles/)
+constexpr int X_MINB = 12;                        // ring of exactly one chunk (X_LJ + S - 1 rows), 12 warps per SM
 constexpr int YZ_W = 4;                           // y/z sweeps: warps per block = face rows per chunk
 
-__host__ __device__ constexpr int ring_rows(int LJ) { return 2 * LJ + 5; }
-__host__ __device__ inline size_t warp_smem_doubles(int N, int LI, int RR) {
-  return (size_t)nstaged(N) * RR * LI + 2 * (size_t)(N + 4) * LI;
+__host__ __device__ constexpr int ring_rows(int LJ, int S) { return 2 * LJ + S - 1; }   // S stencil cells per face
+__host__ __device__ inline size_t warp_smem_doubles(int N, int LI, int RR) {   // ring, carry x 2, flux scratch [Nv][32]
+  return (size_t)nstaged(N) * RR * LI + 2 * (size_t)(N + 4) * LI + (size_t)(N + 4) * 32;
 }
 
 __device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc) {
@@ -100,6 +100,11 @@ struct CellWriter {
   }
 };
 
+struct FluxScratch {   // face_flux emitter that only parks the components: scr[v * 32]
+  double *scr;
+  __device__ __forceinline__ void operator()(int v, double F, int) { scr[v * 32] = F; }
+};
+
 // One warp = one segment of one pencil group.  DIR = 0: blockIdx.x enumerates (k-plane, segment of the flat pencil).
 // DIR = 1, 2: blockIdx = (group of LI pencils along i, index along the other transverse direction, segment).
 template <int N_T, int DIR, int LI, int LJ, int RR, int MINB, int RECON>
@@ -109,8 +114,9 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
   static_assert(LI * LJ == 32, "one lane per face");
   const int N = N_T > 0 ? N_T : Nrt;
   const int Nv = N + 4, NST = nstaged(N);
-  static_assert(RR >= LJ + 5 && RR <= 2 * LJ + 5, "ring: one chunk plus 0..LJ rows of prefetch");
-  constexpr int PF = RR - (LJ + 5);                         // rows of the next chunk that land during the arithmetic
+  constexpr int S = stencil_cells(RECON), HW = S / 2, MA = S / 2 - 1;   // stencil cells, ghost width, cell below the face
+  static_assert(RR >= LJ + S - 1 && RR <= 2 * LJ + S - 1, "ring: one chunk plus 0..LJ rows of prefetch");
+  constexpr int PF = RR - (LJ + S - 1);                     // rows of the next chunk that land during the arithmetic
   constexpr int FS = RR * LI;
   extern __shared__ double smem[];
   double *sm = smem;
@@ -132,7 +138,7 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
     constexpr int SEGC = X_NCH * 32 - 1;
     f_begin = seg * SEGC;
     f_end = f_begin + SEGC < L ? f_begin + SEGC : L;
-    base = (long long)(plane + G.g[2]) * G.st[2] + (long long)G.g[1] * G.st[1] - 3;  // row r <-> flat cell r - 3
+    base = (long long)(plane + G.g[2]) * G.st[2] + (long long)G.g[1] * G.st[1] - HW;  // row r <-> flat cell r - HW
     sst = 1;
   } else {
     constexpr int OD = DIR == 1 ? 2 : 1;                     // the other transverse direction
@@ -165,8 +171,8 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
     }
   };
 
-  // ---- prologue: rows f_begin .. f_begin + LJ + 4 into ring slots 0 .. LJ + 4
-  for (int idx = lane; idx < (LJ + 5) * LI; idx += 32) {
+  // ---- prologue: rows f_begin .. f_begin + LJ + S - 2 into ring slots 0 .. LJ + S - 2
+  for (int idx = lane; idx < (LJ + S - 1) * LI; idx += 32) {
     const int r = idx / LI, l = idx - r * LI;
     stage(r * LI + l, row_addr(f_begin + r, l));
   }
@@ -192,34 +198,34 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
   int par = 0;
   bool bad = false;
   for (int fc = f_begin; fc <= f_end; fc += LJ) {
-    // ---- prefetch the first PF new rows of the next chunk (rows fc + LJ + 5 + lj) into the free part of the ring
+    // ---- prefetch the first PF new rows of the next chunk (rows fc + LJ + S - 1 + lj) into the free part of the ring
     if (PF > 0 && lj < PF && fc + LJ <= f_end) {
-      int slot = rb + LJ + 5 + lj;
+      int slot = rb + LJ + S - 1 + lj;
       slot -= slot >= RR ? RR : 0;
-      stage(slot * LI + li, row_addr(fc + LJ + 5 + lj, li));
+      stage(slot * LI + li, row_addr(fc + LJ + S - 1 + lj, li));
     }
     cp_async_commit();
     cp_async_wait<1>();   // everything but the group just committed has landed
     __syncwarp();
 
     const int f = fc + lj;
-    int o[6];
+    int o[S];
 #pragma unroll
-    for (int m = 0; m < 6; ++m) {
+    for (int m = 0; m < S; ++m) {
       int s = rb + lj + m;
       s -= s >= RR ? RR : 0;
       o[m] = s * LI + li;
     }
-    // the cell this lane updates: f - 1 (between faces f - 1 and f), staged at stencil row f + 2 (m = 2)
+    // the cell this lane updates: f - 1 (between faces f - 1 and f), staged at stencil row f + MA (m = MA)
     bool ok = lane_ok && f > f_begin && f <= f_end;
     long long gi;
     if (DIR == 0) {
       const int cc = f - 1;
       const int i = cc % G.np[0];
       ok = ok && i >= G.g[0] && i < G.g[0] + G.n[0];
-      gi = base + 3 + cc;
+      gi = base + HW + cc;
     } else {
-      gi = base + (i0 + li) + (long long)(f + 2) * sst;
+      gi = base + (i0 + li) + (long long)(f + MA) * sst;
     }
     W.write_ok = ok;
     W.gi = gi;
@@ -229,20 +235,35 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
       if (lane_ok && f + LJ <= f_end && gnext < G.cells) W.prefetch_l2(gnext, Nv);
     }
 #pragma unroll
-    for (int m = 0; m < 6; ++m) asm volatile("" : "+r"(o[m]));   // keep the six ring offsets in registers (see the y/z kernel)
-    W.sm_us = sm + o[2];
+    for (int m = 0; m < S; ++m) asm volatile("" : "+r"(o[m]));   // keep the ring offsets in registers (see the y/z kernel)
+    W.sm_us = sm + o[MA];
     W.carry_rd = carry + par * Nv * LI;
     W.carry_wr = carry + (par ^ 1) * Nv * LI;
     W.preload(0);
-    const bool c2ok = face_flux<DIR, RECON>(N, sm, sm + Nv * FS, FS, o, sm + (Nv + 3) * FS, FS, o[2], o[3], E.visc, E.lam_glob + 3 * DIR, W);
+    bool c2ok;
+    if (E.pp) {   // the limiter needs the whole flux vector: park it in the warp's scratch, blend (Eq. 20), then difference
+      double *scr = carry + 2 * Nv * LI + lane;
+      FluxScratch fs{scr};
+      c2ok = face_flux<DIR, RECON>(N, sm, sm + Nv * FS, FS, o, sm + (Nv + 3) * FS, FS, o[MA], o[MA + 1], E.visc, E.lam_glob + 3 * DIR, fs);
+      positivity_blend<DIR>(N, sm, sm + Nv * FS, FS, o[MA], o[MA + 1], pp_kappa(E, G, DIR), scr, 32);
+      constexpr int nd = Axes<DIR>::nd, t1 = Axes<DIR>::t1, t2 = Axes<DIR>::t2;
+      W(0, scr[0], 1 + nd);                                 // same component order as face_flux emits
+      W(1 + nd, scr[(1 + nd) * 32], 1 + t1);
+      W(1 + t1, scr[(1 + t1) * 32], 1 + t2);
+      W(1 + t2, scr[(1 + t2) * 32], N > 1 ? 5 : 4);
+      for (int i = 0; i < N - 1; ++i) W(5 + i, scr[(5 + i) * 32], i + 2 < N ? 6 + i : 4);
+      W(4, scr[4 * 32], -1);
+    } else {
+      c2ok = face_flux<DIR, RECON>(N, sm, sm + Nv * FS, FS, o, sm + (Nv + 3) * FS, FS, o[MA], o[MA + 1], E.visc, E.lam_glob + 3 * DIR, W);
+    }
     bad = bad || (!c2ok && lane_ok && f <= f_end);
     __syncwarp();         // all lanes are done with the rows the next iteration's prefetch overwrites
     if (PF < LJ) {        // the remaining LJ - PF rows of the next chunk go where this chunk's first rows were
       if (lj >= PF && fc + LJ <= f_end) {
-        int slot = rb + LJ + 5 + lj;
+        int slot = rb + LJ + S - 1 + lj;
         slot -= slot >= RR ? RR : 0;
         slot -= slot >= RR ? RR : 0;
-        stage(slot * LI + li, row_addr(fc + LJ + 5 + lj, li));
+        stage(slot * LI + li, row_addr(fc + LJ + S - 1 + lj, li));
       }
       cp_async_commit();
     }
@@ -263,17 +284,17 @@ sweep_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, const 
 // row 0 is the last face of the previous chunk) and are differenced from there.
 // ---------------------------------------------------------------------------------------------------------------
 // TMA layout (doubles).  A box must start 16-byte aligned in global memory and 128-byte aligned in shared memory
-// (measured: anything else raises "illegal instruction" / "misaligned address"), and the interior starts at the odd
-// index 3, so a row is fetched as 34 doubles from i0 - 1: lane l reads element l + 1.  One ring row = the U box
+// (measured: anything else raises "illegal instruction" / "misaligned address"), and with ghost width 3 the interior
+// starts at the odd index 3, so a row is fetched as 34 doubles from i0 - (g & 1): lane l reads element l + (g & 1).  One ring row = the U box
 // [Nv][34] and the p, c, 1/rho box [3][34], each padded to 128 bytes; Gamma and chi_s (needed only at the two cells
 // next to a face) live in a second, shallower ring of [N + 1][34] boxes.
 constexpr int TMA_RW = 34;
 __host__ __device__ constexpr int tma_box_doubles(int nf) { return (nf * TMA_RW * 8 + 127) / 128 * 16; }
 __host__ __device__ constexpr int tma_deep_slot(int N) { return tma_box_doubles(N + 4) + tma_box_doubles(3); }
 __host__ __device__ constexpr int tma_shallow_slot(int N) { return tma_box_doubles(N + 1); }
-__host__ __device__ inline size_t yz_smem_doubles(int N, int W) {   // ring(s), flux buffer, two mbarriers
-  const size_t plain = (size_t)nstaged(N) * ring_rows(W) * 32;
-  const size_t tma = (size_t)ring_rows(W) * tma_deep_slot(N) + (size_t)(2 * W + 1) * tma_shallow_slot(N);
+__host__ __device__ inline size_t yz_smem_doubles(int N, int W, int S) {   // ring(s), flux buffer, two mbarriers
+  const size_t plain = (size_t)nstaged(N) * ring_rows(W, S) * 32;
+  const size_t tma = (size_t)ring_rows(W, S) * tma_deep_slot(N) + (size_t)(2 * W + 1) * tma_shallow_slot(N);
   return (plain > tma ? plain : tma) + (size_t)(N + 4) * (W + 1) * 32 + 4;
 }
 
@@ -354,11 +375,12 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
                    const XfEpilogue E, int *__restrict__ status, const int seg_len,
                    const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmP,
                    const __grid_constant__ CUtensorMap tmS) {
-  static_assert(W >= 3, "the service warps' ring-row hand-over needs W >= 3");
+  constexpr int S = stencil_cells(RECON), MA = S / 2 - 1;    // stencil cells per face; m of the cell below the face
+  static_assert(W > MA, "the service warps' ring-row hand-over needs W > S/2 - 1");
   const int N = N_T > 0 ? N_T : Nrt;
   const int Nv = N + 4, NST = nstaged(N);
   constexpr int NVS = N_T > 0 ? N_T + 4 : XF_MAXNV;        // static bound of Nv for register arrays
-  constexpr int RR = ring_rows(W);
+  constexpr int RR = ring_rows(W, S);
   // ring layout: TMA -> sm[slot][box][field][34] (see above), cp.async -> sm[field][slot][32]
   constexpr int RS = 2 * W + 1;                             // rows of the shallow ring (TMA only)
   const int FS = TMA ? TMA_RW : RR * 32;                    // doubles between fields
@@ -386,6 +408,7 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
   const bool service = threadIdx.y >= W;
   const int w = service ? threadIdx.y - W : threadIdx.y;    // face row within the chunk / ring row staged
   constexpr int OD = DIR == 1 ? 2 : 1;                      // the other transverse direction
+  const int lo = TMA ? (G.g[0] & 1) : 0;                    // TMA rows start at the even index below the strip's first cell
   const int i = G.g[0] + blockIdx.x * 32 + lane;
   const int imax = G.g[0] + G.n[0] - 1;
   const bool lane_ok = i <= imax;
@@ -401,29 +424,29 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
     unsigned phase = 0;
     bool bad = false, first = true;
     for (int fc = f_begin; fc <= f_end; fc += W) {
-      if (TMA) mbar_wait(full_bar + 8 * par, phase);        // rows fc .. fc + W + 4 are in the ring
+      if (TMA) mbar_wait(full_bar + 8 * par, phase);        // rows fc .. fc + W + S - 2 are in the ring
       else named_sync(BAR_RING_FULL + par, NT);
       const int f = fc + w;
-      int o[6];
+      int o[S];
 #pragma unroll
-      for (int m = 0; m < 6; ++m) {
+      for (int m = 0; m < S; ++m) {
         int sl = rb + w + m;
         sl -= sl >= RR ? RR : 0;
-        o[m] = sl * SLOT + lane + (TMA ? 1 : 0);
+        o[m] = sl * SLOT + lane + lo;
       }
-      int s2 = o[2], s3 = o[3];
-      if (TMA) {                                            // shallow ring: slot of stencil row r is (r - f_begin - 2) mod RS
+      int s2 = o[MA], s3 = o[MA + 1];
+      if (TMA) {                                            // shallow ring: slot of stencil row r is (r - f_begin - MA) mod RS
         int q2 = rs + w;
         q2 -= q2 >= RS ? RS : 0;
         int q3 = q2 + 1;
         q3 -= q3 >= RS ? RS : 0;
-        s2 = q2 * SSLOT + lane + 1;
-        s3 = q3 * SSLOT + lane + 1;
+        s2 = q2 * SSLOT + lane + lo;
+        s3 = q3 * SSLOT + lane + lo;
       }
       // the ring offsets are made opaque: otherwise the compiler, short of registers, re-derives every one of them
       // (wrap selects and multiplies, ~40 integer instructions per species field) instead of keeping six registers
 #pragma unroll
-      for (int m = 0; m < 6; ++m) asm volatile("" : "+r"(o[m]));
+      for (int m = 0; m < S; ++m) asm volatile("" : "+r"(o[m]));
       asm volatile("" : "+r"(s2), "+r"(s3));
       if (f <= f_end) {                                     // warp-uniform
         // fb_empty[c & 1] completes each time the service warps have read the fluxes of a chunk c - 1: for the
@@ -432,6 +455,8 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
         FluxStoreWS st{fb + (w + 1) * 32 + lane, FBS, first ? 0u : fbe_bar + 8 * par, par ? phase : phase ^ 1u};
         const bool c2ok = face_flux<DIR, RECON>(N, sm, smp, FS, o, sms, FS, s2, s3, E.visc, E.lam_glob + 3 * DIR, st);
         bad = bad || (!c2ok && lane_ok);
+        if (E.pp)                                           // Eq. 20 on this lane's own flux, before the hand-over
+          positivity_blend<DIR>(N, sm, smp, FS, o[MA], o[MA + 1], pp_kappa(E, G, DIR), fb + (w + 1) * 32 + lane, FBS);
       }
       named_arrive(BAR_FLUX_READY + par, NT);
       rb += W;
@@ -451,7 +476,7 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
   const int rmax = G.np[DIR] - 1;
   const unsigned deep_bytes = (unsigned)(Nv + 3) * TMA_RW * sizeof(double);
   const unsigned shallow_bytes = (unsigned)(N + 1) * TMA_RW * sizeof(double);
-  const int c0 = G.g[0] + blockIdx.x * 32 - 1, co = blockIdx.y + G.g[OD];      // TMA box origin (c0 is even)
+  const int c0 = G.g[0] + blockIdx.x * 32 - lo, co = blockIdx.y + G.g[OD];     // TMA box origin (c0 is even)
   auto stage_row = [&](int slot, int r, unsigned bar) {     // stencil row r (= padded row r) -> ring slot
     const int rc = r < rmax ? r : rmax;
     if (TMA) {                                              // boxes U [Nv][34] and p, c, 1/rho [3][34]
@@ -481,7 +506,7 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
   const bool need_acc = E.mode == 1 || (E.mode == 2 && E.has_acc);
   const bool need_un = (E.mode == 2 && E.alpha != 0.0) || E.mode == 3;
 
-  // cell row of face f (cell f - 1, staged at stencil row f + 2): Eq. 13 and the stage combination
+  // cell row of face f (cell f - 1, staged at stencil row f + MA): Eq. 13 and the stage combination
   double d[NVS];
   auto read_fluxes = [&](int ous) {                         // part 1: everything the update needs from shared memory
 #pragma unroll
@@ -504,14 +529,14 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
   double opnd[NVS];
   auto load_operands = [&](int f) {
     if (!need_opnd || !(f > f_begin && f <= f_end) || !lane_ok) return;
-    const long long gi = colbase + (long long)(f + 2) * sst;
+    const long long gi = colbase + (long long)(f + MA) * sst;
 #pragma unroll
     for (int v = 0; v < NVS; ++v)
       if (v < Nv) opnd[v] = opnd_src[v * G.cells + gi];
   };
   auto write_cells = [&](int f) {                           // part 2: Eq. 13 / Eq. 16 and the stores
     if (!(f > f_begin && f <= f_end) || !lane_ok) return;
-    const long long gi = colbase + (long long)(f + 2) * sst;
+    const long long gi = colbase + (long long)(f + MA) * sst;
 #pragma unroll
     for (int v = 0; v < NVS; ++v) {
       if (v < Nv) {
@@ -530,13 +555,13 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
     }
   };
 
-  // ---- prologue: rows f_begin .. f_begin + W + 4 into ring slots 0 .. W + 4
-  if (TMA) {                                                // shallow rows f_begin + 2 .. f_begin + W + 2 into slots 0 .. W
+  // ---- prologue: rows f_begin .. f_begin + W + S - 2 into ring slots 0 .. W + S - 2
+  if (TMA) {                                                // shallow rows f_begin + MA .. f_begin + MA + W into slots 0 .. W
     if (lane == 0)
-      mbar_expect_tx(full_bar, deep_bytes * (unsigned)((W + 5 - w + W - 1) / W) + shallow_bytes * (w == 0 ? 2u : 1u));
-    for (int r = w; r < W + 1; r += W) stage_shallow(r, f_begin + 2 + r, full_bar);
+      mbar_expect_tx(full_bar, deep_bytes * (unsigned)((W + S - 1 - w + W - 1) / W) + shallow_bytes * (w == 0 ? 2u : 1u));
+    for (int r = w; r < W + 1; r += W) stage_shallow(r, f_begin + MA + r, full_bar);
   }
-  for (int r = w; r < W + 5; r += W) stage_row(r, f_begin + r, full_bar);
+  for (int r = w; r < W + S - 1; r += W) stage_row(r, f_begin + r, full_bar);
   cp_async_commit();
 
   int rb = 0, rs = 0, par = 0;
@@ -554,29 +579,29 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
       __syncwarp();
       if (lane == 0) mbar_arrive(fbe_bar + 8 * par);
     }
-    if (fc + W <= f_end) {                                  // the W new rows of the next chunk: rows fc + W + 5 + q
-      // warp w fetches row q = (w + 2) mod W: it lands in the ring slot of the previous chunk's row q, and the only
-      // service warp that has just read U^s from that slot (stencil row f + 2 of its cell row) is warp q - 2 = w
-      // itself; rows 0 and 1 hold no cell of the previous chunk.  So no barrier among the service warps is needed.
-      const int q = w + 2 < W ? w + 2 : w + 2 - W;
-      int slot = rb + W + 5 + q;
+    if (fc + W <= f_end) {                                  // the W new rows of the next chunk: rows fc + W + S - 1 + q
+      // warp w fetches row q = (w + MA) mod W: it lands in the ring slot of the previous chunk's row q, and the only
+      // service warp that has just read U^s from that slot (stencil row f + MA of its cell row) is warp q - MA = w
+      // itself; rows 0 .. MA - 1 hold no cell of the previous chunk.  So no barrier among the service warps is needed.
+      const int q = w + MA < W ? w + MA : w + MA - W;
+      int slot = rb + W + S - 1 + q;
       slot -= slot >= RR ? RR : 0;
       const unsigned bar = full_bar + 8 * (par ^ 1);
       if (TMA && lane == 0) mbar_expect_tx(bar, deep_bytes + shallow_bytes);
-      stage_row(slot, fc + W + 5 + q, bar);
-      if (TMA) {                                            // shallow row fc + W + 3 + w
+      stage_row(slot, fc + W + S - 1 + q, bar);
+      if (TMA) {                                            // shallow row fc + W + MA + 1 + w
         int q = rs + W + 1 + w;
         q -= q >= RS ? RS : 0;
-        stage_shallow(q, fc + W + 3 + w, bar);
+        stage_shallow(q, fc + W + MA + 1 + w, bar);
       }
     }
     cp_async_commit();
     if (!first) write_cells(fprev);
     fprev = fc + w;
-    {                                                       // where U^s of that cell row (stencil row f + 2) sits
-      int sl = rb + w + 2;
+    {                                                       // where U^s of that cell row (stencil row f + MA) sits
+      int sl = rb + w + MA;
       sl -= sl >= RR ? RR : 0;
-      ous = sl * SLOT + lane + (TMA ? 1 : 0);
+      ous = sl * SLOT + lane + lo;
     }
     rb += W;
     rb -= rb >= RR ? RR : 0;
@@ -601,7 +626,7 @@ sweep_yz_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, 
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int XW_W = 4;                    // compute warps = service warps per block
 constexpr int XW_CH = XW_W * 32;           // faces per chunk
-constexpr int XW_BOX = XW_CH + 8;          // cells per box: 133 needed, from an even index, 16-byte multiple
+constexpr int XW_BOX = XW_CH + 8;          // cells per box: 128 + S - 1 (133 or 135) needed, from an even index, 16-byte multiple
 constexpr int XW_NCH = 16;                 // chunks per block
 constexpr int XW_FBW = XW_CH + 2;          // flux-buffer doubles per component: [0] = last face of the previous chunk
 __host__ __device__ constexpr int xw_box_doubles(int nf) { return (nf * XW_BOX * 8 + 127) / 128 * 16; }
@@ -624,6 +649,8 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
                   int *__restrict__ status, const int segs_per_plane, const __grid_constant__ CUtensorMap tmU,
                   const __grid_constant__ CUtensorMap tmP, const __grid_constant__ CUtensorMap tmS) {
   constexpr int W = XW_W, NT = 64 * W, FS = XW_BOX;
+  constexpr int S = stencil_cells(RECON), HW = S / 2, MA = S / 2 - 1;
+  static_assert(XW_CH + S - 1 + 1 <= XW_BOX, "a chunk's stencil cells (+ one for the even start) fit the box");
   const int N = N_T > 0 ? N_T : Nrt;
   const int Nv = N + 4;
   constexpr int NVS = N_T > 0 ? N_T + 4 : XF_MAXNV;
@@ -650,8 +677,8 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
   const int f_begin = seg * SEGC;                           // faces f_begin .. f_end, cells f_begin .. f_end - 1
   const int f_end = f_begin + SEGC < L ? f_begin + SEGC : L;
   const long long P0 = (long long)(plane + G.g[2]) * G.st[2] + (long long)G.g[1] * G.st[1];  // flat cell 0
-  // chunk c needs flat cells fc - 3 .. fc + 130; its boxes start at the even global index below P0 + fc - 3
-  const long long g0 = P0 + f_begin - 3;
+  // chunk c needs flat cells fc - HW .. fc + 127 + HW; its boxes start at the even global index below P0 + fc - HW
+  const long long g0 = P0 + f_begin - HW;
   const int delta = (int)(g0 & 1);                          // same for every chunk: they are 128 cells apart
   const int u = 32 * w + lane;                              // face within the chunk (compute) / cell slot (service)
 
@@ -665,12 +692,13 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
       mbar_wait(full_bar + 8 * par, phase);
       const double *st = smem + (size_t)par * STAGE;
       const int f = fc + u;
-      int o[6];
+      int o[S];
 #pragma unroll
-      for (int m = 0; m < 6; ++m) o[m] = u + delta + m;
+      for (int m = 0; m < S; ++m) o[m] = u + delta + m;
       // every lane of the block passes the same barriers; lanes past f_end compute on staged (valid or zero) data
       FluxStoreWS fsw{fb + u + 1, XW_FBW, first ? 0u : fbe_bar + 8 * par, par ? phase : phase ^ 1u};
-      const bool c2ok = face_flux<0, RECON>(N, st, st + OFFP, FS, o, st + OFFS, FS, o[2], o[3], E.visc, E.lam_glob, fsw);
+      const bool c2ok = face_flux<0, RECON>(N, st, st + OFFP, FS, o, st + OFFS, FS, o[MA], o[MA + 1], E.visc, E.lam_glob, fsw);
+      if (E.pp) positivity_blend<0>(N, st, st + OFFP, FS, o[MA], o[MA + 1], pp_kappa(E, G, 0), fb + u + 1, XW_FBW);
       {
         const int ia = (f - 1 + G.np[0]) % G.np[0], ib = f % G.np[0];
         const bool used = f <= f_end && ((ia >= G.g[0] && ia < G.g[0] + G.n[0]) || (ib >= G.g[0] && ib < G.g[0] + G.n[0]));
@@ -691,7 +719,7 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
     if (w != 0 || lane != 0) return;
     const unsigned bar = full_bar + 8 * st;
     const unsigned dst = (unsigned)__cvta_generic_to_shared(smem + (size_t)st * STAGE);
-    const int c0 = (int)(P0 + fc - 3 - delta);              // even; may be negative or run past the array: zero-filled
+    const int c0 = (int)(P0 + fc - HW - delta);             // even; may be negative or run past the array: zero-filled
     mbar_expect_tx(bar, stage_bytes);
     tma_load_span(dst, &tmU, c0, bar);
     tma_load_span(dst + (unsigned)(OFFP * sizeof(double)), &tmP, c0, bar);
@@ -706,7 +734,7 @@ sweep_x_ws_kernel(const XfGrid G, const int Nrt, const double *__restrict__ U, c
   // lane (w, lane) of the service group owns slot u of a chunk: cell fc + u - 1, between the chunk's faces u - 1 and u
   double d[NVS];
   auto read_fluxes = [&](int st) {                          // st: stage of the chunk whose cells are updated
-    const double *us = smem + (size_t)st * STAGE + u + delta + 2;   // cell fc + u - 1 = stencil cell m = 2 of face fc + u
+    const double *us = smem + (size_t)st * STAGE + u + delta + MA;  // cell fc + u - 1 = stencil cell m = MA of face fc + u
 #pragma unroll
     for (int v = 0; v < NVS; ++v) {
       if (v < Nv) {

@@ -238,10 +238,12 @@ def _finish(name, nx, ny, nz, dx, dy, dz, table, bc, Uint, Tint, rng, bc_state=N
 # ----------------------------------------------------------------------------------------------------------------
 # config 1: 1-D two-species shock tube
 # ----------------------------------------------------------------------------------------------------------------
-def config1_shock_tube(nx: int = 400, axis: int = 0, seed: Optional[int] = None) -> Workload:
+def config1_shock_tube(nx: int = 400, axis: int = 0, seed: Optional[int] = None, y_floor: float = 0.0) -> Workload:
     """BASELINE.json configs[0]; shape of the paper's inert shock tube.
 
-    ``axis`` lays the tube along x (0), y (1) or z (2) -- used by direction-consistency tests.
+    ``axis`` lays the tube along x (0), y (1) or z (2) -- used by direction-consistency tests.  ``y_floor`` > 0 keeps both
+    mass fractions inside [y_floor, 1 - y_floor] (the role of zeta in the paper's Eq. 32): without it
+    the tanh tails hold cells with Y ~ 1e-16, where the positivity limiter's decision rests on round-off.
     """
     rng = np.random.default_rng(SEED_BASE + 1 if seed is None else seed)
     table = calorically_perfect_table(W=(28.0, 4.0), gamma=(1.4, 5.0 / 3.0), Ru=1.0)
@@ -251,6 +253,8 @@ def config1_shock_tube(nx: int = 400, axis: int = 0, seed: Optional[int] = None)
     rho = np.where(left, 1.0, 0.125)
     p = np.where(left, 1.0, 0.1)
     YA = 0.5 * (1.0 - np.tanh((x - 0.5) / (2.0 * dx)))
+    if y_floor > 0.0:
+        YA = np.clip(YA, y_floor, 1.0 - y_floor)
     Y = np.stack([YA, 1.0 - YA])
     rho = rho * (1.0 + 1e-3 * rng.uniform(-1.0, 1.0, nx))
     T = p / (rho * table.mixture_R(Y))
@@ -605,4 +609,26 @@ def random_smooth_box(nx: int, ny: int, nz: int, nspecies: int, seed: int, bc=(B
     if BC_DIRICHLET in bc:
         bc_state = np.tile(Ui.reshape(nspecies + 4, -1)[:, :1].T, (6, 1))
     return _finish(f"random_smooth_{nx}x{ny}x{nz}_{nspecies}sp", nx, ny, nz, d[0], d[1], d[2], table, bc, Ui, T, rng,
+                   bc_state=bc_state)
+
+
+def rough_box(nx: int, ny: int, nz: int, nspecies: int = 4, seed: int = 3, bc=(BC_PERIODIC,) * 6) -> Workload:
+    """Cell-to-cell random composition (species 1 absent from 30 % of the cells), density and temperature with moderate
+    velocities: the unlimited scheme undershoots Y by several per cent here, so this is the input on which the
+    positivity-preserving flux blending is active at many faces."""
+    rng = np.random.default_rng(seed)
+    table = synthetic_nasa7_table(rng.uniform(2, 60, nspecies), Ru=0.1, rng=rng, formation=True)
+    shape = (nz, ny, nx)
+    Y = rng.standard_gamma(0.3, (nspecies,) + shape)
+    Y /= Y.sum(axis=0)
+    Y[0][rng.uniform(size=shape) < 0.3] = 0.0
+    Y /= Y.sum(axis=0)
+    rho = 10 ** rng.uniform(-0.5, 0.5, shape)
+    T = 10 ** rng.uniform(2.5, 3.2, shape)
+    c = np.sqrt(table.frozen_gamma(Y, T) * table.mixture_R(Y) * T)
+    u = [rng.uniform(-0.5, 0.5, shape) * c if m > 1 else np.zeros(shape) for m in (nx, ny, nz)]
+    Ui = conserved_from_primitive(table, rho, u[0], u[1], u[2], T, Y)
+    d = [1.0 / m if m > 1 else 1.0 for m in (nx, ny, nz)]
+    bc_state = np.tile(Ui.reshape(nspecies + 4, -1)[:, :1].T, (6, 1)) if BC_DIRICHLET in bc else None
+    return _finish(f"rough_{nx}x{ny}x{nz}_{nspecies}sp", nx, ny, nz, d[0], d[1], d[2], table, bc, Ui, T, rng,
                    bc_state=bc_state)

@@ -19,14 +19,14 @@ LIB_PATH = _HERE / "libxf.so"
 XF_OK, XF_EINVAL, XF_ECUDA, XF_ENOMEM, XF_ENONPHYSICAL, XF_ENOCONV = 0, -1, -2, -3, -4, -5
 XF_BC_PERIODIC, XF_BC_TRANSMISSIVE, XF_BC_REFLECTIVE, XF_BC_DIRICHLET = 0, 1, 2, 3
 XF_VISC_LLF, XF_VISC_ROE, XF_VISC_GLF = 0, 1, 2
-XF_RECON_WENO5, XF_RECON_WENOCU6 = 0, 1
+XF_RECON_WENO5, XF_RECON_WENOCU6, XF_RECON_WENO7 = 0, 1, 2
 XF_MAX_SPECIES = 16
 
 # every symbol include/xf.h declares (tests check that the library exports all of them)
 ABI_SYMBOLS = (
     "xf_create", "xf_destroy", "xf_num_vars", "xf_padded_cells", "xf_rhs_workspace_bytes", "xf_workspace_bytes",
     "xf_fill_ghosts", "xf_primitives", "xf_convective_rhs", "xf_rk3_step", "xf_rk3_step_cfl", "xf_step_cfl",
-    "xf_max_wavespeed",
+    "xf_max_wavespeed", "xf_set_rhs_dt",
     "xf_status", "xf_newton_mean_iterations", "xf_launch_count", "xf_convective_rhs_host", "xf_rk3_steps_host",
     "xf_probe_fp64_peak", "xf_strerror", "xf_timing_enable", "xf_timing_read",
 )
@@ -42,6 +42,7 @@ class XfConfig(C.Structure):
         ("Tlo", C.c_double), ("Thi", C.c_double),
         ("bc", C.c_int * 6), ("bc_state", C.POINTER(C.c_double)),
         ("newton_rtol", C.c_double), ("newton_maxit", C.c_int), ("device", C.c_int), ("viscosity", C.c_int), ("reconstruction", C.c_int),
+        ("positivity", C.c_int),
     ]
 
 
@@ -71,6 +72,7 @@ def lib() -> C.CDLL:
         L.xf_fill_ghosts.argtypes = [ctx, dp, vp]
         L.xf_primitives.argtypes = [ctx, dp, dp, dp, dp, vp]
         L.xf_convective_rhs.argtypes = [ctx, dp, dp, dp, vp, vp]
+        L.xf_set_rhs_dt.argtypes = [ctx, C.c_double]
         L.xf_rk3_step.argtypes = [ctx, dp, dp, C.c_double, vp, vp]
         L.xf_rk3_step_cfl.argtypes = [ctx, dp, dp, C.c_double, dp, vp, vp]
         L.xf_step_cfl.argtypes = [ctx, dp, dp, C.c_double, dp, vp, vp]
@@ -133,13 +135,15 @@ class Context:
 
     def __init__(self, nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, W: Sequence[float], nasa7, Ru: float,
                  Tlo: float, Thi: float, bc=(0,) * 6, bc_state=None, newton_rtol: float = 0.0, newton_maxit: int = 0,
-                 device: int = 0, viscosity: int = XF_VISC_LLF, reconstruction: int = XF_RECON_WENO5):
+                 device: int = 0, viscosity: int = XF_VISC_LLF, reconstruction: int = XF_RECON_WENO5,
+                 positivity: bool = False, ng: Optional[int] = None):
         W = np.ascontiguousarray(W, dtype=np.float64)
         nasa7 = np.ascontiguousarray(nasa7, dtype=np.float64)
         n = int(W.shape[0])
         assert nasa7.shape == (n, 7)
         cfg = XfConfig()
-        cfg.nx, cfg.ny, cfg.nz, cfg.ng = int(nx), int(ny), int(nz), 3
+        ng = (4 if int(reconstruction) == XF_RECON_WENO7 else 3) if ng is None else int(ng)
+        cfg.nx, cfg.ny, cfg.nz, cfg.ng = int(nx), int(ny), int(nz), ng
         cfg.dx, cfg.dy, cfg.dz = float(dx), float(dy), float(dz)
         cfg.nspecies, cfg.Ru = n, float(Ru)
         cfg.W = W.ctypes.data_as(C.POINTER(C.c_double))
@@ -155,12 +159,14 @@ class Context:
         cfg.newton_rtol, cfg.newton_maxit, cfg.device = float(newton_rtol), int(newton_maxit), int(device)
         cfg.viscosity = int(viscosity)
         cfg.reconstruction = int(reconstruction)
+        cfg.positivity = int(bool(positivity))
         self._h = C.c_void_p()
         _check(lib().xf_create(C.byref(self._h), C.byref(cfg)), "xf_create")
         self.device = int(device)
         self.N, self.Nv = n, n + 4
         self.cells = int(lib().xf_padded_cells(self._h))
-        self.shape = (nz + 6 if nz > 1 else 1, ny + 6 if ny > 1 else 1, nx + 6 if nx > 1 else 1)
+        self.ng = ng
+        self.shape = tuple(m + 2 * ng if m > 1 else 1 for m in (nz, ny, nx))
         self.interior_cells = int(nx) * int(ny) * int(nz)
         self.rhs_workspace_bytes = int(lib().xf_rhs_workspace_bytes(self._h))
         self.workspace_bytes = int(lib().xf_workspace_bytes(self._h))
@@ -168,6 +174,7 @@ class Context:
     @classmethod
     def from_workload(cls, wl, **kw) -> "Context":
         t = wl.table
+        kw.setdefault("ng", getattr(wl, "ng", 3))
         return cls(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, t.W, t.nasa7, t.Ru, t.Tlo, t.Thi, wl.bc, wl.bc_state, **kw)
 
     def close(self) -> None:
@@ -208,6 +215,9 @@ class Context:
         assert work.numel() * work.element_size() >= self.rhs_workspace_bytes
         _check(lib().xf_convective_rhs(self._h, _ptr(U), _ptr(T), _ptr(rhs), _ptr(work), _stream(stream)),
                "xf_convective_rhs")
+
+    def xf_set_rhs_dt(self, dt: float) -> None:
+        _check(lib().xf_set_rhs_dt(self._h, float(dt)), "xf_set_rhs_dt")
 
     def xf_rk3_step(self, U, T, dt: float, work, stream=None) -> None:
         assert work.numel() * work.element_size() >= self.workspace_bytes

@@ -93,22 +93,7 @@ def test_one_face_blend_written_out(oracle_mod, d):
 
 
 def _rough(nx, ny, nz, n=4, seed=3):
-    """random cell-to-cell composition (one species absent from 30 % of the cells), density and temperature; moderate
-    velocities: the unlimited scheme undershoots Y by several per cent here"""
-    rng = np.random.default_rng(seed)
-    table = wl.synthetic_nasa7_table(rng.uniform(2, 60, n), Ru=0.1, rng=rng, formation=True)
-    shape = (nz, ny, nx)
-    Y = rng.standard_gamma(0.3, (n,) + shape)
-    Y /= Y.sum(axis=0)
-    Y[0][rng.uniform(size=shape) < 0.3] = 0.0
-    Y /= Y.sum(axis=0)
-    rho = 10 ** rng.uniform(-0.5, 0.5, shape)
-    T = 10 ** rng.uniform(2.5, 3.2, shape)
-    c = np.sqrt(table.frozen_gamma(Y, T) * table.mixture_R(Y) * T)
-    u = [rng.uniform(-0.5, 0.5, shape) * c if m > 1 else np.zeros(shape) for m in (nx, ny, nz)]
-    Ui = wl.conserved_from_primitive(table, rho, u[0], u[1], u[2], T, Y)
-    d = [1.0 / m if m > 1 else 1.0 for m in (nx, ny, nz)]
-    return wl._finish("rough", nx, ny, nz, d[0], d[1], d[2], table, (0,) * 6, Ui, T, rng)
+    return wl.rough_box(nx, ny, nz, nspecies=n, seed=seed)
 
 
 @pytest.mark.parametrize("dims", [(40, 1, 1), (14, 12, 1), (12, 10, 8)])

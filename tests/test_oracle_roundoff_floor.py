@@ -9,12 +9,8 @@ than 1e-12 of the row's own scale on such rows, and by < 2e-13 on the scale DESI
 max(own scale, max Y_s x density-row scale) -- the scale tests/test_gpu_parity.py uses at full size.
 
 The long-double library is produced from oracle/xf_oracle.c by text substitution (double -> long double, libm calls and
-literals suffixed); nothing of the CUDA path is involved.
+literals suffixed; fixture `oracle_ld` of tests/conftest.py); nothing of the CUDA path is involved.
 """
-import ctypes as C
-import re
-import subprocess
-
 import numpy as np
 import pytest
 
@@ -23,62 +19,6 @@ from paper_2403_05910_b200 import workloads as wl
 LD = np.longdouble
 pytestmark = pytest.mark.skipif(np.finfo(LD).eps >= np.finfo(np.float64).eps,
                                 reason="no extended-precision long double on this platform")
-MAXN, MAXNV = 16, 20
-
-
-@pytest.fixture(scope="module")
-def oracle_ld(tmp_path_factory, oracle_mod):
-    import oracle
-
-    src_dir = __import__("pathlib").Path(oracle.__file__).resolve().parent
-    out = tmp_path_factory.mktemp("oracle_ld")
-    lit = re.compile(r"(?<![\w.])(\d+\.\d*(?:[eE][-+]?\d+)?|\d+[eE][-+]?\d+)(?![\w.])")
-    for name in ("xf_oracle.c", "xf_oracle.h"):
-        t = (src_dir / name).read_text()
-        t = re.sub(r"\bdouble\b", "long double", t)
-        for f in ("sqrt", "fabs", "fmax"):
-            t = re.sub(rf"\b{f}\(", f"{f}l(", t)
-        t = lit.sub(r"\1L", t)
-        (out / name).write_text(t)
-    so = out / "libxf_oracle_ld.so"
-    subprocess.run(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-o", str(so),
-                    str(out / "xf_oracle.c"), "-lm"], check=True)
-    ld = C.c_longdouble
-
-    class Cfg(C.Structure):
-        _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("ng", C.c_int),
-                    ("dx", ld), ("dy", ld), ("dz", ld), ("N", C.c_int), ("Ru", ld),
-                    ("W", ld * MAXN), ("a", (ld * 7) * MAXN), ("Tlo", ld), ("Thi", ld),
-                    ("bc", C.c_int * 6), ("bc_state", (ld * MAXNV) * 6),
-                    ("rtol", ld), ("maxit", C.c_int), ("ideal_weights", C.c_int), ("viscosity", C.c_int),
-                    ("lam_glob", (ld * 3) * 3), ("recon", C.c_int)]
-
-    lib = C.CDLL(str(so))
-    lib.xo_rhs_cells.argtypes = [C.POINTER(Cfg), C.c_void_p, C.c_void_p, C.c_long, C.c_void_p, C.c_void_p]
-
-    def rhs_cells(w, U_filled, Tguess, idx):
-        """long-double rhs at the sampled cells; the INPUTS are the doubles of the fp64 run, converted exactly"""
-        cfg = Cfg()
-        cfg.nx, cfg.ny, cfg.nz, cfg.ng = w.nx, w.ny, w.nz, 3
-        cfg.dx, cfg.dy, cfg.dz = w.dx, w.dy, w.dz
-        t = w.table
-        cfg.N, cfg.Ru = t.n, t.Ru
-        for s in range(t.n):
-            cfg.W[s] = t.W[s]
-            for q in range(7):
-                cfg.a[s][q] = t.nasa7[s, q]
-        cfg.Tlo, cfg.Thi = t.Tlo, t.Thi
-        cfg.rtol, cfg.maxit = 1e-17, 60
-        Ul = np.ascontiguousarray(U_filled, dtype=LD)
-        Tl = np.ascontiguousarray(Tguess, dtype=LD)
-        idx = np.ascontiguousarray(idx, dtype=np.int64)
-        outl = np.zeros((idx.shape[0], t.n + 4), dtype=LD)
-        st = lib.xo_rhs_cells(C.byref(cfg), Ul.ctypes.data, Tl.ctypes.data, idx.shape[0], idx.ctypes.data,
-                              outl.ctypes.data)
-        assert st in (0, 5)          # rtol 1e-17 is below what even 80 bits resolve: "not converged" means "to round-off"
-        return outl
-
-    return rhs_cells
 
 
 def _samples(w, rng, n_rand, x_bands):
