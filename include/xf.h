@@ -174,6 +174,9 @@ int xf_rk3_steps_host(xf_ctx *ctx, double *U_host, double *T_host, double cfl, i
 /* Measurement aid for the roofline denominator: runs a register-resident chain of dependent-free fp64 FMAs on
  * every SM for `iters` rounds and returns the achieved TFLOP/s (2 flops per FMA) in *tflops.  Synchronous. */
 int xf_probe_fp64_peak(int device, int iters, double *tflops, double *ms);
+/* The same probe launched back to back for at least `seconds` (<= 30): the SUSTAINED figure, at the clocks the GPU
+ * holds under a long fp64 load (the burst figure above is the best of five short launches). *ms = the timed span. */
+int xf_probe_fp64_sustained(int device, double seconds, double *tflops, double *ms);
 
 const char *xf_strerror(int code);
 

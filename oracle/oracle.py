@@ -28,6 +28,25 @@ class OConfig(C.Structure):
     ]
 
 
+class OTransport(C.Structure):
+    _fields_ = [("mu", (C.c_double * 4) * MAXN), ("kappa", (C.c_double * 4) * MAXN),
+                ("D", ((C.c_double * 4) * MAXN) * MAXN), ("p_ref", C.c_double)]
+
+
+def make_transport(tr) -> OTransport:
+    """tr: an object with mu[N,4], kappa[N,4], D[N,N,4], p_ref (workloads.TransportFits)."""
+    o = OTransport()
+    n = tr.mu.shape[0]
+    for s in range(n):
+        for q in range(4):
+            o.mu[s][q] = tr.mu[s, q]
+            o.kappa[s][q] = tr.kappa[s, q]
+            for t in range(n):
+                o.D[s][t][q] = tr.D[s, t, q]
+    o.p_ref = float(tr.p_ref)
+    return o
+
+
 class OPrim(C.Structure):
     _fields_ = [
         ("rho", C.c_double), ("vel", C.c_double * 3), ("Y", C.c_double * MAXN), ("e", C.c_double),
@@ -92,6 +111,14 @@ def lib():
         L.xo_rk3_step.argtypes = [cp, dp, dp, C.c_double]
         L.xo_max_wavespeed.argtypes = [cp, dp, dp, C.POINTER(C.c_int)]
         L.xo_max_wavespeed.restype = C.c_double
+        tp = C.POINTER(OTransport)
+        L.xo_transport_cell.argtypes = [cp, tp, C.c_double, dp, C.c_double, dp, dp, dp, dp]
+        L.xo_transport_cell.restype = None
+        L.xo_viscous_face_flux.argtypes = [cp, tp, dp, dp, C.c_long, C.c_int, dp, dp]
+        L.xo_viscous_face_flux.restype = None
+        L.xo_viscous_rhs.argtypes = [cp, tp, dp, dp, dp]
+        L.xo_rhs_ns.argtypes = [cp, tp, dp, dp, dp]
+        L.xo_rk3_step_ns.argtypes = [cp, tp, dp, dp, C.c_double]
         _lib = L
     return _lib
 
@@ -257,6 +284,40 @@ class Oracle:
     def rk3_step(self, U, T, dt: float) -> int:
         self._chk(U, T)
         return lib().xo_rk3_step(C.byref(self.cfg), _dp(U), _dp(T), float(dt))
+
+    # ---- viscous / diffusive terms (xf_oracle.h: readings R19-R23); tr = make_transport(workloads.TransportFits) ----
+    def transport_cell(self, tr: OTransport, rho: float, Y, T: float):
+        """-> (mu, kappa, rho D_sm [N], h_s [N])"""
+        Y = np.ascontiguousarray(Y, dtype=np.float64)
+        mu, ka = C.c_double(), C.c_double()
+        rD, h = np.zeros(self.N), np.zeros(self.N)
+        lib().xo_transport_cell(C.byref(self.cfg), C.byref(tr), float(rho), _dp(Y), float(T), C.byref(mu), C.byref(ka),
+                                _dp(rD), _dp(h))
+        return mu.value, ka.value, rD, h
+
+    def viscous_face_flux(self, tr: OTransport, U, T, ia: int, d: int):
+        """-> (F_v [Nv] at the face above padded cell ia in direction d, J_s.n [N])"""
+        self._chk(U, T)
+        F, J = np.zeros(self.Nv), np.zeros(self.N)
+        lib().xo_viscous_face_flux(C.byref(self.cfg), C.byref(tr), _dp(U), _dp(T), int(ia), int(d), _dp(F), _dp(J))
+        return F, J
+
+    def viscous_rhs(self, tr: OTransport, U, T) -> np.ndarray:
+        """div F_v at interior cells from ghost-filled U and the converged T of every padded cell"""
+        self._chk(U, T)
+        out = np.zeros_like(U)
+        lib().xo_viscous_rhs(C.byref(self.cfg), C.byref(tr), _dp(U), _dp(T), _dp(out))
+        return out
+
+    def rhs_ns(self, tr: OTransport, U, T) -> np.ndarray:
+        self._chk(U, T)
+        out = np.zeros_like(U)
+        self.last_status = lib().xo_rhs_ns(C.byref(self.cfg), C.byref(tr), _dp(U), _dp(T), _dp(out))
+        return out
+
+    def rk3_step_ns(self, tr: OTransport, U, T, dt: float) -> int:
+        self._chk(U, T)
+        return lib().xo_rk3_step_ns(C.byref(self.cfg), C.byref(tr), _dp(U), _dp(T), float(dt))
 
     def max_wavespeed(self, U, T) -> float:
         self._chk(U, T)

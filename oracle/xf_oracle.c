@@ -648,7 +648,199 @@ int xo_rhs_cells(const xo_config *c_in, const double *U, const double *Tguess, l
 /* ------------------------------------------------------------------------------------------------------------ */
 /* SSP-RK3 (Eq. 16); ghosts + primitives before each of the three residuals     */
 /* ------------------------------------------------------------------------------------------------------------ */
-int xo_rk3_step(const xo_config *c_in, double *U, double *T, double dt) {
+/* ------------------------------------------------------------------------------------------------------------ */
+/* Viscous / diffusive right-hand side (Eq. 1-6; 155-178 Eq. 22, 26; 505-513 Eq. 29; readings R19-R23) */
+/* ------------------------------------------------------------------------------------------------------------ */
+static double fit_eval(const double a[4], double lnT) {           /* Eq. 29: ln eta = sum_n a_n (ln T)^n */
+  return exp(a[0] + lnT * (a[1] + lnT * (a[2] + lnT * a[3])));
+}
+
+void xo_transport_cell(const xo_config *c, const xo_transport *tr, double rho, const double *Y, double T, double *mu,
+                       double *kappa, double *rhoD, double *h) {
+  const int N = c->N;
+  const double lnT = log(T);
+  double X[XO_MAXN], ms[XO_MAXN], ks[XO_MAXN];
+  double sum = 0.0, Rbar = 0.0;
+  for (int s = 0; s < N; ++s) sum += Y[s] / c->W[s];
+  for (int s = 0; s < N; ++s) {
+    X[s] = (Y[s] / c->W[s]) / sum;                                /* mole fractions */
+    ms[s] = fit_eval(tr->mu[s], lnT);
+    ks[s] = fit_eval(tr->kappa[s], lnT);
+    Rbar += Y[s] * (c->Ru / c->W[s]);
+    double cp, es;
+    xo_species_thermo(c, s, T, &cp, &h[s], &es);
+  }
+  const double p = rho * Rbar * T;                                /* Eq. 7 */
+  /* Eq. 22 (Wilke), for mu and for kappa with the ratio of the respective property */
+  double m = 0.0, k = 0.0;
+  for (int s = 0; s < N; ++s) {
+    double dm = 0.0, dk = 0.0;
+    for (int t = 0; t < N; ++t) {
+      const double w = 1.0 / sqrt(8.0) / sqrt(1.0 + c->W[s] / c->W[t]);
+      const double q4 = sqrt(sqrt(c->W[t] / c->W[s]));
+      const double bm = 1.0 + sqrt(ms[s] / ms[t]) * q4, bk = 1.0 + sqrt(ks[s] / ks[t]) * q4;
+      dm += X[t] * w * bm * bm;
+      dk += X[t] * w * bk * bk;
+    }
+    m += X[s] * ms[s] / dm;
+    k += X[s] * ks[s] / dk;
+  }
+  *mu = m;
+  *kappa = k;
+  /* Eq. 26 with X_t + 1e-12 (reading R20); D_st(T, p) = D_st(T, p_ref) p_ref / p (reading R19) */
+  double Wbar = 0.0;
+  for (int s = 0; s < N; ++s) Wbar += X[s] * c->W[s];
+  for (int s = 0; s < N; ++s) {
+    double num = 0.0, den = 0.0;
+    for (int t = 0; t < N; ++t) {
+      if (t == s) continue;
+      const double Dst = fit_eval(tr->D[s][t], lnT) * tr->p_ref / p;
+      num += (X[t] + 1e-12) * c->W[t];
+      den += (X[t] + 1e-12) / Dst;
+    }
+    rhoD[s] = N > 1 ? rho * num / (Wbar * den) : 0.0;
+  }
+}
+
+typedef struct { double u[3], T, Y[XO_MAXN], h[XO_MAXN], mu, kappa, rD[XO_MAXN]; } vcell;
+
+static void vcell_at(const xo_config *c, const xo_transport *tr, const double *U, const double *T, long cells, long id,
+                     vcell *V) {
+  const int N = c->N;
+  const double rho = U[id];
+  for (int q = 0; q < 3; ++q) V->u[q] = U[(1 + q) * cells + id] / rho;
+  double sum = 0.0;
+  for (int i = 0; i < N - 1; ++i) {
+    V->Y[i] = U[(5 + i) * cells + id] / rho;
+    sum += V->Y[i];
+  }
+  V->Y[N - 1] = 1.0 - sum;
+  V->T = T[id];
+  xo_transport_cell(c, tr, rho, V->Y, V->T, &V->mu, &V->kappa, V->rD, V->h);
+}
+
+static double interp4(double m1, double a, double b, double p2) { return (9.0 * (a + b) - (m1 + p2)) / 16.0; }
+static double dnorm4(double m1, double a, double b, double p2, double dx) { return (27.0 * (b - a) - (p2 - m1)) / (24.0 * dx); }
+static double dctr4(double mm, double m, double p, double pp, double dx) { return (mm - 8.0 * m + 8.0 * p - pp) / (12.0 * dx); }
+
+/* face above padded cell ia in direction d, from the per-cell table V (all padded cells) */
+static void vface(const xo_config *c, const vcell *V, const long st[3], const int n[3], long ia, int d, double *F,
+                  double *J_out) {
+  const int N = c->N, Nv = N + 4;
+  const double dxs[3] = {c->dx, c->dy, c->dz};
+  const vcell *q[4];
+  for (int k = 0; k < 4; ++k) q[k] = V + ia + (long)(k - 1) * st[d];
+#define FACE(field) interp4(q[0]->field, q[1]->field, q[2]->field, q[3]->field)
+#define DN(field) dnorm4(q[0]->field, q[1]->field, q[2]->field, q[3]->field, dxs[d])
+  double G[3][3];                                                 /* G[p][e] = d u_p / d x_e at the face */
+  for (int p = 0; p < 3; ++p)
+    for (int e = 0; e < 3; ++e) {
+      if (e == d) G[p][e] = DN(u[p]);
+      else if (n[e] == 1) G[p][e] = 0.0;
+      else {
+        double t[4];
+        for (int k = 0; k < 4; ++k) {
+          const vcell *z = q[k];
+          t[k] = dctr4((z - 2 * st[e])->u[p], (z - st[e])->u[p], (z + st[e])->u[p], (z + 2 * st[e])->u[p], dxs[e]);
+        }
+        G[p][e] = interp4(t[0], t[1], t[2], t[3]);
+      }
+    }
+  const double mu = FACE(mu), kappa = FACE(kappa);
+  const double div = G[0][0] + G[1][1] + G[2][2];
+  double tau[3];                                                  /* tau_{p d}, Eq. 3 */
+  for (int p = 0; p < 3; ++p) tau[p] = mu * (G[p][d] + G[d][p]) - (p == d ? 2.0 / 3.0 * mu * div : 0.0);
+  double J[XO_MAXN], dY[XO_MAXN], corr = 0.0;
+  for (int s = 0; s < N; ++s) {
+    dY[s] = DN(Y[s]);
+    corr += FACE(rD[s]) * dY[s];
+  }
+  double qd = 0.0;
+  for (int s = 0; s < N; ++s) {                                   /* Eq. 6 (reading R21), Eq. 5 */
+    J[s] = -(FACE(rD[s]) * dY[s] - FACE(Y[s]) * corr);
+    qd += FACE(h[s]) * J[s];
+  }
+  for (int v = 0; v < Nv; ++v) F[v] = 0.0;
+  double work = 0.0;
+  for (int p = 0; p < 3; ++p) {
+    F[1 + p] = tau[p];
+    work += tau[p] * FACE(u[p]);
+  }
+  F[4] = work + kappa * DN(T) - qd;                               /* tau.u - q_c - q_d, q_c = -kappa grad T (Eq. 4) */
+  for (int s = 0; s < N - 1; ++s) F[5 + s] = -J[s];
+  if (J_out) for (int s = 0; s < N; ++s) J_out[s] = J[s];
+#undef FACE
+#undef DN
+}
+
+static vcell *vcell_table(const xo_config *c, const xo_transport *tr, const double *U, const double *T) {
+  const long cells = xo_padded_cells(c);
+  vcell *V = (vcell *)malloc(sizeof(vcell) * cells);
+#pragma omp parallel for schedule(static) if (cells > 16384)
+  for (long id = 0; id < cells; ++id) vcell_at(c, tr, U, T, cells, id, &V[id]);
+  return V;
+}
+
+void xo_viscous_face_flux(const xo_config *c, const xo_transport *tr, const double *U, const double *T, long ia, int d,
+                          double *F, double *J_out) {
+  int np[3], n[3], g[3];
+  long st[3];
+  grid(c, np, n, g, st);
+  vcell *V = vcell_table(c, tr, U, T);
+  vface(c, V, st, n, ia, d, F, J_out);
+  free(V);
+}
+
+int xo_viscous_rhs(const xo_config *c, const xo_transport *tr, const double *U, const double *T, double *rhs) {
+  const int Nv = c->N + 4;
+  int np[3], n[3], g[3];
+  long st[3];
+  grid(c, np, n, g, st);
+  const long cells = xo_padded_cells(c);
+  const double dxs[3] = {c->dx, c->dy, c->dz};
+  vcell *V = vcell_table(c, tr, U, T);
+  memset(rhs, 0, sizeof(double) * Nv * cells);
+  for (int d = 0; d < 3; ++d) {
+    if (n[d] == 1) continue;
+    const int a1 = (d + 1) % 3, a2 = (d + 2) % 3;
+    const long npen = (long)n[a1] * n[a2];
+#pragma omp parallel if (npen > 16)
+    {
+      double *Fv = (double *)malloc(sizeof(double) * (n[d] + 3) * Nv);
+#pragma omp for schedule(dynamic, 4)
+      for (long pen = 0; pen < npen; ++pen) {
+        const int p = g[a1] + (int)(pen / n[a2]), q = g[a2] + (int)(pen % n[a2]);
+        const long base = (long)p * st[a1] + (long)q * st[a2];
+        /* faces above cells g-2 .. g+n: the n+1 faces of the interior cells and one more on either side */
+        for (int f = 0; f < n[d] + 3; ++f) vface(c, V, st, n, base + (long)(g[d] - 2 + f) * st[d], d, Fv + f * Nv, NULL);
+        for (int i = 0; i < n[d]; ++i) {                          /* cell g+i: faces f = i+1 (below), i+2 (above) */
+          const long idx = base + (long)(g[d] + i) * st[d];
+          for (int v = 0; v < Nv; ++v)
+            rhs[v * cells + idx] += (27.0 * (Fv[(i + 2) * Nv + v] - Fv[(i + 1) * Nv + v]) -
+                                     (Fv[(i + 3) * Nv + v] - Fv[i * Nv + v])) / (24.0 * dxs[d]);
+        }
+      }
+      free(Fv);
+    }
+  }
+  free(V);
+  return 0;
+}
+
+int xo_rhs_ns(const xo_config *c, const xo_transport *tr, double *U, double *T, double *rhs) {
+  int status = xo_rhs(c, U, T, rhs);                    /* ghosts filled, T converged on every padded cell */
+  if (tr) {
+    const int Nv = c->N + 4;
+    const long cells = xo_padded_cells(c);
+    double *rv = (double *)malloc(sizeof(double) * Nv * cells);
+    status |= xo_viscous_rhs(c, tr, U, T, rv);
+    for (long q = 0; q < Nv * cells; ++q) rhs[q] += rv[q];
+    free(rv);
+  }
+  return status;
+}
+
+static int rk3_step(const xo_config *c_in, const xo_transport *tr, double *U, double *T, double dt) {
   xo_config cc = *c_in;
   cc.pp_dt = dt;                                          /* every stage is a forward-Euler step of size dt (Eq. 16, 17) */
   const xo_config *c = &cc;
@@ -660,7 +852,7 @@ int xo_rk3_step(const xo_config *c_in, double *U, double *T, double dt) {
   const size_t bytes = sizeof(double) * Nv * cells;
   double *U1 = (double *)malloc(bytes), *U2 = (double *)malloc(bytes), *Lr = (double *)malloc(bytes);
   int status = 0;
-  status |= xo_rhs(c, U, T, Lr);                         /* L(U^n) */
+  status |= xo_rhs_ns(c, tr, U, T, Lr);                       /* L(U^n) */
   memcpy(U1, U, bytes);
   memcpy(U2, U, bytes);
 #define FOR_INTERIOR                                                                  \
@@ -672,12 +864,12 @@ int xo_rk3_step(const xo_config *c_in, double *U, double *T, double dt) {
     const long id = v * cells + (long)k * st[2] + (long)j * st[1] + i;
     U1[id] = U[id] + dt * Lr[id];
   }
-  status |= xo_rhs(c, U1, T, Lr);                        /* L(U^1) */
+  status |= xo_rhs_ns(c, tr, U1, T, Lr);                       /* L(U^1) */
   FOR_INTERIOR {
     const long id = v * cells + (long)k * st[2] + (long)j * st[1] + i;
     U2[id] = 0.75 * U[id] + 0.25 * (U1[id] + dt * Lr[id]);
   }
-  status |= xo_rhs(c, U2, T, Lr);                        /* L(U^2) */
+  status |= xo_rhs_ns(c, tr, U2, T, Lr);                       /* L(U^2) */
   FOR_INTERIOR {
     const long id = v * cells + (long)k * st[2] + (long)j * st[1] + i;
     U[id] = 1.0 / 3.0 * U[id] + 2.0 / 3.0 * (U2[id] + dt * Lr[id]);
@@ -685,6 +877,11 @@ int xo_rk3_step(const xo_config *c_in, double *U, double *T, double dt) {
 #undef FOR_INTERIOR
   free(U1); free(U2); free(Lr);
   return status;
+}
+
+int xo_rk3_step(const xo_config *c, double *U, double *T, double dt) { return rk3_step(c, NULL, U, T, dt); }
+int xo_rk3_step_ns(const xo_config *c, const xo_transport *tr, double *U, double *T, double dt) {
+  return rk3_step(c, tr, U, T, dt);
 }
 
 /* ------------------------------------------------------------------------------------------------------------ */

@@ -121,6 +121,43 @@ int xo_rhs_cells(const xo_config *c, const double *U, const double *Tguess, long
 int xo_rk3_step(const xo_config *c, double *U, double *T, double dt);
 double xo_max_wavespeed(const xo_config *c, const double *U, double *T, int *status);
 
+/* ------------------------------------------------------------------------------------------------------------------
+ * Viscous / diffusive right-hand side div F_v (Eq. 1-6, Eq. 22, 26,
+ * PAPER.md:505-513 Eq. 29, "central 4th-order accuracy scheme" PAPER.md:107).  Readings R19-R23 of DESIGN.md:
+ *   R19 transport fits (Eq. 29): ln eta = a_0 + a_1 ln T + a_2 (ln T)^2 + a_3 (ln T)^3 for mu_s, kappa_s and for the binary
+ *       D_st at the reference pressure p_ref; D_st(T, p) = D_st(T, p_ref) p_ref / p (Eq. 25: D ~ 1/p).
+ *   R20 mixture rules as printed: Wilke's formula Eq. 22 for BOTH mu and kappa (Phi with the ratio of the respective
+ *       property); D_sm by Eq. 26 with X_t + 1e-12 in both sums (the printed form is 0/0 for a pure species).
+ *   R21 species diffusion flux, Eq. 6 with its indices repaired: J_s = -rho (D_sm grad Y_s - Y_s sum_i D_im grad Y_i), so
+ *       that sum_s J_s = 0; the species row of F_v is -J_s and the energy row tau.u + kappa grad T - sum_s h_s J_s (the
+ *       signs that make Eq. 1 a diffusion equation; Eq. 2 prints +J_s).
+ *   R22 discretisation: conservative, fourth order.  At the face between cells a and b = a + 1 of direction d, with the
+ *       four cells a-1, a, b, b+1: normal derivative (27 (f_b - f_a) - (f_{b+1} - f_{a-1}))/(24 dx_d); face value
+ *       (9 (f_a + f_b) - (f_{a-1} + f_{b+1}))/16, used for mu, kappa, rho D_sm, Y_s, h_s, u; transverse derivatives =
+ *       that face value of the cell-centred (f_{-2} - 8 f_{-1} + 8 f_{+1} - f_{+2})/(12 dx_e).  Divergence:
+ *       (27 (F_{i+1/2} - F_{i-1/2}) - (F_{i+3/2} - F_{i-3/2}))/(24 dx_d).  Reach: three cells, the ghost width of WENO5.
+ *   R23 the face-interpolated product rho D_sm (one cell quantity), not rho and D_sm apart.
+ * U must have its ghosts filled and T must hold the converged temperature of every padded cell (xo_rhs leaves both so).
+ * ------------------------------------------------------------------------------------------------------------------ */
+typedef struct {
+  double mu[XO_MAXN][4], kappa[XO_MAXN][4];     /* a_0..a_3 of ln mu_s, ln kappa_s in ln T                      */
+  double D[XO_MAXN][XO_MAXN][4];                /* a_0..a_3 of ln D_st(T, p_ref); symmetric, diagonal unused    */
+  double p_ref;
+} xo_transport;
+
+/* mixture transport of one cell: mu (Eq. 22), kappa (Eq. 22), rhoD[s] = rho D_sm (Eq. 26), h[s] (NASA polynomials) */
+void xo_transport_cell(const xo_config *c, const xo_transport *tr, double rho, const double *Y, double T, double *mu,
+                       double *kappa, double *rhoD, double *h);
+/* viscous flux at the face above padded cell ia in direction d (all Nv rows; row 0 is zero); J_out (may be NULL)
+ * receives the N diffusion fluxes J_s.n */
+void xo_viscous_face_flux(const xo_config *c, const xo_transport *tr, const double *U, const double *T, long ia, int d,
+                          double *F, double *J_out);
+/* rhs[v][cell] = div F_v at interior cells (other entries zero) */
+int xo_viscous_rhs(const xo_config *c, const xo_transport *tr, const double *U, const double *T, double *rhs);
+/* convective + viscous residual, and one SSP-RK3 step with it (ghosts and primitives before each residual) */
+int xo_rhs_ns(const xo_config *c, const xo_transport *tr, double *U, double *T, double *rhs);
+int xo_rk3_step_ns(const xo_config *c, const xo_transport *tr, double *U, double *T, double dt);
+
 #ifdef __cplusplus
 }
 #endif

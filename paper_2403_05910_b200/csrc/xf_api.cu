@@ -545,6 +545,43 @@ int xf_probe_fp64_peak(int device, int iters, double *tflops, double *ms_out) {
   return XF_OK;
 }
 
+int xf_probe_fp64_sustained(int device, double seconds, double *tflops, double *ms_out) {
+  if (!tflops || !(seconds > 0.0) || seconds > 30.0) return XF_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return XF_ECUDA;
+  DeviceGuard guard(device);
+  if (!guard.ok) return XF_ECUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return XF_ECUDA;
+  const int threads = 256, blocks = prop.multiProcessorCount * 8, iters = 40000;   // one launch: about 90 ms
+  double *sink = nullptr;
+  if (cudaMalloc(&sink, sizeof(double) * (size_t)blocks * threads) != cudaSuccess) return XF_ENOMEM;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  int rc = xf_probe_fp64_launch(blocks, threads, iters, sink, nullptr);   // warm-up, and the length of one launch
+  cudaEventRecord(e0, nullptr);
+  if (rc == XF_OK) rc = xf_probe_fp64_launch(blocks, threads, iters, sink, nullptr);
+  cudaEventRecord(e1, nullptr);
+  if (cudaEventSynchronize(e1) != cudaSuccess) rc = XF_ECUDA;
+  float one = 0.f;
+  cudaEventElapsedTime(&one, e0, e1);
+  const int n = one > 0.f ? (int)(seconds * 1e3 / one) + 1 : 1;
+  cudaEventRecord(e0, nullptr);
+  for (int q = 0; q < n && rc == XF_OK; ++q) rc = xf_probe_fp64_launch(blocks, threads, iters, sink, nullptr);
+  cudaEventRecord(e1, nullptr);
+  if (cudaEventSynchronize(e1) != cudaSuccess) rc = XF_ECUDA;
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(sink);
+  if (rc != XF_OK) return rc;
+  *tflops = 2.0 * 16.0 * 8.0 * (double)iters * (double)blocks * (double)threads * (double)n / ((double)ms * 1e-3) * 1e-12;
+  if (ms_out) *ms_out = ms;
+  return XF_OK;
+}
+
 const char *xf_strerror(int code) {
   switch (code) {
     case XF_OK: return "ok";

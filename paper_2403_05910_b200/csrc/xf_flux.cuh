@@ -339,7 +339,7 @@ __device__ __forceinline__ bool face_flux(const int N, const double *sm, const d
 #define XF_LINEAR_FIELD(VIDX, V, DEXPR, VNEXT)                                                         \
   {                                                                                                    \
     double fp[S], fm[S];                                                                               \
-    const double C = fma(oma, V[MA], omb * V[MB]);                                                       \
+    const double C = fma(oma, V[MA], omb * V[MB]);                                                     \
     _Pragma("unroll") for (int m = 0; m < S; ++m) {                                                    \
       const double a = fma(-C, rho[m], V[m]);                                                          \
       fp[m] = ap[m] * a;                                                                               \

@@ -632,3 +632,45 @@ def rough_box(nx: int, ny: int, nz: int, nspecies: int = 4, seed: int = 3, bc=(B
     bc_state = np.tile(Ui.reshape(nspecies + 4, -1)[:, :1].T, (6, 1)) if BC_DIRICHLET in bc else None
     return _finish(f"rough_{nx}x{ny}x{nz}_{nspecies}sp", nx, ny, nz, d[0], d[1], d[2], table, bc, Ui, T, rng,
                    bc_state=bc_state)
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# transport fits for the viscous / diffusive terms (Eq. 29)
+# ----------------------------------------------------------------------------------------------------------------
+@dataclass
+class TransportFits:
+    """ln eta = a_0 + a_1 ln T + a_2 (ln T)^2 + a_3 (ln T)^3 for mu_s [N,4], kappa_s [N,4] and the binary D_st at p_ref
+    [N,N,4] (symmetric).  The paper fits these to kinetic-theory values of real species (collision-integral tables,
+    PAPER.md:155-178), which are not in this container; these are seeded synthetic fits of the same SHAPE: power laws
+    mu ~ T^0.7, kappa ~ T^0.75, D ~ T^1.7 with seeded quadratic / cubic corrections in ln T."""
+
+    mu: np.ndarray
+    kappa: np.ndarray
+    D: np.ndarray
+    p_ref: float
+
+
+def synthetic_transport(table: SpeciesTable, seed: int, mu0: float = 2e-3, T0: float = 300.0, p_ref: float = 1.0,
+                        rho0: float = 1.0) -> TransportFits:
+    """mu0: viscosity scale at T0 in the workload's units (rho ~ 1, p ~ 1, lengths ~ 1: mu0 = 2e-3 puts the cell Reynolds
+    number of the test boxes at O(10)); kappa_s = mu_s cp_s(T0) / Pr_s, D_st = mu / (rho0 Sc_st) at (T0, p_ref)."""
+    rng = np.random.default_rng(seed)
+    n = table.n
+    lnT0 = np.log(T0)
+
+    def fit(val0, expo):
+        a = np.zeros(4)
+        a[2], a[3] = rng.uniform(-0.02, 0.02), rng.uniform(-0.002, 0.002)
+        a[1] = expo - 2 * a[2] * lnT0 - 3 * a[3] * lnT0 ** 2     # d ln eta / d ln T = expo at T0
+        a[0] = np.log(val0) - (a[1] * lnT0 + a[2] * lnT0 ** 2 + a[3] * lnT0 ** 3)
+        return a
+
+    mus = mu0 * rng.uniform(0.5, 2.0, n)
+    cp0 = table.Rs * table.cp_over_R(np.float64(min(max(T0, table.Tlo), table.Thi)))
+    mu = np.stack([fit(mus[s], 0.7 + rng.uniform(-0.05, 0.05)) for s in range(n)])
+    kappa = np.stack([fit(mus[s] * cp0[s] / rng.uniform(0.65, 0.8), 0.75 + rng.uniform(-0.05, 0.05)) for s in range(n)])
+    D = np.zeros((n, n, 4))
+    for s in range(n):
+        for t in range(s + 1, n):
+            D[s, t] = D[t, s] = fit(0.5 * (mus[s] + mus[t]) / (rho0 * rng.uniform(0.6, 1.1)), 1.7 + rng.uniform(-0.05, 0.05))
+    return TransportFits(mu=mu, kappa=kappa, D=D, p_ref=float(p_ref))

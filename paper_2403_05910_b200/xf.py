@@ -28,7 +28,7 @@ ABI_SYMBOLS = (
     "xf_fill_ghosts", "xf_primitives", "xf_convective_rhs", "xf_rk3_step", "xf_rk3_step_cfl", "xf_step_cfl",
     "xf_max_wavespeed", "xf_set_rhs_dt",
     "xf_status", "xf_newton_mean_iterations", "xf_launch_count", "xf_convective_rhs_host", "xf_rk3_steps_host",
-    "xf_probe_fp64_peak", "xf_strerror", "xf_timing_enable", "xf_timing_read",
+    "xf_probe_fp64_peak", "xf_probe_fp64_sustained", "xf_strerror", "xf_timing_enable", "xf_timing_read",
 )
 KERNEL_KINDS = ("ghost_fill", "primitives", "sweep_x", "sweep_y", "sweep_z", "max_wavespeed")  # XF_K_* of xf.h
 
@@ -84,6 +84,7 @@ def lib() -> C.CDLL:
         L.xf_convective_rhs_host.argtypes = [ctx, dp, dp, dp]
         L.xf_rk3_steps_host.argtypes = [ctx, dp, dp, C.c_double, C.c_int, C.POINTER(C.c_double)]
         L.xf_probe_fp64_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.xf_probe_fp64_sustained.argtypes = [C.c_int, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.xf_timing_enable.argtypes = [ctx, C.c_int]
         L.xf_timing_read.argtypes = [ctx, vp, C.POINTER(C.c_double), C.POINTER(C.c_long)]
         L.xf_strerror.argtypes = [C.c_int]
@@ -127,6 +128,13 @@ def xf_probe_fp64_peak(device: int = 0, iters: int = 4096):
     """-> (TFLOP/s, ms) of the register-resident fp64 FMA probe kernel."""
     tf, ms = C.c_double(), C.c_double()
     _check(lib().xf_probe_fp64_peak(int(device), int(iters), C.byref(tf), C.byref(ms)), "xf_probe_fp64_peak")
+    return tf.value, ms.value
+
+
+def xf_probe_fp64_sustained(device: int = 0, seconds: float = 1.5):
+    """-> (TFLOP/s, ms) of the same probe launched back to back for at least ``seconds``."""
+    tf, ms = C.c_double(), C.c_double()
+    _check(lib().xf_probe_fp64_sustained(int(device), float(seconds), C.byref(tf), C.byref(ms)), "xf_probe_fp64_sustained")
     return tf.value, ms.value
 
 
