@@ -321,8 +321,13 @@ def run_b200(args, rank: int, local_rank: int, world: int) -> None:
         w = wl.with_ghost_width(w, 4)
     N, Nv, cells = w.nspecies, w.nvars, w.interior_cells
     D = sum(1 for n in (w.nx, w.ny, w.nz) if n > 1)
+    transport = None
+    if args.viscous:
+        from paper_2403_05910_b200 import workloads as wl
+
+        transport = wl.synthetic_transport(w.table, seed=4, mu0=2e-4)
     ctx = xf.Context.from_workload(w, device=local_rank, viscosity=args.viscosity, reconstruction=args.reconstruction,
-                                   positivity=args.positivity)
+                                   positivity=args.positivity, transport=transport)
     U = torch.from_numpy(w.U).to(dev)
     T = torch.from_numpy(w.T_guess).to(dev)
     work = ctx.workspace()
@@ -477,7 +482,7 @@ def run_b200(args, rank: int, local_rank: int, world: int) -> None:
                                "primitives, x/y/z sweeps, RK combine)", "rhs_per_step": 3, "l2": "inputs larger than L2 (one U copy = "
                                f"{Nv * ctx.cells * 8 / 1e9:.2f} GB), no flush", "parallelism": "replicas", "viscosity": ["LLF", "ROE", "GLF"][args.viscosity],
                        "reconstruction": ["WENO5-JS", "WENO-CU6", "WENO7"][args.reconstruction],
-                       "positivity_limiter": bool(args.positivity)},
+                       "positivity_limiter": bool(args.positivity), "viscous_terms": bool(args.viscous)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
             "step_roofline": step_roofline, "rhs_only": rhs_only, "source_hash": lib_source_hash(),
         }
@@ -563,6 +568,8 @@ def main() -> None:
     ap.add_argument("--viscosity", type=int, default=0, help="0 LLF (the benchmark), 1 ROE, 2 GLF")
     ap.add_argument("--reconstruction", type=int, default=0, help="0 WENO5-JS (the benchmark), 1 WENO-CU6, 2 WENO7")
     ap.add_argument("--positivity", action="store_true", help="positivity-preserving flux blending on (not the benchmark)")
+    ap.add_argument("--viscous", action="store_true",
+                    help="viscous / diffusive terms on, seeded synthetic transport fits (not the benchmark)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

@@ -64,6 +64,9 @@ typedef struct {
   int viscosity;           /* XF_VISC_*: the artificial viscosity Lambda~ of Eq. 14 (options 374)  */
   int reconstruction;      /* XF_RECON_*: the reconstruction of Eq. 15                            */
   int positivity;          /* != 0: positivity-preserving flux blending of Eq. 17-20, see below */
+  const double *transport; /* host: fitted transport coefficients (Eq. 29), or NULL = no viscous /
+                              diffusive terms.  ln eta = a_0 + a_1 ln T + a_2 (ln T)^2 + a_3 (ln T)^3, laid out as
+                              mu [N][4], kappa [N][4], D [N][N][4] (binary D_st at p_ref, symmetric), then p_ref   */
 } xf_config;
 
 /* Positivity-preserving flux blending (theta is deferred by the paper to its ref 41 -> DESIGN.md
@@ -121,6 +124,17 @@ int xf_primitives(xf_ctx *ctx, const double *U, double *T, double *p, double *c,
  * entries are written.  work: xf_rhs_workspace_bytes. */
 int xf_convective_rhs(xf_ctx *ctx, double *U, double *T, double *rhs, void *work, void *stream);
 
+/* Viscous / diffusive terms (context created with cfg.transport; Eq. 1-6; readings R19-R23):
+ * F_v = (0, tau, tau.u + kappa grad T - sum_s h_s J_s, -J_s) with tau of Eq. 3, mu and kappa by Wilke's rule (Eq. 22) from
+ * the fitted species values, J_s = -rho (D_sm grad Y_s - Y_s sum_i D_im grad Y_i) (Eq. 6), D_sm by Eq. 26, D_st ~ p_ref / p;
+ * conservative fourth-order central discretisation within the three ghost layers of WENO5.
+ *   xf_viscous_rhs   rhs = div F_v at interior cells.  U must have its ghosts filled and T must be the converged
+ *                    temperature of every padded cell (both are as xf_convective_rhs leaves them).  work:
+ *                    xf_rhs_workspace_bytes.
+ * With a transport table the three RK3 entry points integrate L = convective + viscous residual (the viscous part is
+ * evaluated first, into the partial-residual buffer the sweeps accumulate on); xf_convective_rhs stays convective. */
+int xf_viscous_rhs(xf_ctx *ctx, const double *U, const double *T, double *rhs, void *work, void *stream);
+
 /* The time step assumed by the positivity limiter of a bare xf_convective_rhs (see xf_config.positivity); dt >= 0. */
 int xf_set_rhs_dt(xf_ctx *ctx, double dt);
 
@@ -159,7 +173,7 @@ long xf_launch_count(const xf_ctx *ctx);
  * resets the record list.  max_records = 0 switches timing off.  The ghost fill (one launch per active direction)
  * is timed as one record. */
 enum { XF_K_GHOST = 0, XF_K_PRIM = 1, XF_K_SWEEP_X = 2, XF_K_SWEEP_Y = 3, XF_K_SWEEP_Z = 4, XF_K_WAVESPEED = 5,
-       XF_K_COUNT = 6 };
+       XF_K_TRANSPORT = 6, XF_K_VISCOUS = 7, XF_K_COUNT = 8 };
 int xf_timing_enable(xf_ctx *ctx, int max_records);
 int xf_timing_read(xf_ctx *ctx, void *stream, double *ms_out, long *count_out);
 

@@ -26,6 +26,7 @@ struct xf_ctx {
   double *S_dev;                      // max wave speed scalar used by the host-buffer entry points
   double *lam_glob_dev;               // GLF: [3][3] global maxima of the current residual evaluation
   int visc, recon;                    // XF_VISC_*, XF_RECON_*
+  XfTransportDev *tr_dev;             // transport fits (device), or nullptr: no viscous / diffusive terms
   int positivity;                     // positivity-preserving flux blending on (Eq. 17-20)
   double rhs_dt;                      // the step the limiter of a bare xf_convective_rhs guards (xf_set_rhs_dt)
   long launches;
@@ -97,7 +98,7 @@ int count_active(const XfGrid &G) { return (G.n[0] > 1) + (G.n[1] > 1) + (G.n[2]
 // ghosts -> primitives -> sweeps.  E_last describes what the LAST active sweep writes (residual or RK combine);
 // earlier sweeps accumulate the partial residual in `acc`.
 int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfEpilogue &E_last, cudaStream_t s,
-             double *S_out = nullptr) {
+             double *S_out = nullptr, bool with_stage_buffers = false) {
   int rc;
   {
     Timed t(c, XF_K_GHOST, s);
@@ -114,23 +115,41 @@ int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfE
   if (rc != XF_OK) return rc;
   const int nact = count_active(c->G);
   int done = 0;
+  // Viscous / diffusive terms (context created with a transport table): div F_v goes into the partial-residual buffer
+  // first -- with the alpha / (beta dt) U^n term of the stage, which the first sweep would otherwise carry -- and the
+  // sweeps accumulate on top of it, so the fused stage combination of the last sweep stays as it is.
+  const bool visc = c->tr_dev != nullptr;
+  if (visc) {
+    double *vtab = prim + (size_t)(c->N + 4) * (size_t)c->G.cells + (with_stage_buffers ? 3 * (size_t)c->Nv * (size_t)c->G.cells : 0);
+    {
+      Timed t(c, XF_K_TRANSPORT, s);
+      rc = xf_launch_transport(c->G, c->Th, c->tr_dev, U, T, vtab, s);
+      ++c->launches;
+    }
+    if (rc != XF_OK) return rc;
+    const bool carry_un = E_last.mode == 2 && E_last.alpha != 0.0;
+    Timed t(c, XF_K_VISCOUS, s);
+    rc = xf_launch_viscous(c->G, c->N, vtab, T, acc, carry_un ? &E_last : nullptr, s, &c->launches);
+    if (rc != XF_OK) return rc;
+  }
   for (int dd = 0; dd < 3; ++dd) {
     const int d = dd;
     if (c->G.n[d] == 1) continue;
     XfEpilogue E;
     // a stage with alpha != 0 and more than one sweep: the first sweep adds alpha/(beta dt) U^n to the partial
     // residual and the last one no longer reads U^n (XfEpilogue mode 3)
-    const bool un_first = E_last.mode == 2 && E_last.alpha != 0.0 && nact > 1;
+    const bool un_first = E_last.mode == 2 && E_last.alpha != 0.0 && (nact > 1 || visc);
+    const bool have_acc = done > 0 || visc;                 // a partial residual is already in `acc`
     if (done == nact - 1) {
       E = E_last;
-      E.has_acc = done > 0;
-      if (E.mode != 2) E.mode = done > 0 ? 1 : 0;
+      E.has_acc = have_acc;
+      if (E.mode != 2) E.mode = have_acc ? 1 : 0;
       if (un_first) E.alpha = 0.0;
       E.acc = acc;
     } else {
       memset(&E, 0, sizeof(E));
-      E.mode = done > 0 ? 1 : 0;
-      if (done == 0 && un_first) {
+      E.mode = have_acc ? 1 : 0;
+      if (done == 0 && un_first && !visc) {
         E = E_last;
         E.mode = 3;
       }
@@ -172,13 +191,13 @@ int rk3(xf_ctx *c, double *U, double *T, double dt, double cfl, const double *S_
   E.Un = U;
   // Eq. 16: U1 = Un + dt L(Un); U2 = 3/4 Un + 1/4 (U1 + dt L(U1)); Un+1 = 1/3 Un + 2/3 (U2 + dt L(U2))
   E.alpha = 0.0; E.beta = 1.0; E.out = U1;
-  int rc = residual(c, U, T, work, acc, E, s, S_out);
+  int rc = residual(c, U, T, work, acc, E, s, S_out, true);
   if (rc != XF_OK) return rc;
   E.alpha = 0.75; E.beta = 0.25; E.out = U2;
-  rc = residual(c, U1, T, work, acc, E, s);
+  rc = residual(c, U1, T, work, acc, E, s, nullptr, true);
   if (rc != XF_OK) return rc;
   E.alpha = 1.0 / 3.0; E.beta = 2.0 / 3.0; E.out = U;
-  return residual(c, U2, T, work, acc, E, s);
+  return residual(c, U2, T, work, acc, E, s, nullptr, true);
 }
 
 int ensure_host_mirrors(xf_ctx *c) {
@@ -283,6 +302,30 @@ int xf_create(xf_ctx **out, const xf_config *cfg) {
          cudaMemset(c->status_dev, 0, sizeof(int)) == cudaSuccess &&
          cudaMemset(c->itersum_dev, 0, sizeof(unsigned long long)) == cudaSuccess;
   }
+  if (ok && cfg->transport) {   // Eq. 29 fits [N][4] mu, [N][4] kappa, [N][N][4] D_st, p_ref -> evaluation form on the device
+    XfTransportDev *h = new (std::nothrow) XfTransportDev;
+    ok = h != nullptr;
+    if (ok) {
+      memset(h, 0, sizeof(*h));
+      const double *t = cfg->transport;
+      for (int s = 0; s < N; ++s)
+        for (int q = 0; q < 4; ++q) {
+          h->mu[s][q] = t[4 * s + q];
+          h->kappa[s][q] = t[4 * N + 4 * s + q];
+        }
+      for (int s = 0; s < N; ++s)
+        for (int u = 0; u < N; ++u) {
+          for (int q = 0; q < 4; ++q) h->D[s][u][q] = t[8 * N + 4 * (s * N + u) + q];
+          h->w8[s][u] = 1.0 / sqrt(8.0) / sqrt(1.0 + cfg->W[s] / cfg->W[u]);
+          h->q4[s][u] = sqrt(sqrt(cfg->W[u] / cfg->W[s]));
+        }
+      for (int s = 0; s < N; ++s) h->W[s] = cfg->W[s];
+      h->p_ref = t[8 * N + 4 * N * N];
+      ok = h->p_ref > 0.0 && cudaMalloc(&c->tr_dev, sizeof(XfTransportDev)) == cudaSuccess &&
+           cudaMemcpy(c->tr_dev, h, sizeof(XfTransportDev), cudaMemcpyHostToDevice) == cudaSuccess;
+      delete h;
+    }
+  }
   if (ok) ok = xf_sweep_x_init() == XF_OK && xf_sweep_y_init() == XF_OK && xf_sweep_z_init() == XF_OK;
   if (!ok) {
     xf_destroy(c);
@@ -300,6 +343,7 @@ int xf_destroy(xf_ctx *c) {
   cudaFree(c->bc_state_dev);
   cudaFree(c->S_dev);
   cudaFree(c->lam_glob_dev);
+  cudaFree(c->tr_dev);
   cudaFree(c->hU);
   cudaFree(c->hT);
   cudaFree(c->hR);
@@ -311,9 +355,13 @@ int xf_destroy(xf_ctx *c) {
 
 size_t xf_num_vars(const xf_ctx *c) { return c ? (size_t)c->Nv : 0; }
 size_t xf_padded_cells(const xf_ctx *c) { return c ? (size_t)c->G.cells : 0; }
-size_t xf_rhs_workspace_bytes(const xf_ctx *c) { return c ? field_bytes(c) * (size_t)(c->N + 4) : 0; }
+// workspace layout: [p, c, 1/rho, Gamma, chi_s: N + 4] ([U1, U2, partial residual: 3 Nv] for the RK3 calls) [cell table of
+// the viscous terms: 3 N + 5, only with a transport table]
+size_t xf_rhs_workspace_bytes(const xf_ctx *c) {
+  return c ? field_bytes(c) * (size_t)(c->N + 4 + (c->tr_dev ? 3 * c->N + 5 : 0)) : 0;
+}
 size_t xf_workspace_bytes(const xf_ctx *c) {
-  return c ? field_bytes(c) * (size_t)(c->N + 4 + 3 * c->Nv) : 0;
+  return c ? field_bytes(c) * (size_t)(c->N + 4 + 3 * c->Nv + (c->tr_dev ? 3 * c->N + 5 : 0)) : 0;
 }
 
 int xf_fill_ghosts(xf_ctx *c, double *U, void *stream) {
@@ -345,6 +393,24 @@ int xf_convective_rhs(xf_ctx *c, double *U, double *T, double *rhs, void *work, 
   E.mode = 0;
   E.out = rhs;
   return residual(c, U, T, work, rhs, E, static_cast<cudaStream_t>(stream));
+}
+
+int xf_viscous_rhs(xf_ctx *c, const double *U, const double *T, double *rhs, void *work, void *stream) {
+  if (!c || !U || !T || !rhs || !work || !c->tr_dev) return XF_EINVAL;
+  Range r("xf_viscous_rhs");
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  double *vtab = static_cast<double *>(work) + (size_t)(c->N + 4) * (size_t)c->G.cells;
+  int rc;
+  {
+    Timed t(c, XF_K_TRANSPORT, s);
+    rc = xf_launch_transport(c->G, c->Th, c->tr_dev, U, T, vtab, s);
+    ++c->launches;
+  }
+  if (rc != XF_OK) return rc;
+  Timed t(c, XF_K_VISCOUS, s);
+  return xf_launch_viscous(c->G, c->N, vtab, T, rhs, nullptr, s, &c->launches);
 }
 
 int xf_set_rhs_dt(xf_ctx *c, double dt) {

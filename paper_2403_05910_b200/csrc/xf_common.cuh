@@ -36,6 +36,17 @@ struct XfThermo {
   int N;
 };
 
+// Transport fits of the viscous / diffusive terms in evaluation form, in DEVICE memory (13 KB: too large for the
+// kernel-parameter bank): Eq. 29 coefficients and the species-pair constants of Wilke's rule (Eq. 22),
+// w8[s][t] = 1 / sqrt(8) / sqrt(1 + W_s/W_t), q4[s][t] = (W_t/W_s)^(1/4).
+struct XfTransportDev {
+  double mu[XF_MAXN][4], kappa[XF_MAXN][4];
+  double D[XF_MAXN][XF_MAXN][4];
+  double w8[XF_MAXN][XF_MAXN], q4[XF_MAXN][XF_MAXN];
+  double W[XF_MAXN];
+  double p_ref;
+};
+
 struct XfBc {
   int kind[6];
 };
@@ -95,6 +106,13 @@ int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *pri
                       XfTmapCache *tc, cudaStream_t s);
 int xf_launch_sweep_z(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
                       XfTmapCache *tc, cudaStream_t s);
+
+// viscous / diffusive terms (xf_visc.cu): the cell table vtab [3 N + 5][padded] from U, T; then out = base + div F_v with
+// base = alpha / (beta dt) U^n if `stage` (an XfEpilogue of mode 2 with alpha != 0) is given, else 0
+int xf_launch_transport(const XfGrid &G, const XfThermo &Th, const XfTransportDev *tr_dev, const double *U, const double *T,
+                        double *vtab, cudaStream_t s);
+int xf_launch_viscous(const XfGrid &G, int N, const double *vtab, const double *T, double *out, const XfEpilogue *stage,
+                      cudaStream_t s, long *launches);
 
 // fp64 reciprocal: MUFU.RCP64H seed (relative error e <= 1e-6) refined as r (1 + e + e^2), which leaves e^3:
 // 3 DFMA, measured max relative error 2.2e-16 over 1e-13 .. 1e13.  The path is bound by the fp64 pipe, and an

@@ -1,0 +1,316 @@
+// xf_visc.cu -- viscous / diffusive right-hand side div F_v for sm_100a (Eq. 1-6,
+// PAPER.md:155-178 Eq. 22 and 26, Eq. 29, "central 4th-order accuracy scheme" PAPER.md:107; readings
+// R19-R23 of DESIGN.md).  Two kernels:
+//
+//   transport_kernel   one thread per padded cell: u, v, w, Y_s, h_s(T), and the mixture transport coefficients from the
+//                      fitted ln-polynomials (Eq. 29) -- Wilke's rule for mu and kappa (Eq. 22), rho D_sm (Eq. 26) -- into
+//                      the cell table vtab [3 N + 5 fields][padded cells].  This is where the exponentials, square roots
+//                      and the O(N^2) pair sums live.
+//   visc_dir_kernel    one launch per active direction d: a block owns a tile of LD cells along d (x LT lanes along i);
+//                      each thread computes ONE face flux F_v (fourth-order face operators of reading R22: normal
+//                      derivative, face value, face value of the cell-centred transverse derivatives) into shared memory,
+//                      then the cells of the tile take the fourth-order divergence (27 (F_{+1/2} - F_{-1/2}) - (F_{+3/2} -
+//                      F_{-3/2}))/(24 dx) of the LD + 3 faces and add it to the residual.  A face flux never reaches HBM.
+//
+// HBM-bound (stencil reads of the cell table through L1/L2), unlike the convective sweeps.  No tensor cores: nothing
+// here is a contraction.  No code is shared with oracle/.
+#include "xf_common.cuh"
+
+namespace {
+
+// vtab field order
+constexpr int VT_U = 0, VT_MU = 3, VT_KAPPA = 4, VT_Y = 5;
+__host__ __device__ constexpr int vt_h(int N) { return 5 + N; }
+__host__ __device__ constexpr int vt_rd(int N) { return 5 + 2 * N; }
+
+__device__ __forceinline__ double fit_eval(const double *a, double lnT) {   // Eq. 29
+  return exp(fma(lnT, fma(lnT, fma(lnT, a[3], a[2]), a[1]), a[0]));
+}
+
+template <int N_T>
+__global__ void __launch_bounds__(128)
+transport_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const XfTransportDev *__restrict__ tr,
+                 const double *__restrict__ U, const double *__restrict__ T, double *__restrict__ vtab) {
+  constexpr int NS = N_T > 0 ? N_T : XF_MAXN;
+  const int N = N_T > 0 ? N_T : th.N;
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= G.cells) return;
+  const long long C = G.cells;
+  const double rho = U[idx], rinv = 1.0 / rho;
+#pragma unroll
+  for (int q = 0; q < 3; ++q) vtab[(VT_U + q) * C + idx] = U[(1 + q) * C + idx] * rinv;
+  double X[NS];   // first Y_s / W_s, then the mole fractions
+  double sumY = 0.0, sumYW = 0.0, Rbar = 0.0;
+#pragma unroll
+  for (int s = 0; s < NS; ++s) {
+    if (s < N) {
+      const double Y = s < N - 1 ? U[(5 + s) * C + idx] * rinv : 1.0 - sumY;   // closure, no clipping (reading R12)
+      sumY += Y;
+      vtab[(VT_Y + s) * C + idx] = Y;
+      X[s] = Y / tr->W[s];
+      sumYW += X[s];
+      Rbar = fma(Y, th.Rs[s], Rbar);
+    }
+  }
+  const double Tk = T[idx], lnT = log(Tk);
+  const double p = rho * Rbar * Tk;   // Eq. 7
+  double Wbar = 0.0;
+#pragma unroll
+  for (int s = 0; s < NS; ++s)
+    if (s < N) {
+      X[s] /= sumYW;
+      Wbar = fma(X[s], tr->W[s], Wbar);
+    }
+  // ---- species enthalpies h_s(T) (NASA polynomials with the constant-cp continuation, reading R3)
+  const double Tc = fmin(fmax(Tk, th.Tlo), th.Thi);
+#pragma unroll
+  for (int s = 0; s < NS; ++s)
+    if (s < N) {
+      const double *a = th.a[s], *b = th.b[s];
+      const double hp = fma(Tc, fma(Tc, fma(Tc, fma(Tc, b[3], b[2]), b[1]), b[0]), a[0]);
+      const double cp = fma(Tc, fma(Tc, fma(Tc, fma(Tc, a[4], a[3]), a[2]), a[1]), a[0]);
+      vtab[(vt_h(N) + s) * C + idx] = th.Rs[s] * fma(cp, Tk - Tc, fma(Tc, hp, a[5]));
+    }
+  // ---- Wilke's rule (Eq. 22), once for mu and once for kappa: sqrt(a_s / a_t) = sqrt(a_s) / sqrt(a_t)
+#pragma unroll 1
+  for (int which = 0; which < 2; ++which) {
+    double a[NS], sq[NS], isq[NS];
+#pragma unroll
+    for (int s = 0; s < NS; ++s)
+      if (s < N) {
+        a[s] = fit_eval(which == 0 ? tr->mu[s] : tr->kappa[s], lnT);
+        sq[s] = sqrt(a[s]);
+        isq[s] = 1.0 / sq[s];
+      }
+    double mix = 0.0;
+#pragma unroll
+    for (int s = 0; s < NS; ++s)
+      if (s < N) {
+        double den = 0.0;
+#pragma unroll
+        for (int t = 0; t < NS; ++t)
+          if (t < N) {
+            const double bb = fma(sq[s] * isq[t], tr->q4[s][t], 1.0);
+            den = fma(X[t] * tr->w8[s][t], bb * bb, den);
+          }
+        mix += X[s] * a[s] / den;
+      }
+    vtab[(which == 0 ? VT_MU : VT_KAPPA) * C + idx] = mix;
+  }
+  // ---- rho D_sm (Eq. 26 with X_t + 1e-12, reading R20; D_st(T, p) = D_st(T, p_ref) p_ref / p, reading R19)
+  double num[NS], den[NS];
+#pragma unroll
+  for (int s = 0; s < NS; ++s) num[s] = den[s] = 0.0;
+  const double pscale = p / tr->p_ref;
+#pragma unroll
+  for (int s = 0; s < NS; ++s)
+#pragma unroll
+    for (int t = s + 1; t < NS; ++t)
+      if (t < N) {
+        const double invD = pscale / fit_eval(tr->D[s][t], lnT);   // 1 / D_st, symmetric
+        const double xs = X[s] + 1e-12, xt = X[t] + 1e-12;
+        num[s] = fma(xt, tr->W[t], num[s]);
+        num[t] = fma(xs, tr->W[s], num[t]);
+        den[s] = fma(xt, invD, den[s]);
+        den[t] = fma(xs, invD, den[t]);
+      }
+#pragma unroll
+  for (int s = 0; s < NS; ++s)
+    if (s < N) vtab[(vt_rd(N) + s) * C + idx] = N > 1 ? rho * num[s] / (Wbar * den[s]) : 0.0;
+}
+
+__device__ __forceinline__ double interp4(double m1, double a, double b, double p2) {
+  return (9.0 * (a + b) - (m1 + p2)) * (1.0 / 16.0);
+}
+
+struct ViscArgs {
+  const double *vtab, *T;
+  double *out;
+  const double *Un;        // base term kappa_un * U^n of the FIRST launch of a residual evaluation (or nullptr)
+  double alpha, beta, dt, cfl;
+  const double *S_dev;     // dt = cfl / *S_dev if set (the device-side time step of xf_step_cfl)
+  int first;               // 1: out = base + div, 0: out += div
+  int seg;                 // cells along d per block
+};
+
+// DIR = 0: block = LDF threads along i, one face each, LDF - 3 cells; DIR = 1, 2: block = 32 lanes along i x LDF face rows
+template <int N_T, int DIR, int LDF>
+__global__ void __launch_bounds__(DIR == 0 ? LDF : 32 * LDF)
+visc_dir_kernel(const XfGrid G, const int Nrt, const ViscArgs A) {
+  constexpr int NS = N_T > 0 ? N_T : XF_MAXN;
+  const int N = N_T > 0 ? N_T : Nrt, Nv = N + 4;
+  constexpr int LT = DIR == 0 ? 1 : 32, LD = LDF - 3;
+  extern __shared__ double fs[];                                  // [Nv - 1][LDF][LT]
+  const long long C = G.cells;
+  const int k = DIR == 0 ? threadIdx.x : threadIdx.y;             // face index within the tile
+  const int lt = DIR == 0 ? 0 : threadIdx.x;
+  // tile origin: first cell along d (interior numbering), the transverse position
+  int c0, i, j2;                                                  // j2: index along the remaining transverse direction
+  if (DIR == 0) {
+    c0 = blockIdx.x * LD;
+    i = 0;
+    j2 = 0;
+  } else {
+    c0 = blockIdx.y * LD;
+    i = blockIdx.x * 32 + lt;
+    j2 = blockIdx.z;
+  }
+  const bool lane_ok = DIR == 0 || i < G.n[0];
+  long long base;                                                 // padded index of the pencil's cell 0 along d
+  if (DIR == 0) base = (long long)(blockIdx.y + G.g[1]) * G.st[1] + (long long)(blockIdx.z + G.g[2]) * G.st[2];
+  else if (DIR == 1) base = (long long)(G.g[0] + (lane_ok ? i : 0)) + (long long)(j2 + G.g[2]) * G.st[2];
+  else base = (long long)(G.g[0] + (lane_ok ? i : 0)) + (long long)(j2 + G.g[1]) * G.st[1];
+  const long long sd = G.st[DIR];
+  const int n = G.n[DIR], g = G.g[DIR];
+  const int a = c0 - 2 + k;                                       // interior number of the cell below this thread's face
+  if (lane_ok && a <= n && a >= -2) {                             // faces above cells -2 .. n (reading R22)
+    const long long ia = base + (long long)(g + a) * sd;
+    const long long q0 = ia - sd, q1 = ia, q2 = ia + sd, q3 = ia + 2 * sd;
+    const double *V = A.vtab;
+    const double in = G.inv_d[DIR] * (1.0 / 24.0);
+#define FACE(f) interp4(V[(f) * C + q0], V[(f) * C + q1], V[(f) * C + q2], V[(f) * C + q3])
+#define DN(f) ((27.0 * (V[(f) * C + q2] - V[(f) * C + q1]) - (V[(f) * C + q3] - V[(f) * C + q0])) * in)
+    double Gr[3][3];                                              // Gr[p][e] = d u_p / d x_e at the face
+#pragma unroll
+    for (int p = 0; p < 3; ++p) {
+#pragma unroll
+      for (int e = 0; e < 3; ++e) {
+        if (e == DIR) Gr[p][e] = DN(VT_U + p);
+        else if (G.n[e] == 1) Gr[p][e] = 0.0;
+        else {
+          const long long se = G.st[e];
+          const double ie = G.inv_d[e] * (1.0 / 12.0);
+          const double *u = V + (VT_U + p) * C;
+          double t[4];
+#pragma unroll
+          for (int m = 0; m < 4; ++m) {
+            const long long z = ia + (long long)(m - 1) * sd;
+            t[m] = ((u[z - 2 * se] - u[z + 2 * se]) - 8.0 * (u[z - se] - u[z + se])) * ie;
+          }
+          Gr[p][e] = interp4(t[0], t[1], t[2], t[3]);
+        }
+      }
+    }
+    const double mu = FACE(VT_MU), kappa = FACE(VT_KAPPA);
+    const double div = Gr[0][0] + Gr[1][1] + Gr[2][2];
+    double work = 0.0;
+#pragma unroll
+    for (int p = 0; p < 3; ++p) {                                 // tau_{p d}, Eq. 3
+      const double tau = mu * (Gr[p][DIR] + Gr[DIR][p]) - (p == DIR ? (2.0 / 3.0) * mu * div : 0.0);
+      fs[(p * LDF + k) * LT + lt] = tau;
+      work = fma(tau, FACE(VT_U + p), work);
+    }
+    double tJ[NS], corr = 0.0;
+#pragma unroll
+    for (int s = 0; s < NS; ++s)
+      if (s < N) {
+        tJ[s] = FACE(vt_rd(N) + s) * DN(VT_Y + s);
+        corr += tJ[s];
+      }
+    double qd = 0.0;
+#pragma unroll
+    for (int s = 0; s < NS; ++s)
+      if (s < N) {                                                // Eq. 6 (reading R21), Eq. 5
+        const double J = -(tJ[s] - FACE(VT_Y + s) * corr);
+        qd = fma(FACE(vt_h(N) + s), J, qd);
+        if (s < N - 1) fs[((4 + s) * LDF + k) * LT + lt] = -J;
+      }
+    const double dT = (27.0 * (A.T[q2] - A.T[q1]) - (A.T[q3] - A.T[q0])) * in;
+    fs[(3 * LDF + k) * LT + lt] = work + kappa * dT - qd;         // tau.u - q_c - q_d (Eq. 2, 4)
+#undef FACE
+#undef DN
+  }
+  __syncthreads();
+  const int cell = c0 + k;                                        // this thread's cell: faces k .. k + 3 of the tile
+  if (k < LD && lane_ok && cell < n) {
+    const long long ic = base + (long long)(g + cell) * sd;
+    const double in = G.inv_d[DIR] * (1.0 / 24.0);
+    double kap = 0.0;
+    if (A.first && A.Un) {                                        // the stage's alpha / (beta dt) U^n term (XfEpilogue mode 3)
+      const double dt = A.S_dev ? A.cfl / *A.S_dev : A.dt;
+      kap = A.alpha / (A.beta * dt);
+    }
+    if (A.first) A.out[ic] = A.Un ? kap * A.Un[ic] : 0.0;         // the density row has no viscous flux
+    for (int v = 1; v < Nv; ++v) {
+      const double *f = fs + ((v - 1) * LDF + k) * LT + lt;
+      const double dv = (27.0 * (f[2 * LT] - f[LT]) - (f[3 * LT] - f[0])) * in;
+      const long long o = v * C + ic;
+      A.out[o] = (A.first ? (A.Un ? kap * A.Un[o] : 0.0) : A.out[o]) + dv;
+    }
+  }
+}
+
+#define XF_DISPATCH_N(N, CALL)        \
+  switch (N) {                        \
+    case 1: { CALL(1); break; }       \
+    case 2: { CALL(2); break; }       \
+    case 3: { CALL(3); break; }       \
+    case 4: { CALL(4); break; }       \
+    case 10: { CALL(10); break; }     \
+    default: { CALL(0); break; }      \
+  }
+
+constexpr int LDF_X = 256, LDF_YZ = 16;
+
+template <int NT, int DIR>
+int launch_dir(const XfGrid &G, int N, const ViscArgs &A, cudaStream_t s) {
+  constexpr int LDF = DIR == 0 ? LDF_X : LDF_YZ, LD = LDF - 3;
+  const int OD = DIR == 1 ? 2 : 1;
+  const dim3 block = DIR == 0 ? dim3(LDF) : dim3(32, LDF);
+  const dim3 grid = DIR == 0 ? dim3((G.n[0] + LD - 1) / LD, G.n[1], G.n[2])
+                             : dim3((G.n[0] + 31) / 32, (G.n[DIR] + LD - 1) / LD, G.n[OD]);
+  const size_t smem = sizeof(double) * (size_t)(N + 3) * LDF * (DIR == 0 ? 1 : 32);
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaFuncSetAttribute(visc_dir_kernel<NT, DIR, LDF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         (int)(sizeof(double) * (XF_MAXN + 3) * LDF * (DIR == 0 ? 1 : 32)));
+    attr_done = true;
+  }
+  visc_dir_kernel<NT, DIR, LDF><<<grid, block, smem, s>>>(G, N, A);
+  return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
+}
+
+}  // namespace
+
+int xf_launch_transport(const XfGrid &G, const XfThermo &Th, const XfTransportDev *tr_dev, const double *U, const double *T,
+                        double *vtab, cudaStream_t s) {
+  const int threads = 128;
+  const unsigned blocks = (unsigned)((G.cells + threads - 1) / threads);
+#define CALL(NT) transport_kernel<NT><<<blocks, threads, 0, s>>>(G, Th, tr_dev, U, T, vtab)
+  XF_DISPATCH_N(Th.N, CALL)
+#undef CALL
+  return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
+}
+
+// out = base + sum over active directions of the fourth-order divergence of F_v; base = kappa_un U^n or 0 (see ViscArgs)
+int xf_launch_viscous(const XfGrid &G, int N, const double *vtab, const double *T, double *out, const XfEpilogue *stage,
+                      cudaStream_t s, long *launches) {
+  ViscArgs A;
+  A.vtab = vtab;
+  A.T = T;
+  A.out = out;
+  A.Un = nullptr;
+  A.alpha = A.beta = A.dt = A.cfl = 0.0;
+  A.S_dev = nullptr;
+  if (stage) {   // the first sweep of this stage would have carried alpha / (beta dt) U^n: the viscous term carries it instead
+    A.Un = stage->Un;
+    A.alpha = stage->alpha;
+    A.beta = stage->beta;
+    A.dt = stage->dt;
+    A.cfl = stage->cfl;
+    A.S_dev = stage->S_dev;
+  }
+  A.first = 1;
+  A.seg = 0;
+  for (int d = 0; d < 3; ++d) {
+    if (G.n[d] == 1) continue;
+    int rc = XF_OK;
+#define CALL(NT) rc = d == 0 ? launch_dir<NT, 0>(G, N, A, s) : (d == 1 ? launch_dir<NT, 1>(G, N, A, s) : launch_dir<NT, 2>(G, N, A, s))
+    XF_DISPATCH_N(N, CALL)
+#undef CALL
+    if (rc != XF_OK) return rc;
+    if (launches) ++*launches;
+    A.first = 0;
+  }
+  return XF_OK;
+}

@@ -26,11 +26,12 @@ XF_MAX_SPECIES = 16
 ABI_SYMBOLS = (
     "xf_create", "xf_destroy", "xf_num_vars", "xf_padded_cells", "xf_rhs_workspace_bytes", "xf_workspace_bytes",
     "xf_fill_ghosts", "xf_primitives", "xf_convective_rhs", "xf_rk3_step", "xf_rk3_step_cfl", "xf_step_cfl",
-    "xf_max_wavespeed", "xf_set_rhs_dt",
+    "xf_max_wavespeed", "xf_set_rhs_dt", "xf_viscous_rhs",
     "xf_status", "xf_newton_mean_iterations", "xf_launch_count", "xf_convective_rhs_host", "xf_rk3_steps_host",
     "xf_probe_fp64_peak", "xf_probe_fp64_sustained", "xf_strerror", "xf_timing_enable", "xf_timing_read",
 )
-KERNEL_KINDS = ("ghost_fill", "primitives", "sweep_x", "sweep_y", "sweep_z", "max_wavespeed")  # XF_K_* of xf.h
+KERNEL_KINDS = ("ghost_fill", "primitives", "sweep_x", "sweep_y", "sweep_z", "max_wavespeed", "transport",
+                "viscous")  # XF_K_* of xf.h
 
 
 class XfConfig(C.Structure):
@@ -42,7 +43,7 @@ class XfConfig(C.Structure):
         ("Tlo", C.c_double), ("Thi", C.c_double),
         ("bc", C.c_int * 6), ("bc_state", C.POINTER(C.c_double)),
         ("newton_rtol", C.c_double), ("newton_maxit", C.c_int), ("device", C.c_int), ("viscosity", C.c_int), ("reconstruction", C.c_int),
-        ("positivity", C.c_int),
+        ("positivity", C.c_int), ("transport", C.POINTER(C.c_double)),
     ]
 
 
@@ -73,6 +74,7 @@ def lib() -> C.CDLL:
         L.xf_primitives.argtypes = [ctx, dp, dp, dp, dp, vp]
         L.xf_convective_rhs.argtypes = [ctx, dp, dp, dp, vp, vp]
         L.xf_set_rhs_dt.argtypes = [ctx, C.c_double]
+        L.xf_viscous_rhs.argtypes = [ctx, dp, dp, dp, vp, vp]
         L.xf_rk3_step.argtypes = [ctx, dp, dp, C.c_double, vp, vp]
         L.xf_rk3_step_cfl.argtypes = [ctx, dp, dp, C.c_double, dp, vp, vp]
         L.xf_step_cfl.argtypes = [ctx, dp, dp, C.c_double, dp, vp, vp]
@@ -144,7 +146,7 @@ class Context:
     def __init__(self, nx: int, ny: int, nz: int, dx: float, dy: float, dz: float, W: Sequence[float], nasa7, Ru: float,
                  Tlo: float, Thi: float, bc=(0,) * 6, bc_state=None, newton_rtol: float = 0.0, newton_maxit: int = 0,
                  device: int = 0, viscosity: int = XF_VISC_LLF, reconstruction: int = XF_RECON_WENO5,
-                 positivity: bool = False, ng: Optional[int] = None):
+                 positivity: bool = False, ng: Optional[int] = None, transport=None):
         W = np.ascontiguousarray(W, dtype=np.float64)
         nasa7 = np.ascontiguousarray(nasa7, dtype=np.float64)
         n = int(W.shape[0])
@@ -168,6 +170,14 @@ class Context:
         cfg.viscosity = int(viscosity)
         cfg.reconstruction = int(reconstruction)
         cfg.positivity = int(bool(positivity))
+        tr = None
+        if transport is not None:   # an object with mu [N,4], kappa [N,4], D [N,N,4], p_ref (workloads.TransportFits)
+            tr = np.ascontiguousarray(np.concatenate([np.asarray(transport.mu, dtype=np.float64).ravel(),
+                                                      np.asarray(transport.kappa, dtype=np.float64).ravel(),
+                                                      np.asarray(transport.D, dtype=np.float64).ravel(),
+                                                      [float(transport.p_ref)]]))
+            assert tr.shape[0] == 8 * n + 4 * n * n + 1
+            cfg.transport = tr.ctypes.data_as(C.POINTER(C.c_double))
         self._h = C.c_void_p()
         _check(lib().xf_create(C.byref(self._h), C.byref(cfg)), "xf_create")
         self.device = int(device)
@@ -223,6 +233,10 @@ class Context:
         assert work.numel() * work.element_size() >= self.rhs_workspace_bytes
         _check(lib().xf_convective_rhs(self._h, _ptr(U), _ptr(T), _ptr(rhs), _ptr(work), _stream(stream)),
                "xf_convective_rhs")
+
+    def xf_viscous_rhs(self, U, T, rhs, work, stream=None) -> None:
+        assert work.numel() * work.element_size() >= self.rhs_workspace_bytes
+        _check(lib().xf_viscous_rhs(self._h, _ptr(U), _ptr(T), _ptr(rhs), _ptr(work), _stream(stream)), "xf_viscous_rhs")
 
     def xf_set_rhs_dt(self, dt: float) -> None:
         _check(lib().xf_set_rhs_dt(self._h, float(dt)), "xf_set_rhs_dt")
