@@ -273,12 +273,14 @@ def measured_peaks() -> dict:
 
 
 def lib_source_hash() -> str:
-    """Hash of the CUDA sources the library is built from: ties an ncu capture under profiles/ to the code it describes."""
+    """Hash of the CUDA sources of the benchmark path (sweeps, face flux, primitives, ghost fill, shared declarations): ties
+    an ncu capture under profiles/ to the code it describes."""
     h = hashlib.sha256()
     src = ROOT / "paper_2403_05910_b200" / "csrc"
-    for f in sorted(list(src.glob("*.cu")) + list(src.glob("*.cuh")) + [ROOT / "include" / "xf.h"]):
-        h.update(f.name.encode())
-        h.update(f.read_bytes())
+    for name in ("xf_common.cuh", "xf_flux.cuh", "xf_sweeps.cuh", "xf_sweep_x.cu", "xf_sweep_y.cu", "xf_sweep_z.cu",
+                 "xf_prim.cu", "xf_ghost.cu"):
+        h.update(name.encode())
+        h.update((src / name).read_bytes())
     return h.hexdigest()[:16]
 
 

@@ -27,96 +27,96 @@ __device__ __forceinline__ double fit_eval(const double *a, double lnT) {   // E
   return exp(fma(lnT, fma(lnT, fma(lnT, a[3], a[2]), a[1]), a[0]));
 }
 
+// Per-thread arrays live in shared memory ([species][thread]: conflict-free, dynamically indexable), so the O(N^2) pair
+// loops stay ROLLED: a fully unrolled version (45 exponentials inline at N = 10) took 255 registers, spilled and ran at a
+// quarter of this one's speed.
+constexpr int TR_THREADS = 128;
 template <int N_T>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(TR_THREADS)
 transport_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const XfTransportDev *__restrict__ tr,
                  const double *__restrict__ U, const double *__restrict__ T, double *__restrict__ vtab) {
-  constexpr int NS = N_T > 0 ? N_T : XF_MAXN;
   const int N = N_T > 0 ? N_T : th.N;
+  extern __shared__ double sh[];                     // X, a, sq, isq: 4 arrays [N][TR_THREADS]; num, den reuse a, sq
+  double *X = sh + threadIdx.x, *a = X + N * TR_THREADS, *sq = a + N * TR_THREADS, *isq = sq + N * TR_THREADS;
+  double *num = a, *den = sq;
+#define AT(arr, s) arr[(s) * TR_THREADS]
   const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= G.cells) return;
   const long long C = G.cells;
   const double rho = U[idx], rinv = 1.0 / rho;
 #pragma unroll
   for (int q = 0; q < 3; ++q) vtab[(VT_U + q) * C + idx] = U[(1 + q) * C + idx] * rinv;
-  double X[NS];   // first Y_s / W_s, then the mole fractions
   double sumY = 0.0, sumYW = 0.0, Rbar = 0.0;
-#pragma unroll
-  for (int s = 0; s < NS; ++s) {
-    if (s < N) {
-      const double Y = s < N - 1 ? U[(5 + s) * C + idx] * rinv : 1.0 - sumY;   // closure, no clipping (reading R12)
-      sumY += Y;
-      vtab[(VT_Y + s) * C + idx] = Y;
-      X[s] = Y / tr->W[s];
-      sumYW += X[s];
-      Rbar = fma(Y, th.Rs[s], Rbar);
-    }
+  for (int s = 0; s < N; ++s) {
+    const double Y = s < N - 1 ? U[(5 + s) * C + idx] * rinv : 1.0 - sumY;   // closure, no clipping (reading R12)
+    sumY += Y;
+    vtab[(VT_Y + s) * C + idx] = Y;
+    const double x = Y / tr->W[s];
+    AT(X, s) = x;
+    sumYW += x;
+    Rbar = fma(Y, th.Rs[s], Rbar);
   }
   const double Tk = T[idx], lnT = log(Tk);
   const double p = rho * Rbar * Tk;   // Eq. 7
+  const double isum = 1.0 / sumYW;
   double Wbar = 0.0;
-#pragma unroll
-  for (int s = 0; s < NS; ++s)
-    if (s < N) {
-      X[s] /= sumYW;
-      Wbar = fma(X[s], tr->W[s], Wbar);
-    }
+  for (int s = 0; s < N; ++s) {
+    const double x = AT(X, s) * isum;
+    AT(X, s) = x;
+    Wbar = fma(x, tr->W[s], Wbar);
+  }
   // ---- species enthalpies h_s(T) (NASA polynomials with the constant-cp continuation, reading R3)
   const double Tc = fmin(fmax(Tk, th.Tlo), th.Thi);
-#pragma unroll
-  for (int s = 0; s < NS; ++s)
-    if (s < N) {
-      const double *a = th.a[s], *b = th.b[s];
-      const double hp = fma(Tc, fma(Tc, fma(Tc, fma(Tc, b[3], b[2]), b[1]), b[0]), a[0]);
-      const double cp = fma(Tc, fma(Tc, fma(Tc, fma(Tc, a[4], a[3]), a[2]), a[1]), a[0]);
-      vtab[(vt_h(N) + s) * C + idx] = th.Rs[s] * fma(cp, Tk - Tc, fma(Tc, hp, a[5]));
-    }
+  for (int s = 0; s < N; ++s) {
+    const double *ca = th.a[s], *cb = th.b[s];
+    const double hp = fma(Tc, fma(Tc, fma(Tc, fma(Tc, cb[3], cb[2]), cb[1]), cb[0]), ca[0]);
+    const double cp = fma(Tc, fma(Tc, fma(Tc, fma(Tc, ca[4], ca[3]), ca[2]), ca[1]), ca[0]);
+    vtab[(vt_h(N) + s) * C + idx] = th.Rs[s] * fma(cp, Tk - Tc, fma(Tc, hp, ca[5]));
+  }
   // ---- Wilke's rule (Eq. 22), once for mu and once for kappa: sqrt(a_s / a_t) = sqrt(a_s) / sqrt(a_t)
 #pragma unroll 1
   for (int which = 0; which < 2; ++which) {
-    double a[NS], sq[NS], isq[NS];
-#pragma unroll
-    for (int s = 0; s < NS; ++s)
-      if (s < N) {
-        a[s] = fit_eval(which == 0 ? tr->mu[s] : tr->kappa[s], lnT);
-        sq[s] = sqrt(a[s]);
-        isq[s] = 1.0 / sq[s];
-      }
+    for (int s = 0; s < N; ++s) {
+      const double v = fit_eval(which == 0 ? tr->mu[s] : tr->kappa[s], lnT);
+      const double ir = rsqrt(v);
+      AT(a, s) = v;
+      AT(sq, s) = v * ir;
+      AT(isq, s) = ir;
+    }
     double mix = 0.0;
-#pragma unroll
-    for (int s = 0; s < NS; ++s)
-      if (s < N) {
-        double den = 0.0;
-#pragma unroll
-        for (int t = 0; t < NS; ++t)
-          if (t < N) {
-            const double bb = fma(sq[s] * isq[t], tr->q4[s][t], 1.0);
-            den = fma(X[t] * tr->w8[s][t], bb * bb, den);
-          }
-        mix += X[s] * a[s] / den;
+#pragma unroll 1
+    for (int s = 0; s < N; ++s) {
+      double dn = 0.0;
+      const double sqs = AT(sq, s);
+#pragma unroll 5
+      for (int t = 0; t < N; ++t) {
+        const double bb = fma(sqs * AT(isq, t), tr->q4[s][t], 1.0);
+        dn = fma(AT(X, t) * tr->w8[s][t], bb * bb, dn);
       }
+      mix = fma(AT(X, s) * AT(a, s), xf_rcp(dn), mix);
+    }
     vtab[(which == 0 ? VT_MU : VT_KAPPA) * C + idx] = mix;
   }
   // ---- rho D_sm (Eq. 26 with X_t + 1e-12, reading R20; D_st(T, p) = D_st(T, p_ref) p_ref / p, reading R19)
-  double num[NS], den[NS];
-#pragma unroll
-  for (int s = 0; s < NS; ++s) num[s] = den[s] = 0.0;
+  for (int s = 0; s < N; ++s) AT(num, s) = AT(den, s) = 0.0;
   const double pscale = p / tr->p_ref;
-#pragma unroll
-  for (int s = 0; s < NS; ++s)
-#pragma unroll
-    for (int t = s + 1; t < NS; ++t)
-      if (t < N) {
-        const double invD = pscale / fit_eval(tr->D[s][t], lnT);   // 1 / D_st, symmetric
-        const double xs = X[s] + 1e-12, xt = X[t] + 1e-12;
-        num[s] = fma(xt, tr->W[t], num[s]);
-        num[t] = fma(xs, tr->W[s], num[t]);
-        den[s] = fma(xt, invD, den[s]);
-        den[t] = fma(xs, invD, den[t]);
-      }
-#pragma unroll
-  for (int s = 0; s < NS; ++s)
-    if (s < N) vtab[(vt_rd(N) + s) * C + idx] = N > 1 ? rho * num[s] / (Wbar * den[s]) : 0.0;
+#pragma unroll 1
+  for (int s = 0; s < N; ++s) {
+    const double xs = AT(X, s) + 1e-12, Ws = tr->W[s];
+    double ns = AT(num, s), ds = AT(den, s);
+#pragma unroll 3
+    for (int t = s + 1; t < N; ++t) {
+      const double *c = tr->D[s][t];
+      const double invD = pscale * exp(-fma(lnT, fma(lnT, fma(lnT, c[3], c[2]), c[1]), c[0]));   // 1 / D_st, symmetric
+      const double xt = AT(X, t) + 1e-12;
+      ns = fma(xt, tr->W[t], ns);
+      ds = fma(xt, invD, ds);
+      AT(num, t) = fma(xs, Ws, AT(num, t));
+      AT(den, t) = fma(xs, invD, AT(den, t));
+    }
+    vtab[(vt_rd(N) + s) * C + idx] = N > 1 ? rho * ns * xf_rcp(Wbar * ds) : 0.0;
+  }
+#undef AT
 }
 
 __device__ __forceinline__ double interp4(double m1, double a, double b, double p2) {
@@ -274,9 +274,12 @@ int launch_dir(const XfGrid &G, int N, const ViscArgs &A, cudaStream_t s) {
 
 int xf_launch_transport(const XfGrid &G, const XfThermo &Th, const XfTransportDev *tr_dev, const double *U, const double *T,
                         double *vtab, cudaStream_t s) {
-  const int threads = 128;
+  const int threads = TR_THREADS;
   const unsigned blocks = (unsigned)((G.cells + threads - 1) / threads);
-#define CALL(NT) transport_kernel<NT><<<blocks, threads, 0, s>>>(G, Th, tr_dev, U, T, vtab)
+  const size_t smem = sizeof(double) * 4 * (size_t)Th.N * TR_THREADS;   // N = 16: 64 KB
+#define CALL(NT)                                                                                                   \
+  cudaFuncSetAttribute(transport_kernel<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(double) * 4 * XF_MAXN * TR_THREADS)); \
+  transport_kernel<NT><<<blocks, threads, smem, s>>>(G, Th, tr_dev, U, T, vtab)
   XF_DISPATCH_N(Th.N, CALL)
 #undef CALL
   return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
