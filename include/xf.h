@@ -43,7 +43,8 @@ enum {
   XF_ENOCONV = -5       /* Newton iteration hit newton_maxit                                 */
 };
 
-enum { XF_BC_PERIODIC = 0, XF_BC_TRANSMISSIVE = 1, XF_BC_REFLECTIVE = 2, XF_BC_DIRICHLET = 3 };
+enum { XF_BC_PERIODIC = 0, XF_BC_TRANSMISSIVE = 1, XF_BC_REFLECTIVE = 2, XF_BC_DIRICHLET = 3,
+       XF_BC_EXCHANGE = 4 /* the face borders another block: its ghosts come from the halo exchange below */ };
 
 #define XF_MAX_SPECIES 16
 
@@ -134,6 +135,27 @@ int xf_convective_rhs(xf_ctx *ctx, double *U, double *T, double *rhs, void *work
  * With a transport table the three RK3 entry points integrate L = convective + viscous residual (the viscous part is
  * evaluated first, into the partial-residual buffer the sweeps accumulate on); xf_convective_rhs stays convective. */
 int xf_viscous_rhs(xf_ctx *ctx, const double *U, const double *T, double *rhs, void *work, void *stream);
+
+/* Domain decomposition (Cartesian blocks, one per GPU, the border layers of a block become the
+ * boundary layers of its face neighbour).  A face of kind XF_BC_EXCHANGE is left alone by the ghost fill.  Per residual
+ * evaluation the driver (paper_2403_05910_b200/halo.py) goes through the directions in order x, y, z and, for each:
+ * xf_fill_ghosts_dir (the physical faces of that direction), xf_pack_halo of its exchange faces, the transfer (NCCL
+ * send / recv, or a device copy between blocks of one process), xf_unpack_halo -- each over the padded extent of the
+ * directions already done, so edges and corners arrive without diagonal messages.  Then xf_rk3_stage, which evaluates the
+ * residual of Uin WITHOUT filling ghosts and writes stage `stage` (0, 1, 2) of Eq. 16: Uout = alpha Un + beta (Uin + dt
+ * L(Uin)); stage 0: Uin = Un; the caller owns the stage arrays.  dt comes from the max over blocks of xf_max_wavespeed.
+ *   xf_halo_doubles  size of one face buffer of direction dir: (Nv + 1) x ng x (transverse cells, padded for
+ *                    directions < dir)
+ *   buffers          caller-owned device memory, layout [Nv + 1][ng][transverse]: U and, as the last field, T (the Newton
+ *                    guess of a ghost cell is then the one of the cell it mirrors, and a decomposed run reproduces the
+ *                    single-block run bit for bit); pack: the ng interior layers next to the face (side 0 = low,
+ *                    1 = high); unpack: the ng ghost layers beyond it. */
+int xf_fill_ghosts_dir(xf_ctx *ctx, double *U, int dir, void *stream);
+size_t xf_halo_doubles(const xf_ctx *ctx, int dir);
+int xf_pack_halo(xf_ctx *ctx, const double *U, const double *T, int dir, int side, double *buf, void *stream);
+int xf_unpack_halo(xf_ctx *ctx, double *U, double *T, int dir, int side, const double *buf, void *stream);
+int xf_rk3_stage(xf_ctx *ctx, int stage, const double *Un, double *Uin, double *Uout, double *T, double dt, void *work,
+                 void *stream);
 
 /* The time step assumed by the positivity limiter of a bare xf_convective_rhs (see xf_config.positivity); dt >= 0. */
 int xf_set_rhs_dt(xf_ctx *ctx, double dt);

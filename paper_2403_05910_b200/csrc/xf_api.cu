@@ -98,9 +98,9 @@ int count_active(const XfGrid &G) { return (G.n[0] > 1) + (G.n[1] > 1) + (G.n[2]
 // ghosts -> primitives -> sweeps.  E_last describes what the LAST active sweep writes (residual or RK combine);
 // earlier sweeps accumulate the partial residual in `acc`.
 int residual(xf_ctx *c, double *U, double *T, void *work, double *acc, const XfEpilogue &E_last, cudaStream_t s,
-             double *S_out = nullptr, bool with_stage_buffers = false) {
-  int rc;
-  {
+             double *S_out = nullptr, bool with_stage_buffers = false, bool skip_fill = false) {
+  int rc = XF_OK;
+  if (!skip_fill) {   // xf_rk3_stage: the caller has filled / exchanged the ghosts itself
     Timed t(c, XF_K_GHOST, s);
     rc = xf_launch_ghosts(c->G, c->Nv, c->bc, c->bc_state_dev, U, s, &c->launches);
   }
@@ -236,7 +236,7 @@ int xf_create(xf_ctx **out, const xf_config *cfg) {
     if (n[d] < ng) return XF_EINVAL;  // ghost layers are copies of interior layers: need >= ng of them
     for (int side = 0; side < 2; ++side) {
       const int b = cfg->bc[2 * d + side];
-      if (b < XF_BC_PERIODIC || b > XF_BC_DIRICHLET) return XF_EINVAL;
+      if (b < XF_BC_PERIODIC || b > XF_BC_EXCHANGE) return XF_EINVAL;
       if (b == XF_BC_DIRICHLET && !cfg->bc_state) return XF_EINVAL;
     }
     if ((cfg->bc[2 * d] == XF_BC_PERIODIC) != (cfg->bc[2 * d + 1] == XF_BC_PERIODIC)) return XF_EINVAL;
@@ -393,6 +393,54 @@ int xf_convective_rhs(xf_ctx *c, double *U, double *T, double *rhs, void *work, 
   E.mode = 0;
   E.out = rhs;
   return residual(c, U, T, work, rhs, E, static_cast<cudaStream_t>(stream));
+}
+
+int xf_fill_ghosts_dir(xf_ctx *c, double *U, int dir, void *stream) {
+  if (!c || !U || dir < 0 || dir > 2) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  return xf_launch_ghosts(c->G, c->Nv, c->bc, c->bc_state_dev, U, static_cast<cudaStream_t>(stream), &c->launches, dir);
+}
+
+size_t xf_halo_doubles(const xf_ctx *c, int dir) {
+  return c && dir >= 0 && dir <= 2 ? (size_t)xf_halo_count(c->G, c->Nv, dir) : 0;
+}
+
+int xf_pack_halo(xf_ctx *c, const double *U, const double *T, int dir, int side, double *buf, void *stream) {
+  if (!c || !U || !T || !buf || dir < 0 || dir > 2 || side < 0 || side > 1 || c->G.n[dir] == 1) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  ++c->launches;
+  return xf_launch_halo(c->G, c->Nv, dir, side, true, const_cast<double *>(U), const_cast<double *>(T), buf,
+                        static_cast<cudaStream_t>(stream));
+}
+
+int xf_unpack_halo(xf_ctx *c, double *U, double *T, int dir, int side, const double *buf, void *stream) {
+  if (!c || !U || !T || !buf || dir < 0 || dir > 2 || side < 0 || side > 1 || c->G.n[dir] == 1) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  ++c->launches;
+  return xf_launch_halo(c->G, c->Nv, dir, side, false, U, T, const_cast<double *>(buf), static_cast<cudaStream_t>(stream));
+}
+
+int xf_rk3_stage(xf_ctx *c, int stage, const double *Un, double *Uin, double *Uout, double *T, double dt, void *work,
+                 void *stream) {
+  if (!c || !Un || !Uin || !Uout || !T || !work || stage < 0 || stage > 2 || !(dt > 0.0) || isinf(dt)) return XF_EINVAL;
+  Range r("xf_rk3_stage");
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  const size_t n = (size_t)c->G.cells;
+  double *acc = static_cast<double *>(work) + (size_t)(c->N + 4) * n + 2 * (size_t)c->Nv * n;   // as in xf_rk3_step
+  static const double al[3] = {0.0, 0.75, 1.0 / 3.0}, be[3] = {1.0, 0.25, 2.0 / 3.0};   // Eq. 16
+  XfEpilogue E;
+  memset(&E, 0, sizeof(E));
+  E.mode = 2;
+  E.dt = dt;
+  E.Un = Un;
+  E.alpha = al[stage];
+  E.beta = be[stage];
+  E.out = Uout;
+  return residual(c, Uin, T, work, acc, E, static_cast<cudaStream_t>(stream), nullptr, true, true);
 }
 
 int xf_viscous_rhs(xf_ctx *c, const double *U, const double *T, double *rhs, void *work, void *stream) {

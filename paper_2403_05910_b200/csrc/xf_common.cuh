@@ -98,8 +98,12 @@ int xf_launch_prim(const XfGrid &G, const XfThermo &Th, const double *U, double 
                    cudaStream_t s);
 int xf_launch_wavespeed(const XfGrid &G, const XfThermo &Th, const double *U, double *T, double *S_dev, int *status,
                         cudaStream_t s);
+// only_dir >= 0: that direction alone (the halo exchange interleaves fill and exchange direction by direction)
 int xf_launch_ghosts(const XfGrid &G, int Nv, const XfBc &bc, const double *bc_state_dev, double *U, cudaStream_t s,
-                     long *launches);
+                     long *launches, int only_dir = -1);
+// halo exchange (xf_halo.cu): doubles per face buffer of direction d; pack (U -> buf) / unpack (buf -> U) of one face
+long long xf_halo_count(const XfGrid &G, int Nv, int d);
+int xf_launch_halo(const XfGrid &G, int Nv, int d, int side, bool pack, double *U, double *T, double *buf, cudaStream_t s);
 int xf_launch_sweep_x(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,
                       XfTmapCache *tc, cudaStream_t s);
 int xf_launch_sweep_y(const XfGrid &G, int N, const double *U, const double *prim, const XfEpilogue &E, int *status,

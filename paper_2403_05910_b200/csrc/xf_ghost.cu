@@ -39,6 +39,7 @@ ghost_kernel(const XfGrid G, int Nv, int d, int bc_lo, int bc_hi, const double *
   const int p2 = lo[a2] + (int)(tr / ext[a1]);
   const int n = G.n[d], g = G.g[d];
   const int bc = side == 0 ? bc_lo : bc_hi;
+  if (bc == XF_BC_EXCHANGE) return;   // filled by the halo exchange with the neighbouring block (xf_halo.cu)
   const int ighost = side == 0 ? g - 1 - l : g + n + l;
   int isrc = ighost;
   if (bc == XF_BC_PERIODIC) isrc = side == 0 ? ighost + n : ighost - n;
@@ -75,9 +76,10 @@ ghost_kernel(const XfGrid G, int Nv, int d, int bc_lo, int bc_hi, const double *
 }  // namespace
 
 int xf_launch_ghosts(const XfGrid &G, int Nv, const XfBc &bc, const double *bc_state_dev, double *U, cudaStream_t s,
-                     long *launches) {
+                     long *launches, int only_dir) {
   for (int d = 0; d < 3; ++d) {
-    if (G.n[d] == 1) continue;
+    if (G.n[d] == 1 || (only_dir >= 0 && d != only_dir)) continue;
+    if (bc.kind[2 * d] == XF_BC_EXCHANGE && bc.kind[2 * d + 1] == XF_BC_EXCHANGE) continue;
     long long ntrans = 1;
     for (int q = 0; q < 3; ++q)
       if (q != d) ntrans *= (q < d ? G.np[q] : G.n[q]);

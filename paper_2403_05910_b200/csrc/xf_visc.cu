@@ -133,13 +133,17 @@ struct ViscArgs {
   int seg;                 // cells along d per block
 };
 
+#ifndef XF_VISC_LT
+#define XF_VISC_LT 16   // lanes along i of a y / z tile (a warp = two rows of 128 bytes)
+#define XF_VISC_MINB 3
+#endif
 // DIR = 0: block = LDF threads along i, one face each, LDF - 3 cells; DIR = 1, 2: block = 32 lanes along i x LDF face rows
 template <int N_T, int DIR, int LDF>
-__global__ void __launch_bounds__(DIR == 0 ? LDF : 32 * LDF)
+__global__ void __launch_bounds__(DIR == 0 ? LDF : XF_VISC_LT * LDF, XF_VISC_MINB)
 visc_dir_kernel(const XfGrid G, const int Nrt, const ViscArgs A) {
   constexpr int NS = N_T > 0 ? N_T : XF_MAXN;
   const int N = N_T > 0 ? N_T : Nrt, Nv = N + 4;
-  constexpr int LT = DIR == 0 ? 1 : 32, LD = LDF - 3;
+  constexpr int LT = DIR == 0 ? 1 : XF_VISC_LT, LD = LDF - 3;
   extern __shared__ double fs[];                                  // [Nv - 1][LDF][LT]
   const long long C = G.cells;
   const int k = DIR == 0 ? threadIdx.x : threadIdx.y;             // face index within the tile
@@ -152,7 +156,7 @@ visc_dir_kernel(const XfGrid G, const int Nrt, const ViscArgs A) {
     j2 = 0;
   } else {
     c0 = blockIdx.y * LD;
-    i = blockIdx.x * 32 + lt;
+    i = blockIdx.x * LT + lt;
     j2 = blockIdx.z;
   }
   const bool lane_ok = DIR == 0 || i < G.n[0];
@@ -256,14 +260,14 @@ template <int NT, int DIR>
 int launch_dir(const XfGrid &G, int N, const ViscArgs &A, cudaStream_t s) {
   constexpr int LDF = DIR == 0 ? LDF_X : LDF_YZ, LD = LDF - 3;
   const int OD = DIR == 1 ? 2 : 1;
-  const dim3 block = DIR == 0 ? dim3(LDF) : dim3(32, LDF);
+  const dim3 block = DIR == 0 ? dim3(LDF) : dim3(XF_VISC_LT, LDF);
   const dim3 grid = DIR == 0 ? dim3((G.n[0] + LD - 1) / LD, G.n[1], G.n[2])
-                             : dim3((G.n[0] + 31) / 32, (G.n[DIR] + LD - 1) / LD, G.n[OD]);
-  const size_t smem = sizeof(double) * (size_t)(N + 3) * LDF * (DIR == 0 ? 1 : 32);
+                             : dim3((G.n[0] + XF_VISC_LT - 1) / XF_VISC_LT, (G.n[DIR] + LD - 1) / LD, G.n[OD]);
+  const size_t smem = sizeof(double) * (size_t)(N + 3) * LDF * (DIR == 0 ? 1 : XF_VISC_LT);
   static bool attr_done = false;
   if (!attr_done) {
     cudaFuncSetAttribute(visc_dir_kernel<NT, DIR, LDF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                         (int)(sizeof(double) * (XF_MAXN + 3) * LDF * (DIR == 0 ? 1 : 32)));
+                         (int)(sizeof(double) * (XF_MAXN + 3) * LDF * (DIR == 0 ? 1 : XF_VISC_LT)));
     attr_done = true;
   }
   visc_dir_kernel<NT, DIR, LDF><<<grid, block, smem, s>>>(G, N, A);

@@ -17,7 +17,7 @@ _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libxf.so"
 
 XF_OK, XF_EINVAL, XF_ECUDA, XF_ENOMEM, XF_ENONPHYSICAL, XF_ENOCONV = 0, -1, -2, -3, -4, -5
-XF_BC_PERIODIC, XF_BC_TRANSMISSIVE, XF_BC_REFLECTIVE, XF_BC_DIRICHLET = 0, 1, 2, 3
+XF_BC_PERIODIC, XF_BC_TRANSMISSIVE, XF_BC_REFLECTIVE, XF_BC_DIRICHLET, XF_BC_EXCHANGE = 0, 1, 2, 3, 4
 XF_VISC_LLF, XF_VISC_ROE, XF_VISC_GLF = 0, 1, 2
 XF_RECON_WENO5, XF_RECON_WENOCU6, XF_RECON_WENO7 = 0, 1, 2
 XF_MAX_SPECIES = 16
@@ -26,7 +26,8 @@ XF_MAX_SPECIES = 16
 ABI_SYMBOLS = (
     "xf_create", "xf_destroy", "xf_num_vars", "xf_padded_cells", "xf_rhs_workspace_bytes", "xf_workspace_bytes",
     "xf_fill_ghosts", "xf_primitives", "xf_convective_rhs", "xf_rk3_step", "xf_rk3_step_cfl", "xf_step_cfl",
-    "xf_max_wavespeed", "xf_set_rhs_dt", "xf_viscous_rhs",
+    "xf_max_wavespeed", "xf_set_rhs_dt", "xf_viscous_rhs", "xf_fill_ghosts_dir", "xf_halo_doubles", "xf_pack_halo",
+    "xf_unpack_halo", "xf_rk3_stage",
     "xf_status", "xf_newton_mean_iterations", "xf_launch_count", "xf_convective_rhs_host", "xf_rk3_steps_host",
     "xf_probe_fp64_peak", "xf_probe_fp64_sustained", "xf_strerror", "xf_timing_enable", "xf_timing_read",
 )
@@ -75,6 +76,12 @@ def lib() -> C.CDLL:
         L.xf_convective_rhs.argtypes = [ctx, dp, dp, dp, vp, vp]
         L.xf_set_rhs_dt.argtypes = [ctx, C.c_double]
         L.xf_viscous_rhs.argtypes = [ctx, dp, dp, dp, vp, vp]
+        L.xf_fill_ghosts_dir.argtypes = [ctx, dp, C.c_int, vp]
+        L.xf_halo_doubles.argtypes = [ctx, C.c_int]
+        L.xf_halo_doubles.restype = C.c_size_t
+        L.xf_pack_halo.argtypes = [ctx, dp, dp, C.c_int, C.c_int, dp, vp]
+        L.xf_unpack_halo.argtypes = [ctx, dp, dp, C.c_int, C.c_int, dp, vp]
+        L.xf_rk3_stage.argtypes = [ctx, C.c_int, dp, dp, dp, dp, C.c_double, vp, vp]
         L.xf_rk3_step.argtypes = [ctx, dp, dp, C.c_double, vp, vp]
         L.xf_rk3_step_cfl.argtypes = [ctx, dp, dp, C.c_double, dp, vp, vp]
         L.xf_step_cfl.argtypes = [ctx, dp, dp, C.c_double, dp, vp, vp]
@@ -233,6 +240,26 @@ class Context:
         assert work.numel() * work.element_size() >= self.rhs_workspace_bytes
         _check(lib().xf_convective_rhs(self._h, _ptr(U), _ptr(T), _ptr(rhs), _ptr(work), _stream(stream)),
                "xf_convective_rhs")
+
+    def xf_fill_ghosts_dir(self, U, d: int, stream=None) -> None:
+        _check(lib().xf_fill_ghosts_dir(self._h, _ptr(U), int(d), _stream(stream)), "xf_fill_ghosts_dir")
+
+    def xf_halo_doubles(self, d: int) -> int:
+        return int(lib().xf_halo_doubles(self._h, int(d)))
+
+    def xf_pack_halo(self, U, T, d: int, side: int, buf, stream=None) -> None:
+        assert buf.numel() >= self.xf_halo_doubles(d)
+        _check(lib().xf_pack_halo(self._h, _ptr(U), _ptr(T), int(d), int(side), _ptr(buf), _stream(stream)), "xf_pack_halo")
+
+    def xf_unpack_halo(self, U, T, d: int, side: int, buf, stream=None) -> None:
+        assert buf.numel() >= self.xf_halo_doubles(d)
+        _check(lib().xf_unpack_halo(self._h, _ptr(U), _ptr(T), int(d), int(side), _ptr(buf), _stream(stream)),
+               "xf_unpack_halo")
+
+    def xf_rk3_stage(self, stage: int, Un, Uin, Uout, T, dt: float, work, stream=None) -> None:
+        assert work.numel() * work.element_size() >= self.workspace_bytes
+        _check(lib().xf_rk3_stage(self._h, int(stage), _ptr(Un), _ptr(Uin), _ptr(Uout), _ptr(T), float(dt), _ptr(work),
+                                  _stream(stream)), "xf_rk3_stage")
 
     def xf_viscous_rhs(self, U, T, rhs, work, stream=None) -> None:
         assert work.numel() * work.element_size() >= self.rhs_workspace_bytes
