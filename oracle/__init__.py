@@ -5,4 +5,4 @@ import this package.  The product (``paper_2403_05910_b200``) never does, and th
 The arithmetic lives in ``xf_oracle.c`` (plain C, fp64, ``-O2 -ffp-contract=off``); this file only builds it
 with gcc, loads it with ctypes and marshals numpy arrays.
 """
-from .oracle import Oracle, build, lib, OPrim, OConfig, OTransport, make_transport, weno5, wenocu6, weno7  # noqa: F401
+from .oracle import Oracle, build, lib, OPrim, OConfig, OTransport, make_transport, OMechanism, make_mechanism, weno5, wenocu6, weno7  # noqa: F401

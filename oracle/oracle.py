@@ -47,6 +47,29 @@ def make_transport(tr) -> OTransport:
     return o
 
 
+MAXR = 64
+
+
+class OMechanism(C.Structure):
+    _fields_ = [("NR", C.c_int), ("nu_r", (C.c_int * MAXN) * MAXR), ("nu_p", (C.c_int * MAXN) * MAXR),
+                ("A", C.c_double * MAXR), ("B", C.c_double * MAXR), ("E", C.c_double * MAXR),
+                ("third", C.c_int * MAXR), ("eff", (C.c_double * MAXN) * MAXR), ("p_atm", C.c_double)]
+
+
+def make_mechanism(m) -> OMechanism:
+    """m: workloads.Mechanism (nu_r, nu_p [NR,N] int, A, B, E [NR], third [NR], eff [NR,N], p_atm)"""
+    o = OMechanism()
+    nr, n = m.nu_r.shape
+    assert nr <= MAXR
+    o.NR = nr
+    for r in range(nr):
+        o.A[r], o.B[r], o.E[r], o.third[r] = float(m.A[r]), float(m.B[r]), float(m.E[r]), int(m.third[r])
+        for s in range(n):
+            o.nu_r[r][s], o.nu_p[r][s], o.eff[r][s] = int(m.nu_r[r, s]), int(m.nu_p[r, s]), float(m.eff[r, s])
+    o.p_atm = float(m.p_atm)
+    return o
+
+
 class OPrim(C.Structure):
     _fields_ = [
         ("rho", C.c_double), ("vel", C.c_double * 3), ("Y", C.c_double * MAXN), ("e", C.c_double),
@@ -111,6 +134,13 @@ def lib():
         L.xo_rk3_step.argtypes = [cp, dp, dp, C.c_double]
         L.xo_max_wavespeed.argtypes = [cp, dp, dp, C.POINTER(C.c_int)]
         L.xo_max_wavespeed.restype = C.c_double
+        mp = C.POINTER(OMechanism)
+        L.xo_qss_alpha.argtypes = [C.c_double]
+        L.xo_qss_alpha.restype = C.c_double
+        L.xo_reaction_rates.argtypes = [cp, mp, C.c_double, dp, C.c_double, dp, dp]
+        L.xo_reaction_rates.restype = None
+        L.xo_react_cell.argtypes = [cp, mp, dp, dp, C.c_double, C.c_int, C.c_int]
+        L.xo_react.argtypes = [cp, mp, dp, dp, C.c_double, C.c_int, C.c_int]
         tp = C.POINTER(OTransport)
         L.xo_transport_cell.argtypes = [cp, tp, C.c_double, dp, C.c_double, dp, dp, dp, dp]
         L.xo_transport_cell.restype = None
@@ -318,6 +348,25 @@ class Oracle:
     def rk3_step_ns(self, tr: OTransport, U, T, dt: float) -> int:
         self._chk(U, T)
         return lib().xo_rk3_step_ns(C.byref(self.cfg), C.byref(tr), _dp(U), _dp(T), float(dt))
+
+    # ---- reaction step (xf_oracle.h: readings R24-R30); m = make_mechanism(workloads.Mechanism) ----
+    def reaction_rates(self, m: OMechanism, rho: float, Y, T: float):
+        """-> (q [N], d [N]): production and destruction rates of Y_s"""
+        Y = np.ascontiguousarray(Y, dtype=np.float64)
+        q, d = np.zeros(self.N), np.zeros(self.N)
+        lib().xo_reaction_rates(C.byref(self.cfg), C.byref(m), float(rho), _dp(Y), float(T), _dp(q), _dp(d))
+        return q, d
+
+    def react_cell(self, m: OMechanism, Ucell, T: float, dt: float, n_sub: int = 1, n_corr: int = 1):
+        """-> (status, Ucell after the reaction step, T)"""
+        Uc = np.array(Ucell, dtype=np.float64)
+        Tk = np.array([T], dtype=np.float64)
+        st = lib().xo_react_cell(C.byref(self.cfg), C.byref(m), _dp(Uc), _dp(Tk), float(dt), int(n_sub), int(n_corr))
+        return st, Uc, float(Tk[0])
+
+    def react(self, m: OMechanism, U, T, dt: float, n_sub: int = 1, n_corr: int = 1) -> int:
+        self._chk(U, T)
+        return lib().xo_react(C.byref(self.cfg), C.byref(m), _dp(U), _dp(T), float(dt), int(n_sub), int(n_corr))
 
     def max_wavespeed(self, U, T) -> float:
         self._chk(U, T)

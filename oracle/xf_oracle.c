@@ -915,3 +915,155 @@ double xo_max_wavespeed(const xo_config *c, const double *U, double *T, int *sta
   if (status_out) *status_out = status;
   return S;
 }
+
+/* ------------------------------------------------------------------------------------------------------------ */
+/* Reaction step: alpha-QSS predictor-corrector (Eq. 8-12; 180-198 Eq. 27-28; readings R24-R30)      */
+/* ------------------------------------------------------------------------------------------------------------ */
+double xo_qss_alpha(double r) {
+  if (r < 0.1) {   /* alpha = 1/(1 - e^-r) - 1/r = 1/2 + r/12 - r^3/720 + r^5/30240 - r^7/1209600 + O(r^9) */
+    const double r2 = r * r;
+    return 0.5 + r * (1.0 / 12.0 - r2 * (1.0 / 720.0 - r2 * (1.0 / 30240.0 - r2 / 1209600.0)));
+  }
+  const double em = 1.0 - exp(-r);
+  return (1.0 - em / r) / em;
+}
+
+static double ipow(double x, int n) {
+  double y = 1.0;
+  for (int k = 0; k < n; ++k) y *= x;
+  return y;
+}
+
+void xo_reaction_rates(const xo_config *c, const xo_mechanism *m, double rho, const double *Y, double T, double *q,
+                       double *d) {
+  const int N = c->N;
+  double conc[XO_MAXN], g0[XO_MAXN];              /* [X_s]; S_s/R_s - h_s/(R_s T) */
+  double Tc = T;
+  if (Tc < c->Tlo) Tc = c->Tlo;
+  if (Tc > c->Thi) Tc = c->Thi;
+  for (int s = 0; s < N; ++s) {
+    conc[s] = rho * Y[s] / c->W[s];
+    const double *a = c->a[s];
+    double cp, h, e;
+    xo_species_thermo(c, s, T, &cp, &h, &e);
+    const double Rs = c->Ru / c->W[s];
+    const double SR = a[0] * log(Tc) + Tc * (a[1] + Tc * (a[2] / 2.0 + Tc * (a[3] / 3.0 + Tc * a[4] / 4.0))) + a[6] +
+                      (cp / Rs) * log(T / Tc);
+    g0[s] = SR - h / (Rs * T);
+    q[s] = 0.0;
+    d[s] = 0.0;
+  }
+  for (int r = 0; r < m->NR; ++r) {
+    const double kf = m->A[r] * pow(T, m->B[r]) * exp(-m->E[r] / (c->Ru * T));     /* Eq. 11 (reading R24) */
+    int dnu = 0;
+    double dg = 0.0;
+    for (int s = 0; s < N; ++s) {
+      const int nu = m->nu_p[r][s] - m->nu_r[r][s];                               /* Eq. 10 */
+      dnu += nu;
+      dg += nu * g0[s];
+    }
+    const double Kc = pow(m->p_atm / (c->Ru * T), (double)dnu) * exp(dg);         /* Eq. 12 */
+    const double kb = kf / Kc;
+    double tb = 1.0;
+    if (m->third[r]) {
+      tb = 0.0;
+      for (int s = 0; s < N; ++s) tb += m->eff[r][s] * conc[s];
+    }
+    double Rf = tb * kf, Rb = tb * kb;
+    for (int s = 0; s < N; ++s) {
+      Rf *= ipow(conc[s], m->nu_r[r][s]);
+      Rb *= ipow(conc[s], m->nu_p[r][s]);
+    }
+    for (int s = 0; s < N; ++s) {                                                 /* Eq. 9 split as Eq. 27 (reading R25) */
+      const double w = c->W[s] / rho;
+      q[s] += w * (m->nu_p[r][s] * Rf + m->nu_r[r][s] * Rb);
+      d[s] += w * (m->nu_r[r][s] * Rf + m->nu_p[r][s] * Rb);
+    }
+  }
+}
+
+/* temperature from the fixed internal energy e and the composition Y (C2's Newton iteration) */
+static int T_of_e(const xo_config *c, const double *Y, double e, double *T) {
+  double Tk = *T;
+  for (int k = 0; k < c->maxit; ++k) {
+    double Rbar, eT, Cv;
+    xo_mixture(c, Y, Tk, &Rbar, &eT, &Cv);
+    const double Tn = Tk + (e - eT) / Cv;
+    const double dT = fabs(Tn - Tk);
+    Tk = Tn;
+    if (dT <= c->rtol * fabs(Tn)) { *T = Tk; return 0; }
+    if (!(Tn == Tn)) break;
+  }
+  *T = Tk;
+  return XO_ENOCONV;
+}
+
+int xo_react_cell(const xo_config *c, const xo_mechanism *m, double *Uc, double *T, double dt, int n_sub, int n_corr) {
+  const int N = c->N;
+  xo_prim P;
+  memset(&P, 0, sizeof(P));
+  cell_basic(c, Uc, &P);                           /* rho, Y (closure), e: rho and e stay fixed (reading R29) */
+  int status = 0;
+  double Y0[XO_MAXN] = {0}, Yp[XO_MAXN] = {0}, q0[XO_MAXN], d0[XO_MAXN], p0[XO_MAXN] = {0}, qp[XO_MAXN], dp[XO_MAXN];
+  for (int s = 0; s < N; ++s) Y0[s] = P.Y[s];
+  double Tk = *T;
+  status |= T_of_e(c, Y0, P.e, &Tk);
+  const double h = dt / n_sub;
+  for (int sub = 0; sub < n_sub; ++sub) {
+    xo_reaction_rates(c, m, P.rho, Y0, Tk, q0, d0);
+    double sum = 0.0;
+    for (int s = 0; s < N - 1; ++s) {              /* predictor, Eq. 28 */
+      p0[s] = Y0[s] > 0.0 ? d0[s] / Y0[s] : 0.0;
+      const double a0 = xo_qss_alpha(p0[s] * h);
+      Yp[s] = Y0[s] + h * (q0[s] - p0[s] * Y0[s]) / (1.0 + a0 * p0[s] * h);
+      sum += Yp[s];
+    }
+    Yp[N - 1] = 1.0 - sum;
+    double Tp = Tk;
+    for (int it = 0; it < n_corr; ++it) {          /* corrector(s) (reading R27) */
+      status |= T_of_e(c, Yp, P.e, &Tp);
+      xo_reaction_rates(c, m, P.rho, Yp, Tp, qp, dp);
+      sum = 0.0;
+      double Yc[XO_MAXN];
+      for (int s = 0; s < N - 1; ++s) {
+        const double pp = Yp[s] > 0.0 ? dp[s] / Yp[s] : 0.0;
+        const double pb = 0.5 * (p0[s] + pp);
+        const double ab = xo_qss_alpha(pb * h);
+        const double qb = ab * qp[s] + (1.0 - ab) * q0[s];
+        Yc[s] = Y0[s] + h * (qb - pb * Y0[s]) / (1.0 + ab * pb * h);
+        sum += Yc[s];
+      }
+      Yc[N - 1] = 1.0 - sum;
+      for (int s = 0; s < N; ++s) Yp[s] = Yc[s];
+    }
+    for (int s = 0; s < N; ++s) Y0[s] = Yp[s];
+    Tk = Tp;
+    status |= T_of_e(c, Y0, P.e, &Tk);
+  }
+  for (int s = 0; s < N - 1; ++s) Uc[5 + s] = P.rho * Y0[s];
+  *T = Tk;
+  if (!(Tk > 0.0)) status |= XO_ENONPHYSICAL;
+  return status;
+}
+
+int xo_react(const xo_config *c, const xo_mechanism *m, double *U, double *T, double dt, int n_sub, int n_corr) {
+  const int Nv = c->N + 4;
+  int np[3], n[3], g[3];
+  long st[3];
+  grid(c, np, n, g, st);
+  const long cells = xo_padded_cells(c);
+  int status = 0;
+#pragma omp parallel for reduction(| : status) collapse(2) if (cells > 4096)
+  for (int k = g[2]; k < g[2] + n[2]; ++k)
+    for (int j = g[1]; j < g[1] + n[1]; ++j)
+      for (int i = g[0]; i < g[0] + n[0]; ++i) {
+        const long idx = (long)k * st[2] + (long)j * st[1] + i;
+        double Uc[XO_MAXNV];
+        gather_cell(c, U, cells, idx, Uc);
+        double Tk = T[idx];
+        status |= xo_react_cell(c, m, Uc, &Tk, dt, n_sub, n_corr);
+        for (int v = 5; v < Nv; ++v) U[v * cells + idx] = Uc[v];
+        T[idx] = Tk;
+      }
+  return status;
+}

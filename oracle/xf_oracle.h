@@ -158,6 +158,44 @@ int xo_viscous_rhs(const xo_config *c, const xo_transport *tr, const double *U, 
 int xo_rhs_ns(const xo_config *c, const xo_transport *tr, double *U, double *T, double *rhs);
 int xo_rk3_step_ns(const xo_config *c, const xo_transport *tr, double *U, double *T, double dt);
 
+/* ------------------------------------------------------------------------------------------------------------------
+ * Reaction step (Eq. 8-12, Eq. 27-28: the alpha-QSS solver
+ * CHEMEQ2 inside a Lie-Trotter / Strang splitting).  Readings R24-R30 of DESIGN.md:
+ *   R24 Arrhenius law k_f = A T^B exp(-E/(Ru T)) (Eq. 11 prints +E/(Ru T)); K_c by Eq. 12 with S_s/R_s = a1 ln T + a2 T +
+ *       a3 T^2/2 + a4 T^3/3 + a5 T^4/4 + a7 and h_s of C1 (outside the fit range: cp frozen, S continued with cp ln(T/Tc));
+ *       k_b = k_f/K_c; p0 ("1 atm") is an input in the caller's units; molar concentrations [X_s] = rho Y_s / W_s; the
+ *       third-body factor of a third-body reaction is sum_s eff_s [X_s], else 1.
+ *   R25 Eq. 27: dY_s/dt = q_s - p_s Y_s with q_s = (W_s/rho) sum_r (nu''_sr R_f,r + nu'_sr R_b,r) and the destruction rate
+ *       d_s = (W_s/rho) sum_r (nu'_sr R_f,r + nu''_sr R_b,r) = p_s Y_s; p_s = d_s/Y_s (0 where Y_s <= 0).
+ *   R26 Eq. 28 with its alpha repaired: alpha(r) = (1 - (1 - e^-r)/r)/(1 - e^-r), r = p dt -- the value for which the update
+ *       is exact when q and p are constant; for r < 0.1 its series 1/2 + r/12 - r^3/720 + r^5/30240 - r^7/1209600 (the
+ *       closed form cancels there).  Predictor Y^p = Y^0 + dt (q^0 - p^0 Y^0)/(1 + alpha^0 p^0 dt); corrector with pbar = (p^0 + p^p)/2,
+ *       abar = alpha(pbar dt), qbar = abar q^p + (1 - abar) q^0: Y^c = Y^0 + dt (qbar - pbar Y^0)/(1 + abar pbar dt).
+ *   R27 "multiple corrector steps": n_corr >= 1 of them, each re-evaluating the rates at the last corrected state.
+ *   R28 "multiple time steps": n_sub equal sub-steps dt/n_sub (the paper gives no step-size control).
+ *   R29 the reaction step holds rho, rho u and E fixed (constant volume, adiabatic); T follows from e(T, Y) = e by the Newton
+ *       iteration of C2 after every update of Y -- Eq. 8's heat release is then carried by the formation constants of h_s.
+ *   R30 species 1..N-1 are integrated, Y_N = 1 - sum by closure as everywhere else (R1).
+ * ------------------------------------------------------------------------------------------------------------------ */
+#define XO_MAXR 64
+typedef struct {
+  int NR;
+  int nu_r[XO_MAXR][XO_MAXN], nu_p[XO_MAXR][XO_MAXN];   /* nu' (reactants), nu'' (products): small non-negative integers */
+  double A[XO_MAXR], B[XO_MAXR], E[XO_MAXR];            /* Arrhenius parameters of the forward rate                       */
+  int third[XO_MAXR];                                   /* 1: third-body reaction                                         */
+  double eff[XO_MAXR][XO_MAXN];                         /* third-body efficiencies                                        */
+  double p_atm;                                         /* the standard pressure of Eq. 12 in the caller's units          */
+} xo_mechanism;
+
+double xo_qss_alpha(double r);
+/* q[s], d[s] (1/time) of all N species at (rho, Y, T) */
+void xo_reaction_rates(const xo_config *c, const xo_mechanism *m, double rho, const double *Y, double T, double *q,
+                       double *d);
+/* one cell: Ucell in/out (rho Y_s updated), T in (guess) / out; returns status bits */
+int xo_react_cell(const xo_config *c, const xo_mechanism *m, double *Ucell, double *T, double dt, int n_sub, int n_corr);
+/* all interior cells */
+int xo_react(const xo_config *c, const xo_mechanism *m, double *U, double *T, double dt, int n_sub, int n_corr);
+
 #ifdef __cplusplus
 }
 #endif

@@ -674,3 +674,74 @@ def synthetic_transport(table: SpeciesTable, seed: int, mu0: float = 2e-3, T0: f
         for t in range(s + 1, n):
             D[s, t] = D[t, s] = fit(0.5 * (mus[s] + mus[t]) / (rho0 * rng.uniform(0.6, 1.1)), 1.7 + rng.uniform(-0.05, 0.05))
     return TransportFits(mu=mu, kappa=kappa, D=D, p_ref=float(p_ref))
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# a seeded synthetic reaction mechanism (Eq. 8-12)
+# ----------------------------------------------------------------------------------------------------------------
+@dataclass
+class Mechanism:
+    nu_r: np.ndarray          # [NR, N] reactant coefficients nu'
+    nu_p: np.ndarray          # [NR, N] product coefficients nu''
+    A: np.ndarray             # [NR] Arrhenius pre-exponential factor, temperature exponent, activation energy (Eq. 11)
+    B: np.ndarray
+    E: np.ndarray
+    third: np.ndarray         # [NR] 1: third-body reaction
+    eff: np.ndarray           # [NR, N] third-body efficiencies
+    p_atm: float              # the standard pressure of Eq. 12 in the workload's units
+
+
+def reacting_table(seed: int = 0, Ru: float = 8.0):
+    """Eight species built from two elements of mass 1.008 and 16.0 -- compositions (2,0) (0,2) (2,1) (1,0) (0,1) (1,1)
+    (1,2) (2,2) -- plus an inert ninth of mass 28.0: molar masses that conserve mass in every element-balanced reaction.
+    Seeded synthetic NASA-7 coefficients with formation-enthalpy and entropy constants (a6, a7).  -> (table, comp [9, 2])"""
+    comp = np.array([(2, 0), (0, 2), (2, 1), (1, 0), (0, 1), (1, 1), (1, 2), (2, 2), (0, 0)])
+    W = comp @ np.array([1.008, 16.0])
+    W[8] = 28.0
+    rng = np.random.default_rng(SEED_BASE + 900 + seed)
+    table = synthetic_nasa7_table(W, Ru=Ru, rng=rng, formation=False)
+    table.nasa7[:, 5] += rng.uniform(-1500.0, 1500.0, 9) * (np.arange(9) != 8)   # formation enthalpies / R (K)
+    # entropy constants: S_s/R_s = O(1) around 1000 K, so that the equilibrium constants of Eq. 12 are moderate
+    table.nasa7[:, 6] = -table.nasa7[:, 0] * np.log(1000.0) + rng.uniform(-1.0, 1.0, 9)
+    return table, comp
+
+
+def synthetic_mechanism(table: SpeciesTable, comp: np.ndarray, n_reactions: int, seed: int, rate: float = 50.0,
+                        p_atm: Optional[float] = None, T_act: float = 1500.0) -> Mechanism:
+    """Element-balanced reversible reactions drawn at random from ALL the balanced ones of the forms A + B <=> C + D and
+    A + B (+ M) <=> C (+ M) among the reactive species (enumerated from the composition table -- no real mechanism is
+    written out), with seeded Arrhenius parameters: A such that the forward rate is ~ `rate` per unit time at
+    concentration ~ 0.05 and 1000 K, B in [-1, 1], E/Ru in [0, T_act] K; a third of the three-body ones get seeded
+    third-body efficiencies in [0.5, 3]."""
+    rng = np.random.default_rng(SEED_BASE + 950 + seed)
+    n = table.n
+    if p_atm is None:
+        p_atm = table.Ru * 1000.0 * 0.05      # p0/(Ru T) = the typical concentration at 1000 K
+    reactive = [s for s in range(n) if comp[s].sum() > 0]
+    cands = []
+    for i, a in enumerate(reactive):
+        for b in reactive[i:]:
+            lhs = comp[a] + comp[b]
+            for c in reactive:                                    # A + B (+M) <=> C (+M)
+                if c not in (a, b) and np.array_equal(comp[c], lhs):
+                    cands.append(((a, b), (c,), 1))
+            for j, c in enumerate(reactive):                      # A + B <=> C + D
+                for d_ in reactive[j:]:
+                    if {a, b} != {c, d_} and (a, b) < (c, d_) and np.array_equal(comp[c] + comp[d_], lhs):
+                        cands.append(((a, b), (c, d_), 0))
+    pick = rng.permutation(len(cands))[:n_reactions]
+    nr = len(pick)
+    nu_r, nu_p = np.zeros((nr, n), dtype=np.int64), np.zeros((nr, n), dtype=np.int64)
+    third, eff = np.zeros(nr, dtype=np.int64), np.ones((nr, n))
+    A, B, E = np.zeros(nr), rng.uniform(-1.0, 1.0, nr), table.Ru * rng.uniform(0.0, T_act, nr)
+    for r, q in enumerate(pick):
+        lhs, rhs, tb = cands[q]
+        for s in lhs:
+            nu_r[r, s] += 1
+        for s in rhs:
+            nu_p[r, s] += 1
+        third[r] = tb
+        if tb:
+            eff[r] = rng.uniform(0.5, 3.0, n)
+        A[r] = rate / 0.05 / (0.5 if tb else 1.0) * rng.uniform(0.3, 3.0) / (1000.0 ** B[r] * np.exp(-E[r] / (table.Ru * 1000.0)))
+    return Mechanism(nu_r=nu_r, nu_p=nu_p, A=A, B=B, E=E, third=third, eff=eff, p_atm=float(p_atm))

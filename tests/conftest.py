@@ -45,7 +45,7 @@ def oracle_ld(tmp_path_factory, oracle_mod):
     for name in ("xf_oracle.c", "xf_oracle.h"):
         t = (src_dir / name).read_text()
         t = re.sub(r"\bdouble\b", "long double", t)
-        for f in ("sqrt", "fabs", "fmax", "fmin"):
+        for f in ("sqrt", "fabs", "fmax", "fmin", "exp", "log", "pow"):
             t = re.sub(rf"\b{f}\(", f"{f}l(", t)
         t = lit.sub(r"\1L", t)
         (out / name).write_text(t)
