@@ -49,6 +49,7 @@ WORKLOADS = {
     "config3": ("config3_shock_bubble_3d", (256, 256, 256), (128, 128, 128), (96, 96, 96)),
     "config2": ("config2_shock_bubble_2d", (2048, 1024, 1), (1024, 512, 1), (1024, 512, 1)),
     "config5": ("config5_random_states", (640, 384, 384), (128, 128, 128), (96, 96, 96)),
+    "react": ("reacting_box", (256, 128, 128), (64, 32, 32), (64, 32, 32)),
 }
 
 
@@ -316,6 +317,8 @@ def run_b200(args, rank: int, local_rank: int, world: int) -> None:
     grid = tuple(args.grid) if args.grid else WORKLOADS[name][1]
     if name == "config5":
         return run_config5(args, rank, local_rank, world, ranks)
+    if name == "react":
+        return run_react(args, rank, local_rank, world, ranks)
     w = make_workload(name, grid)
     if args.reconstruction == 2:
         from paper_2403_05910_b200 import workloads as wl
@@ -553,6 +556,55 @@ def run_config5(args, rank: int, local_rank: int, world: int, ranks) -> None:
             "step_roofline": {"frac": flops / (peak_tf * 1e12) * 1e3 / ms, "newton_mean_iterations": newton_its,
                               "peak": peak_tf, "peak_source": f"xf_probe_fp64_sustained, {sustained_ms:.0f} ms"},
         }), flush=True)
+    ctx.close()
+    ranks.close()
+
+
+def run_react(args, rank: int, local_rank: int, world: int, ranks) -> None:
+    """The reaction step alone (not the bench line): xf_react over dt with 4 sub-steps of one
+    predictor and one corrector on 256x128x128 cells of the nine-species reacting box, 19-reaction seeded mechanism; the
+    state is restored before every timed call (outside the timed span), so every call does the same work."""
+    import torch
+
+    from paper_2403_05910_b200 import workloads as wl
+    from paper_2403_05910_b200 import xf
+
+    grid = tuple(args.grid) if args.grid else WORKLOADS["react"][1]
+    w = wl.reacting_box(*grid, seed=11)
+    mech = wl.synthetic_mechanism(w.table, wl.reacting_table()[1], 19, seed=19, rate=5.0)
+    ctx = xf.Context.from_workload(w, device=local_rank)
+    ctx.xf_set_mechanism(mech)
+    dev = torch.device("cuda", local_rank)
+    U0, T0 = torch.from_numpy(w.U).to(dev), torch.from_numpy(w.T_guess).to(dev)
+    U, T = U0.clone(), T0.clone()
+    n_sub, dt = 4, 5e-4
+    for _ in range(args.warmup):
+        U.copy_(U0); T.copy_(T0)
+        ctx.xf_react(U, T, dt, n_sub, 1)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank)
+    ranks.barrier()
+    sampler.start()
+    for a, b in ev:
+        U.copy_(U0); T.copy_(T0)
+        a.record()
+        ctx.xf_react(U, T, dt, n_sub, 1)
+        b.record()
+    ranks.barrier()
+    clocks = sampler.stop()
+    ms = ranks.max(sum(float(a.elapsed_time(b)) for a, b in ev)) / args.steps
+    if ctx.xf_status() != 0:
+        raise RuntimeError("reaction step failed")
+    cells = w.interior_cells
+    if rank == 0:
+        print(json.dumps({
+            "metric": "cell reaction steps/s (alpha-QSS, 4 sub-steps x (predictor + corrector) = 8 rate evaluations)",
+            "value": cells * world / (ms * 1e-3), "unit": "cell-steps/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "react", "grid": list(grid), "nspecies": w.nspecies, "reactions": 19, "n_sub": n_sub,
+                       "n_corr": 1, "rate_evaluations_per_cell_per_s": cells * world * 2 * n_sub / (ms * 1e-3)},
+            "clocks": clocks, "gpu_launches": args.steps}), flush=True)
     ctx.close()
     ranks.close()
 

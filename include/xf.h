@@ -47,6 +47,7 @@ enum { XF_BC_PERIODIC = 0, XF_BC_TRANSMISSIVE = 1, XF_BC_REFLECTIVE = 2, XF_BC_D
        XF_BC_EXCHANGE = 4 /* the face borders another block: its ghosts come from the halo exchange below */ };
 
 #define XF_MAX_SPECIES 16
+#define XF_MAX_REACTIONS 64
 
 typedef struct {
   int nx, ny, nz;          /* interior cells; == 1 -> direction inactive (no ghosts, no sweep)                  */
@@ -55,7 +56,8 @@ typedef struct {
   int nspecies;            /* N in 1..XF_MAX_SPECIES; Nv = N + 4                                                */
   double Ru;               /* universal gas constant in the caller's units (Eq. 7)                  */
   const double *W;         /* host [N] molar masses                                                             */
-  const double *nasa7;     /* host [N][7] NASA-7 a1..a7, single range (a7 unused on this path)    */
+  const double *nasa7;     /* host [N][7] NASA-7 a1..a7, single range (a7, the entropy constant, is used by the
+                              reaction step only)                                                   */
   double Tlo, Thi;         /* fit range; constant-cp continuation outside it (reading R3)                       */
   int bc[6];               /* xlo, xhi, ylo, yhi, zlo, zhi: XF_BC_*                                             */
   const double *bc_state;  /* host [6][Nv] conserved states of XF_BC_DIRICHLET faces, or NULL                   */
@@ -136,6 +138,18 @@ int xf_convective_rhs(xf_ctx *ctx, double *U, double *T, double *rhs, void *work
  * evaluated first, into the partial-residual buffer the sweeps accumulate on); xf_convective_rhs stays convective. */
 int xf_viscous_rhs(xf_ctx *ctx, const double *U, const double *T, double *rhs, void *work, void *stream);
 
+/* Reaction step (Eq. 8-12; Eq. 27-28: the alpha-QSS solver CHEMEQ2 inside an operator
+ * splitting; readings R24-R30).  xf_set_mechanism copies a mechanism of n_reactions <= XF_MAX_REACTIONS reversible
+ * reactions into the context: nu_r, nu_p host [NR][N] non-negative integer coefficients of reactants and products (at most
+ * three molecules a side), Arrhenius parameters k_f = A T^B exp(-E/(Ru T)), third[r] != 0 for a third-body reaction with
+ * efficiencies eff [NR][N], p_atm the standard pressure of Eq. 12 in the caller's units; backward rates follow from the
+ * equilibrium constants (NASA-7 entropies: a7 of the table).  xf_react advances the species of every INTERIOR cell over dt
+ * at fixed rho, rho u and E: n_sub equal sub-steps of one predictor and n_corr correctors (Eq. 28), the temperature solved
+ * from the internal energy after every update (T: in guess, out T).  Ghost cells are not touched. */
+int xf_set_mechanism(xf_ctx *ctx, int n_reactions, const int *nu_r, const int *nu_p, const double *A, const double *B,
+                     const double *E, const int *third, const double *eff, double p_atm);
+int xf_react(xf_ctx *ctx, double *U, double *T, double dt, int n_sub, int n_corr, void *stream);
+
 /* Domain decomposition (Cartesian blocks, one per GPU, the border layers of a block become the
  * boundary layers of its face neighbour).  A face of kind XF_BC_EXCHANGE is left alone by the ghost fill.  Per residual
  * evaluation the driver (paper_2403_05910_b200/halo.py) goes through the directions in order x, y, z and, for each:
@@ -195,7 +209,7 @@ long xf_launch_count(const xf_ctx *ctx);
  * resets the record list.  max_records = 0 switches timing off.  The ghost fill (one launch per active direction)
  * is timed as one record. */
 enum { XF_K_GHOST = 0, XF_K_PRIM = 1, XF_K_SWEEP_X = 2, XF_K_SWEEP_Y = 3, XF_K_SWEEP_Z = 4, XF_K_WAVESPEED = 5,
-       XF_K_TRANSPORT = 6, XF_K_VISCOUS = 7, XF_K_COUNT = 8 };
+       XF_K_TRANSPORT = 6, XF_K_VISCOUS = 7, XF_K_REACT = 8, XF_K_COUNT = 9 };
 int xf_timing_enable(xf_ctx *ctx, int max_records);
 int xf_timing_read(xf_ctx *ctx, void *stream, double *ms_out, long *count_out);
 

@@ -12,7 +12,7 @@ CSRC = HERE / "csrc"
 INCLUDE = HERE.parent / "include"
 OBJ = CSRC / "build"
 LIB = HERE / "libxf.so"
-SOURCES = ["xf_api.cu", "xf_prim.cu", "xf_ghost.cu", "xf_sweep_x.cu", "xf_sweep_y.cu", "xf_sweep_z.cu", "xf_probe.cu", "xf_visc.cu", "xf_halo.cu"]
+SOURCES = ["xf_api.cu", "xf_prim.cu", "xf_ghost.cu", "xf_sweep_x.cu", "xf_sweep_y.cu", "xf_sweep_z.cu", "xf_probe.cu", "xf_visc.cu", "xf_halo.cu", "xf_react.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", f"-I{INCLUDE}"]
 

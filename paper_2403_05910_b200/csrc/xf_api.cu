@@ -27,6 +27,8 @@ struct xf_ctx {
   double *lam_glob_dev;               // GLF: [3][3] global maxima of the current residual evaluation
   int visc, recon;                    // XF_VISC_*, XF_RECON_*
   XfTransportDev *tr_dev;             // transport fits (device), or nullptr: no viscous / diffusive terms
+  XfMechDev *mech_dev;                // reaction mechanism (device), or nullptr (xf_set_mechanism)
+  double a7[XF_MAXN], W[XF_MAXN], Ru; // kept for xf_set_mechanism
   int positivity;                     // positivity-preserving flux blending on (Eq. 17-20)
   double rhs_dt;                      // the step the limiter of a bare xf_convective_rhs guards (xf_set_rhs_dt)
   long launches;
@@ -286,6 +288,11 @@ int xf_create(xf_ctx **out, const xf_config *cfg) {
     for (int q = 0; q < 4; ++q) Th.b[s][q] = a[q + 1] / (double)(q + 2);
   }
   for (int q = 0; q < 6; ++q) c->bc.kind[q] = cfg->bc[q];
+  for (int s = 0; s < N; ++s) {
+    c->a7[s] = cfg->nasa7[7 * s + 6];
+    c->W[s] = cfg->W[s];
+  }
+  c->Ru = cfg->Ru;
 
   bool ok = cudaMalloc(&c->status_dev, sizeof(int)) == cudaSuccess &&
             cudaMalloc(&c->itersum_dev, sizeof(unsigned long long)) == cudaSuccess &&
@@ -344,6 +351,7 @@ int xf_destroy(xf_ctx *c) {
   cudaFree(c->S_dev);
   cudaFree(c->lam_glob_dev);
   cudaFree(c->tr_dev);
+  cudaFree(c->mech_dev);
   cudaFree(c->hU);
   cudaFree(c->hT);
   cudaFree(c->hR);
@@ -393,6 +401,55 @@ int xf_convective_rhs(xf_ctx *c, double *U, double *T, double *rhs, void *work, 
   E.mode = 0;
   E.out = rhs;
   return residual(c, U, T, work, rhs, E, static_cast<cudaStream_t>(stream));
+}
+
+int xf_set_mechanism(xf_ctx *c, int n_reactions, const int *nu_r, const int *nu_p, const double *A, const double *B,
+                     const double *E, const int *third, const double *eff, double p_atm) {
+  if (!c || n_reactions < 1 || n_reactions > XF_MAXR || !nu_r || !nu_p || !A || !B || !E || !third || !eff || !(p_atm > 0.0))
+    return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  XfMechDev *h = new (std::nothrow) XfMechDev;
+  if (!h) return XF_ENOMEM;
+  memset(h, 0, sizeof(*h));
+  h->NR = n_reactions;
+  const int N = c->N;
+  for (int r = 0; r < n_reactions; ++r) {
+    for (int s = 0; s < N; ++s) {
+      const int a = nu_r[r * N + s], b = nu_p[r * N + s];
+      if (a < 0 || b < 0 || h->n_r[r] + a > 3 || h->n_p[r] + b > 3) {   // at most three reactant and three product molecules
+        delete h;
+        return XF_EINVAL;
+      }
+      for (int k = 0; k < a; ++k) h->re[r][h->n_r[r]++] = s;
+      for (int k = 0; k < b; ++k) h->pr[r][h->n_p[r]++] = s;
+      h->eff[r][s] = eff[r * N + s];
+    }
+    h->A[r] = A[r];
+    h->B[r] = B[r];
+    h->E[r] = E[r];
+    h->third[r] = third[r] != 0;
+  }
+  for (int s = 0; s < N; ++s) {
+    h->a7[s] = c->a7[s];
+    h->W[s] = c->W[s];
+  }
+  h->p_atm = p_atm;
+  h->Ru = c->Ru;
+  bool ok = c->mech_dev || cudaMalloc(&c->mech_dev, sizeof(XfMechDev)) == cudaSuccess;
+  ok = ok && cudaMemcpy(c->mech_dev, h, sizeof(XfMechDev), cudaMemcpyHostToDevice) == cudaSuccess;
+  delete h;
+  return ok ? XF_OK : XF_ECUDA;
+}
+
+int xf_react(xf_ctx *c, double *U, double *T, double dt, int n_sub, int n_corr, void *stream) {
+  if (!c || !U || !T || !c->mech_dev || !(dt >= 0.0) || isinf(dt) || n_sub < 1 || n_corr < 1) return XF_EINVAL;
+  Range r("xf_react");
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  ++c->launches;
+  Timed t(c, XF_K_REACT, static_cast<cudaStream_t>(stream));
+  return xf_launch_react(c->G, c->Th, c->mech_dev, U, T, dt, n_sub, n_corr, c->status_dev, static_cast<cudaStream_t>(stream));
 }
 
 int xf_fill_ghosts_dir(xf_ctx *c, double *U, int dir, void *stream) {

@@ -745,3 +745,31 @@ def synthetic_mechanism(table: SpeciesTable, comp: np.ndarray, n_reactions: int,
             eff[r] = rng.uniform(0.5, 3.0, n)
         A[r] = rate / 0.05 / (0.5 if tb else 1.0) * rng.uniform(0.3, 3.0) / (1000.0 ** B[r] * np.exp(-E[r] / (table.Ru * 1000.0)))
     return Mechanism(nu_r=nu_r, nu_p=nu_p, A=A, B=B, E=E, third=third, eff=eff, p_atm=float(p_atm))
+
+
+def reacting_box(nx: int, ny: int, nz: int, seed: int, bc=(BC_PERIODIC,) * 6, smooth: bool = False) -> Workload:
+    """random (or smooth periodic) composition / temperature / density field on the nine-species reacting table: the input
+    of the reaction-step tests and of bench.py --workload react"""
+    table, _ = reacting_table()
+    rng = np.random.default_rng(seed)
+    shape = (nx, ny, nz)
+    shp = (nz, ny, nx)
+    if smooth:
+        z, y, x = np.meshgrid((np.arange(nz) + 0.5) / nz, (np.arange(ny) + 0.5) / ny, (np.arange(nx) + 0.5) / nx, indexing="ij")
+        ph = lambda: np.sin(2 * np.pi * (x * (nx > 1) + y * (ny > 1) + z * (nz > 1)) + rng.uniform(0, 6))   # noqa: E731
+        Y = np.stack([np.exp(0.8 * ph()) for _ in range(9)])
+        Y /= Y.sum(axis=0)
+        T = 1100.0 + 250.0 * ph()
+        rho = 1.0 + 0.2 * ph()
+        c = np.sqrt(table.frozen_gamma(Y, T) * table.mixture_R(Y) * T)
+        vel = [0.3 * c * ph() if m > 1 else np.zeros(shp) for m in shape]
+    else:
+        Y = rng.dirichlet(0.7 * np.ones(9), size=shp).transpose(3, 0, 1, 2)
+        Y[3][rng.uniform(size=shp) < 0.2] = 0.0                  # a species absent from a fifth of the cells
+        Y /= Y.sum(axis=0)
+        T = rng.uniform(700, 2200, shp)
+        rho = 10 ** rng.uniform(-0.4, 0.4, shp)
+        vel = [rng.normal(size=shp) * 30 if m > 1 else np.zeros(shp) for m in shape]
+    Ui = conserved_from_primitive(table, rho, vel[0], vel[1], vel[2], T, Y)
+    d = [1.0 / m if m > 1 else 1.0 for m in shape]
+    return _finish("reacting_box", nx, ny, nz, d[0], d[1], d[2], table, bc, Ui, T, rng)

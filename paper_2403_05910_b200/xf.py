@@ -27,12 +27,12 @@ ABI_SYMBOLS = (
     "xf_create", "xf_destroy", "xf_num_vars", "xf_padded_cells", "xf_rhs_workspace_bytes", "xf_workspace_bytes",
     "xf_fill_ghosts", "xf_primitives", "xf_convective_rhs", "xf_rk3_step", "xf_rk3_step_cfl", "xf_step_cfl",
     "xf_max_wavespeed", "xf_set_rhs_dt", "xf_viscous_rhs", "xf_fill_ghosts_dir", "xf_halo_doubles", "xf_pack_halo",
-    "xf_unpack_halo", "xf_rk3_stage",
+    "xf_unpack_halo", "xf_rk3_stage", "xf_set_mechanism", "xf_react",
     "xf_status", "xf_newton_mean_iterations", "xf_launch_count", "xf_convective_rhs_host", "xf_rk3_steps_host",
     "xf_probe_fp64_peak", "xf_probe_fp64_sustained", "xf_strerror", "xf_timing_enable", "xf_timing_read",
 )
 KERNEL_KINDS = ("ghost_fill", "primitives", "sweep_x", "sweep_y", "sweep_z", "max_wavespeed", "transport",
-                "viscous")  # XF_K_* of xf.h
+                "viscous", "react")  # XF_K_* of xf.h
 
 
 class XfConfig(C.Structure):
@@ -76,6 +76,10 @@ def lib() -> C.CDLL:
         L.xf_convective_rhs.argtypes = [ctx, dp, dp, dp, vp, vp]
         L.xf_set_rhs_dt.argtypes = [ctx, C.c_double]
         L.xf_viscous_rhs.argtypes = [ctx, dp, dp, dp, vp, vp]
+        ip = C.POINTER(C.c_int)
+        ddp = C.POINTER(C.c_double)
+        L.xf_set_mechanism.argtypes = [ctx, C.c_int, ip, ip, ddp, ddp, ddp, ip, ddp, C.c_double]
+        L.xf_react.argtypes = [ctx, dp, dp, C.c_double, C.c_int, C.c_int, vp]
         L.xf_fill_ghosts_dir.argtypes = [ctx, dp, C.c_int, vp]
         L.xf_halo_doubles.argtypes = [ctx, C.c_int]
         L.xf_halo_doubles.restype = C.c_size_t
@@ -240,6 +244,20 @@ class Context:
         assert work.numel() * work.element_size() >= self.rhs_workspace_bytes
         _check(lib().xf_convective_rhs(self._h, _ptr(U), _ptr(T), _ptr(rhs), _ptr(work), _stream(stream)),
                "xf_convective_rhs")
+
+    def xf_set_mechanism(self, m) -> None:
+        """m: an object with nu_r, nu_p [NR, N] (int), A, B, E [NR], third [NR], eff [NR, N], p_atm (workloads.Mechanism)"""
+        i32 = lambda a: np.ascontiguousarray(a, dtype=np.int32)       # noqa: E731
+        f64 = lambda a: np.ascontiguousarray(a, dtype=np.float64)     # noqa: E731
+        nu_r, nu_p, third, A, B, E, eff = i32(m.nu_r), i32(m.nu_p), i32(m.third), f64(m.A), f64(m.B), f64(m.E), f64(m.eff)
+        assert nu_r.shape == nu_p.shape == eff.shape == (A.shape[0], self.N)
+        ip, ddp = C.POINTER(C.c_int), C.POINTER(C.c_double)
+        _check(lib().xf_set_mechanism(self._h, int(A.shape[0]), nu_r.ctypes.data_as(ip), nu_p.ctypes.data_as(ip),
+                                      A.ctypes.data_as(ddp), B.ctypes.data_as(ddp), E.ctypes.data_as(ddp),
+                                      third.ctypes.data_as(ip), eff.ctypes.data_as(ddp), float(m.p_atm)), "xf_set_mechanism")
+
+    def xf_react(self, U, T, dt: float, n_sub: int = 1, n_corr: int = 1, stream=None) -> None:
+        _check(lib().xf_react(self._h, _ptr(U), _ptr(T), float(dt), int(n_sub), int(n_corr), _stream(stream)), "xf_react")
 
     def xf_fill_ghosts_dir(self, U, d: int, stream=None) -> None:
         _check(lib().xf_fill_ghosts_dir(self._h, _ptr(U), int(d), _stream(stream)), "xf_fill_ghosts_dir")
