@@ -27,18 +27,28 @@ __device__ __forceinline__ double fit_eval(const double *a, double lnT) {   // E
   return exp(fma(lnT, fma(lnT, fma(lnT, a[3], a[2]), a[1]), a[0]));
 }
 
-// Per-thread arrays live in shared memory ([species][thread]: conflict-free, dynamically indexable), so the O(N^2) pair
-// loops stay ROLLED: a fully unrolled version (45 exponentials inline at N = 10) took 255 registers, spilled and ran at a
-// quarter of this one's speed.
+// Per-thread arrays live in shared memory ([species][thread]: conflict-free, indexable by a runtime species number) and
+// the transport table is copied there once per block.  What is unrolled and what is not was measured on config 4
+// (N = 10): everything unrolled (45 + 20 exponentials inline) took 255 registers, spilled and ran 27.8 ms; everything
+// rolled with the table in global memory 15.4 ms at 81 % of the L1 throughput (four memory operations per five fp64
+// ones in the pair loops); table in shared memory, the t side of Wilke's pair loop in registers with the s loop rolled,
+// and the symmetric 1/D_st pair loop unrolled with its denominators in registers: 10.9 ms at 92 registers.
 constexpr int TR_THREADS = 128;
 template <int N_T>
 __global__ void __launch_bounds__(TR_THREADS)
-transport_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const XfTransportDev *__restrict__ tr,
+transport_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const XfTransportDev *__restrict__ tr_glob,
                  const double *__restrict__ U, const double *__restrict__ T, double *__restrict__ vtab) {
   const int N = N_T > 0 ? N_T : th.N;
-  extern __shared__ double sh[];                     // X, a, sq, isq: 4 arrays [N][TR_THREADS]; num, den reuse a, sq
-  double *X = sh + threadIdx.x, *a = X + N * TR_THREADS, *sq = a + N * TR_THREADS, *isq = sq + N * TR_THREADS;
-  double *num = a, *den = sq;
+  // shared memory: a copy of the transport table (its coefficients are read at warp-uniform addresses inside the pair
+  // loops: broadcast LDS instead of one L1 transaction per coefficient -- the kernel sat at 81 % of the L1 throughput
+  // with the table in global memory), then X, a, sq, isq: 4 arrays [N][TR_THREADS]; den reuses sq
+  extern __shared__ double sh[];
+  constexpr int TBL = (int)(sizeof(XfTransportDev) / sizeof(double));
+  for (int q = threadIdx.x; q < TBL; q += TR_THREADS) sh[q] = reinterpret_cast<const double *>(tr_glob)[q];
+  __syncthreads();
+  const XfTransportDev *tr = reinterpret_cast<const XfTransportDev *>(sh);
+  double *X = sh + TBL + threadIdx.x, *a = X + N * TR_THREADS, *sq = a + N * TR_THREADS, *isq = sq + N * TR_THREADS;
+  double *den = sq;
 #define AT(arr, s) arr[(s) * TR_THREADS]
   const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= G.cells) return;
@@ -84,37 +94,76 @@ transport_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const XfTr
       AT(isq, s) = ir;
     }
     double mix = 0.0;
-#pragma unroll 1
-    for (int s = 0; s < N; ++s) {
-      double dn = 0.0;
-      const double sqs = AT(sq, s);
-#pragma unroll 5
-      for (int t = 0; t < N; ++t) {
-        const double bb = fma(sqs * AT(isq, t), tr->q4[s][t], 1.0);
-        dn = fma(AT(X, t) * tr->w8[s][t], bb * bb, dn);
+    if constexpr (N_T > 0) {   // the t-side operands in registers, the t loop unrolled, the s loop rolled
+      double Xr[N_T], ir[N_T];
+#pragma unroll
+      for (int t = 0; t < N_T; ++t) {
+        Xr[t] = AT(X, t);
+        ir[t] = AT(isq, t);
       }
-      mix = fma(AT(X, s) * AT(a, s), xf_rcp(dn), mix);
+#pragma unroll 1
+      for (int s = 0; s < N_T; ++s) {
+        double dn = 0.0;
+        const double sqs = AT(sq, s);
+#pragma unroll
+        for (int t = 0; t < N_T; ++t) {
+          const double bb = fma(sqs * ir[t], tr->q4[s][t], 1.0);
+          dn = fma(Xr[t] * tr->w8[s][t], bb * bb, dn);
+        }
+        mix = fma(AT(X, s) * AT(a, s), xf_rcp(dn), mix);
+      }
+    } else {
+#pragma unroll 1
+      for (int s = 0; s < N; ++s) {
+        double dn = 0.0;
+        const double sqs = AT(sq, s);
+        for (int t = 0; t < N; ++t) {
+          const double bb = fma(sqs * AT(isq, t), tr->q4[s][t], 1.0);
+          dn = fma(AT(X, t) * tr->w8[s][t], bb * bb, dn);
+        }
+        mix = fma(AT(X, s) * AT(a, s), xf_rcp(dn), mix);
+      }
     }
     vtab[(which == 0 ? VT_MU : VT_KAPPA) * C + idx] = mix;
   }
   // ---- rho D_sm (Eq. 26 with X_t + 1e-12, reading R20; D_st(T, p) = D_st(T, p_ref) p_ref / p, reading R19)
-  for (int s = 0; s < N; ++s) AT(num, s) = AT(den, s) = 0.0;
   const double pscale = p / tr->p_ref;
-#pragma unroll 1
-  for (int s = 0; s < N; ++s) {
-    const double xs = AT(X, s) + 1e-12, Ws = tr->W[s];
-    double ns = AT(num, s), ds = AT(den, s);
-#pragma unroll 3
-    for (int t = s + 1; t < N; ++t) {
-      const double *c = tr->D[s][t];
-      const double invD = pscale * exp(-fma(lnT, fma(lnT, fma(lnT, c[3], c[2]), c[1]), c[0]));   // 1 / D_st, symmetric
-      const double xt = AT(X, t) + 1e-12;
-      ns = fma(xt, tr->W[t], ns);
-      ds = fma(xt, invD, ds);
-      AT(num, t) = fma(xs, Ws, AT(num, t));
-      AT(den, t) = fma(xs, invD, AT(den, t));
+  // numerator of Eq. 26: sum_{t != s} (X_t + eps) W_t = (the sum over all t) - its own term
+  double wsum = 0.0;
+  for (int t = 0; t < N; ++t) wsum = fma(AT(X, t) + 1e-12, tr->W[t], wsum);
+  if constexpr (N_T > 0) {   // the N (N - 1)/2 pair terms unrolled, the denominators in registers
+    double xe[N_T], dn[N_T];
+#pragma unroll
+    for (int t = 0; t < N_T; ++t) {
+      xe[t] = AT(X, t) + 1e-12;
+      dn[t] = 0.0;
     }
-    vtab[(vt_rd(N) + s) * C + idx] = N > 1 ? rho * ns * xf_rcp(Wbar * ds) : 0.0;
+#pragma unroll
+    for (int s = 0; s < N_T; ++s)
+#pragma unroll
+      for (int t = s + 1; t < N_T; ++t) {
+        const double *c = tr->D[s][t];
+        const double invD = pscale * exp(-fma(lnT, fma(lnT, fma(lnT, c[3], c[2]), c[1]), c[0]));   // 1 / D_st, symmetric
+        dn[s] = fma(xe[t], invD, dn[s]);
+        dn[t] = fma(xe[s], invD, dn[t]);
+      }
+#pragma unroll
+    for (int s = 0; s < N_T; ++s)
+      vtab[(vt_rd(N) + s) * C + idx] = N > 1 ? rho * fma(-xe[s], tr->W[s], wsum) * xf_rcp(Wbar * dn[s]) : 0.0;
+  } else {
+    for (int s = 0; s < N; ++s) AT(den, s) = 0.0;
+#pragma unroll 1
+    for (int s = 0; s < N; ++s) {
+      const double xs = AT(X, s) + 1e-12;
+      double ds = AT(den, s);
+      for (int t = s + 1; t < N; ++t) {
+        const double *c = tr->D[s][t];
+        const double invD = pscale * exp(-fma(lnT, fma(lnT, fma(lnT, c[3], c[2]), c[1]), c[0]));
+        ds = fma(AT(X, t) + 1e-12, invD, ds);
+        AT(den, t) = fma(xs, invD, AT(den, t));
+      }
+      vtab[(vt_rd(N) + s) * C + idx] = N > 1 ? rho * fma(-xs, tr->W[s], wsum) * xf_rcp(Wbar * ds) : 0.0;
+    }
   }
 #undef AT
 }
@@ -135,7 +184,7 @@ struct ViscArgs {
 
 #ifndef XF_VISC_LT
 #define XF_VISC_LT 16   // lanes along i of a y / z tile (a warp = two rows of 128 bytes)
-#define XF_VISC_MINB 3
+#define XF_VISC_MINB 4
 #endif
 // DIR = 0: block = LDF threads along i, one face each, LDF - 3 cells; DIR = 1, 2: block = 32 lanes along i x LDF face rows
 template <int N_T, int DIR, int LDF>
@@ -172,8 +221,12 @@ visc_dir_kernel(const XfGrid G, const int Nrt, const ViscArgs A) {
     const long long q0 = ia - sd, q1 = ia, q2 = ia + sd, q3 = ia + 2 * sd;
     const double *V = A.vtab;
     const double in = G.inv_d[DIR] * (1.0 / 24.0);
-#define FACE(f) interp4(V[(f) * C + q0], V[(f) * C + q1], V[(f) * C + q2], V[(f) * C + q3])
-#define DN(f) ((27.0 * (V[(f) * C + q2] - V[(f) * C + q1]) - (V[(f) * C + q3] - V[(f) * C + q0])) * in)
+    // every load of the cell table goes through the read-only path (__ldg): the table is a generic pointer inside a
+    // struct, and without this the compiler must keep each load behind the previous shared-memory store of a flux
+    // component -- one or two loads in flight per thread on a kernel that is bound by memory latency
+#define VL(f, q) __ldg(V + (f) * C + (q))
+#define FACE(f) interp4(VL(f, q0), VL(f, q1), VL(f, q2), VL(f, q3))
+#define DN(f) ((27.0 * (VL(f, q2) - VL(f, q1)) - (VL(f, q3) - VL(f, q0))) * in)
     double Gr[3][3];                                              // Gr[p][e] = d u_p / d x_e at the face
 #pragma unroll
     for (int p = 0; p < 3; ++p) {
@@ -189,7 +242,7 @@ visc_dir_kernel(const XfGrid G, const int Nrt, const ViscArgs A) {
 #pragma unroll
           for (int m = 0; m < 4; ++m) {
             const long long z = ia + (long long)(m - 1) * sd;
-            t[m] = ((u[z - 2 * se] - u[z + 2 * se]) - 8.0 * (u[z - se] - u[z + se])) * ie;
+            t[m] = ((__ldg(u + z - 2 * se) - __ldg(u + z + 2 * se)) - 8.0 * (__ldg(u + z - se) - __ldg(u + z + se))) * ie;
           }
           Gr[p][e] = interp4(t[0], t[1], t[2], t[3]);
         }
@@ -219,10 +272,11 @@ visc_dir_kernel(const XfGrid G, const int Nrt, const ViscArgs A) {
         qd = fma(FACE(vt_h(N) + s), J, qd);
         if (s < N - 1) fs[((4 + s) * LDF + k) * LT + lt] = -J;
       }
-    const double dT = (27.0 * (A.T[q2] - A.T[q1]) - (A.T[q3] - A.T[q0])) * in;
+    const double dT = (27.0 * (__ldg(A.T + q2) - __ldg(A.T + q1)) - (__ldg(A.T + q3) - __ldg(A.T + q0))) * in;
     fs[(3 * LDF + k) * LT + lt] = work + kappa * dT - qd;         // tau.u - q_c - q_d (Eq. 2, 4)
 #undef FACE
 #undef DN
+#undef VL
   }
   __syncthreads();
   const int cell = c0 + k;                                        // this thread's cell: faces k .. k + 3 of the tile
@@ -280,9 +334,9 @@ int xf_launch_transport(const XfGrid &G, const XfThermo &Th, const XfTransportDe
                         double *vtab, cudaStream_t s) {
   const int threads = TR_THREADS;
   const unsigned blocks = (unsigned)((G.cells + threads - 1) / threads);
-  const size_t smem = sizeof(double) * 4 * (size_t)Th.N * TR_THREADS;   // N = 16: 64 KB
+  const size_t smem = sizeof(XfTransportDev) + sizeof(double) * 4 * (size_t)Th.N * TR_THREADS;   // N = 16: 13 + 64 KB
 #define CALL(NT)                                                                                                   \
-  cudaFuncSetAttribute(transport_kernel<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(double) * 4 * XF_MAXN * TR_THREADS)); \
+  cudaFuncSetAttribute(transport_kernel<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(XfTransportDev) + sizeof(double) * 4 * XF_MAXN * TR_THREADS)); \
   transport_kernel<NT><<<blocks, threads, smem, s>>>(G, Th, tr_dev, U, T, vtab)
   XF_DISPATCH_N(Th.N, CALL)
 #undef CALL
