@@ -2,7 +2,7 @@
  * xf.h -- C ABI of libxf.so: the convective right-hand side of the multicomponent compressible Euler equations
  * (the per-Runge-Kutta-stage hot path of XFluids, arxiv 2403.05910) as hand-written CUDA for sm_100a.
  *
- * Citations are PAPER.md:<line> (the paper) and DESIGN.md readings R1..R15 where the paper prints no formula.
+ * Citations are PAPER.md:<line> (the paper) and DESIGN.md readings R1..R30 where the paper prints no formula.
  *
  * Conventions
  *   Variables   Nv = N + 4 per cell: v = 0 rho, 1..3 rho u, rho v, rho w, 4 E, 5.. rho Y_1 .. rho Y_{N-1}
@@ -107,8 +107,9 @@ int xf_destroy(xf_ctx *ctx);
 
 size_t xf_num_vars(const xf_ctx *ctx);            /* Nv                                                        */
 size_t xf_padded_cells(const xf_ctx *ctx);        /* product of padded extents                                 */
-size_t xf_rhs_workspace_bytes(const xf_ctx *ctx); /* scratch for xf_convective_rhs: (N + 4) fields             */
-size_t xf_workspace_bytes(const xf_ctx *ctx);     /* scratch for xf_rk3_step: the above + 3 U-sized buffers    */
+size_t xf_rhs_workspace_bytes(const xf_ctx *ctx); /* scratch for xf_convective_rhs / xf_viscous_rhs: (N + 4) fields
+                                                     (+ 3 N + 5 with a transport table)                        */
+size_t xf_workspace_bytes(const xf_ctx *ctx);     /* scratch for the RK3 calls: the above + 3 U-sized buffers  */
 
 /* Ghost-cell fill ("specific boundary conditions"; reading R10): periodic wrap,
  * transmissive copy of the nearest interior cell, reflective mirror with the wall-normal momentum negated, or the

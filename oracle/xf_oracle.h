@@ -4,7 +4,7 @@
  *
  * This is the slow, obviously-correct fp64 restatement of what the hot path computes.  It follows the paper
  * step by step (citations are PAPER.md:<line>, section / equation) and, where the paper prints no formula,
- * the readings R1..R15 listed in DESIGN.md (taken from SURVEY.md 8(c)).  It shares NO code with the CUDA path
+ * the readings R1..R30 listed in DESIGN.md (R1-R15 taken from SURVEY.md 8(c)).  It shares NO code with the CUDA path
  * (paper_2403_05910_b200/csrc): dense Nv x Nv eigenvector matrices and dense mat-vec products here, an expanded
  * structured form there; plain Jiang-Shu weights with three divisions here, a common-denominator form there.
  *
