@@ -295,7 +295,8 @@ def test_step_cfl_matches_wavespeed_then_rk3():
 
 
 def w_interior(U, w):
-    gx, gy, gz = (3 if w.nx > 1 else 0), (3 if w.ny > 1 else 0), (3 if w.nz > 1 else 0)
+    ng = getattr(w, "ng", 3)
+    gx, gy, gz = (ng if w.nx > 1 else 0), (ng if w.ny > 1 else 0), (ng if w.nz > 1 else 0)
     return U[:, gz:gz + w.nz, gy:gy + w.ny, gx:gx + w.nx]
 
 
@@ -646,3 +647,30 @@ def test_full_size_runs_stay_physical(name, steps):
     a, b = w_interior(g.U, w)[..., far], w_interior(U0, w)[..., far]
     assert float((a - b).abs().max()) <= 1e-12 * float(b.abs().max())
     g.close()
+
+
+def test_full_size_config4_with_the_widening_options_stays_physical():
+    """config 4 at its stated size through the SURVEY 8(f) options, checked by properties that hold at any size: WENO7 (four
+    ghost layers), the positivity limiter (rho, every Y_s incl. the closure species >= 0 where the plain scheme
+    undershoots), viscous terms; status word clean, everything finite, the far field untouched."""
+    import torch
+
+    w3 = wl.config4_shock_bubble_3d_10sp(512, 256, 256)
+    tr = wl.synthetic_transport(w3.table, seed=4, mu0=2e-4)
+    for name, w, kw, steps in (("limiter", w3, dict(positivity=True), 12), ("viscous", w3, dict(transport=tr), 6),
+                               ("weno7", wl.with_ghost_width(w3, 4), dict(reconstruction=2), 8)):
+        g = _gpu(w, **kw)
+        U0 = g.U.clone()
+        for _ in range(steps):
+            g.ctx.xf_step_cfl(g.U, g.T, w.cfl, g.S, g.work)
+        assert g.ctx.xf_status() == 0, name
+        Ui, U0i = w_interior(g.U, w), w_interior(U0, w)
+        assert bool(torch.isfinite(Ui).all()) and float(Ui[0].min()) > 0.0, name
+        if name == "limiter":
+            Y = Ui[5:] / Ui[0]
+            assert float(Y.min()) >= 0.0 and float((1.0 - Y.sum(dim=0)).min()) >= 0.0
+        far = slice(int(0.9 * w.nx), w.nx)
+        assert float((Ui[..., far] - U0i[..., far]).abs().max()) <= 1e-12 * float(U0i[..., far].abs().max()), name
+        g.close()
+        del g, U0, Ui, U0i
+        torch.cuda.empty_cache()
