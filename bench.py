@@ -319,6 +319,8 @@ def run_b200(args, rank: int, local_rank: int, world: int) -> None:
         return run_config5(args, rank, local_rank, world, ranks)
     if name == "react":
         return run_react(args, rank, local_rank, world, ranks)
+    if args.blocks:
+        return run_blocks(args, rank, local_rank, world, ranks)
     w = make_workload(name, grid)
     if args.reconstruction == 2:
         from paper_2403_05910_b200 import workloads as wl
@@ -560,6 +562,49 @@ def run_config5(args, rank: int, local_rank: int, world: int, ranks) -> None:
     ranks.close()
 
 
+def run_blocks(args, rank: int, local_rank: int, world: int, ranks) -> None:
+    """The workload cut into px x py x pz blocks that live in this one process (halo.LocalTransport): every step goes through
+    xf_fill_ghosts_dir / xf_pack_halo / device copy / xf_unpack_halo per direction and xf_rk3_stage per block -- the calls a
+    multi-GPU run makes, minus the wire.  Reports the step time beside which the single-block figure can be set."""
+    import torch
+
+    from paper_2403_05910_b200 import halo
+
+    name = args.workload
+    grid = tuple(args.grid) if args.grid else WORKLOADS[name][1]
+    w = make_workload(name, grid)
+    dec, blocks = halo.make_blocks(w, args.blocks, device=local_rank)
+    sol = halo.Solver(halo.LocalTransport(blocks))
+    for _ in range(args.warmup):
+        sol.step_cfl(float(w.cfl))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = sum(b.ctx.xf_launch_count() for b in blocks.values())
+    ranks.barrier()
+    e0.record()
+    for _ in range(args.steps):
+        sol.step_cfl(float(w.cfl))
+    e1.record()
+    ranks.barrier()
+    ms = ranks.max(float(e0.elapsed_time(e1))) / args.steps
+    launches = sum(b.ctx.xf_launch_count() for b in blocks.values()) - l0
+    for b in blocks.values():
+        if b.ctx.xf_status() != 0:
+            raise RuntimeError("non-physical state in a block")
+    halo_bytes = sum(8 * buf.numel() for b in blocks.values() for buf in b.send.values()) * 3
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": w.interior_cells * 3 * world / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": name, "grid": list(grid), "blocks": list(args.blocks), "transport": "in-process device copies",
+                       "halo_bytes_per_step": halo_bytes, "step": "max wave speed over the blocks (host reduction) + 3 x (per "
+                       "direction: ghost fill, pack, copy, unpack; xf_rk3_stage per block)"},
+            "gpu_launches": launches}), flush=True)
+    for b in blocks.values():
+        b.ctx.close()
+    ranks.close()
+
+
 def run_react(args, rank: int, local_rank: int, world: int, ranks) -> None:
     """The reaction step alone (not the bench line): xf_react over dt with 4 sub-steps of one
     predictor and one corrector on 256x128x128 cells of the nine-species reacting box, 19-reaction seeded mechanism; the
@@ -622,6 +667,9 @@ def main() -> None:
     ap.add_argument("--viscosity", type=int, default=0, help="0 LLF (the benchmark), 1 ROE, 2 GLF")
     ap.add_argument("--reconstruction", type=int, default=0, help="0 WENO5-JS (the benchmark), 1 WENO-CU6, 2 WENO7")
     ap.add_argument("--positivity", action="store_true", help="positivity-preserving flux blending on (not the benchmark)")
+    ap.add_argument("--blocks", type=int, nargs=3, default=None,
+                    help="run the workload as px py pz blocks IN THIS PROCESS through the halo-exchange path (halo.py, "
+                         "LocalTransport): what the decomposition costs on one GPU; not the benchmark")
     ap.add_argument("--viscous", action="store_true",
                     help="viscous / diffusive terms on, seeded synthetic transport fits (not the benchmark)")
     args = ap.parse_args()
