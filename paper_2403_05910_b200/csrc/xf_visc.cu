@@ -186,6 +186,9 @@ struct ViscArgs {
 #define XF_VISC_LT 16   // lanes along i of a y / z tile (a warp = two rows of 128 bytes)
 #define XF_VISC_MINB 4
 #endif
+#ifndef XF_VISC_PREFETCH
+#define XF_VISC_PREFETCH 1
+#endif
 // DIR = 0: block = LDF threads along i, one face each, LDF - 3 cells; DIR = 1, 2: block = 32 lanes along i x LDF face rows
 template <int N_T, int DIR, int LDF>
 __global__ void __launch_bounds__(DIR == 0 ? LDF : XF_VISC_LT * LDF, XF_VISC_MINB)
@@ -215,6 +218,38 @@ visc_dir_kernel(const XfGrid G, const int Nrt, const ViscArgs A) {
   else base = (long long)(G.g[0] + (lane_ok ? i : 0)) + (long long)(j2 + G.g[1]) * G.st[1];
   const long long sd = G.st[DIR];
   const int n = G.n[DIR], g = G.g[DIR];
+#if XF_VISC_PREFETCH
+  // ---- the tile's lines of the cell table are asked into L2 before the first face needs them: a face issues ~250 loads
+  //      and a thread holds a dozen of them in flight, so without this every species pays a DRAM round trip of its own
+  //      (config 4, three launches: 17.9 -> 15.7 ms; also asking for the transverse neighbour rows of u, v, w and for
+  //      the residual rows cost more than it gave: 18.5 ms)
+  {
+    const int tid = DIR == 0 ? threadIdx.x : threadIdx.y * LT + threadIdx.x;
+    constexpr int NTH = DIR == 0 ? LDF : LT * LDF;
+    const int nf = 3 * N + 6;                                     // the cell table and T
+    const int r0 = c0 - 3 > -g ? c0 - 3 : -g, r1 = c0 + LD + 2 < n + g - 1 ? c0 + LD + 2 : n + g - 1;
+    if (DIR == 0) {                                               // cells r0 .. r1 of one row: consecutive doubles
+      const long long q0 = base + g + r0;
+      const int span = r1 - r0, nl = span / 16 + 2;               // 128-byte lines (one more: the row starts anywhere in a line)
+      for (int it = tid; it < nf * nl; it += NTH) {
+        const int f = it / nl, l = it - f * nl;
+        const long long q = q0 + (l * 16 < span ? l * 16 : span);
+        const double *ptr = f < nf - 1 ? A.vtab + f * C + q : A.T + q;
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
+      }
+    } else {                                                      // rows r0 .. r1, LT lanes: first and last lane of each row
+      const int i0 = blockIdx.x * LT, i1 = i0 + LT - 1 < G.n[0] - 1 ? i0 + LT - 1 : G.n[0] - 1;
+      const long long b0 = base - (lane_ok ? i : 0);              // padded index of the pencil of lane i = 0
+      const int nr = r1 - r0 + 1;
+      for (int it = tid; it < nf * nr * 2; it += NTH) {
+        const int f = it / (nr * 2), rem = it - f * nr * 2, r = rem >> 1;
+        const long long q = b0 + ((rem & 1) ? i1 : i0) + (long long)(g + r0 + r) * sd;
+        const double *ptr = f < nf - 1 ? A.vtab + f * C + q : A.T + q;
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
+      }
+    }
+  }
+#endif
   const int a = c0 - 2 + k;                                       // interior number of the cell below this thread's face
   if (lane_ok && a <= n && a >= -2) {                             // faces above cells -2 .. n (reading R22)
     const long long ia = base + (long long)(g + a) * sd;
@@ -289,12 +324,23 @@ visc_dir_kernel(const XfGrid G, const int Nrt, const ViscArgs A) {
       kap = A.alpha / (A.beta * dt);
     }
     if (A.first) A.out[ic] = A.Un ? kap * A.Un[ic] : 0.0;         // the density row has no viscous flux
-    for (int v = 1; v < Nv; ++v) {
-      const double *f = fs + ((v - 1) * LDF + k) * LT + lt;
-      const double dv = (27.0 * (f[2 * LT] - f[LT]) - (f[3 * LT] - f[0])) * in;
-      const long long o = v * C + ic;
-      A.out[o] = (A.first ? (A.Un ? kap * A.Un[o] : 0.0) : A.out[o]) + dv;
-    }
+    // all the operands of the update first, then the stores: written as one loop the compiler must keep every load of
+    // `out` behind the previous store to it (it cannot tell the rows apart), a chain of DRAM round trips
+    // (config 4, three launches: 21.6 -> 17.9 ms)
+    double old[NS + 4];
+#pragma unroll
+    for (int v = 1; v < NS + 4; ++v)
+      if (v < Nv) {
+        const long long o = v * C + ic;
+        old[v] = A.first ? (A.Un ? kap * A.Un[o] : 0.0) : A.out[o];
+      }
+#pragma unroll
+    for (int v = 1; v < NS + 4; ++v)
+      if (v < Nv) {
+        const double *f = fs + ((v - 1) * LDF + k) * LT + lt;
+        const double dv = (27.0 * (f[2 * LT] - f[LT]) - (f[3 * LT] - f[0])) * in;
+        A.out[v * C + ic] = old[v] + dv;
+      }
   }
 }
 
