@@ -40,7 +40,8 @@ enum {
   XF_ECUDA = -2,
   XF_ENOMEM = -3,
   XF_ENONPHYSICAL = -4, /* NaN or rho, p, T <= 0 (or c~^2 <= 0 at a face) seen on the device */
-  XF_ENOCONV = -5       /* Newton iteration hit newton_maxit                                 */
+  XF_ENOCONV = -5,      /* Newton iteration hit newton_maxit                                 */
+  XF_ETOOBIG = -6       /* problem exceeds the static scratch of xf_convective_rhs_noalloc     */
 };
 
 enum { XF_BC_PERIODIC = 0, XF_BC_TRANSMISSIVE = 1, XF_BC_REFLECTIVE = 2, XF_BC_DIRICHLET = 3,
@@ -127,6 +128,27 @@ int xf_primitives(xf_ctx *ctx, const double *U, double *T, double *p, double *c,
  * overwritten, interior read-only), primitives (T in/out), the x, y, z sweeps.  rhs is [Nv][padded]; only interior
  * entries are written.  work: xf_rhs_workspace_bytes. */
 int xf_convective_rhs(xf_ctx *ctx, double *U, double *T, double *rhs, void *work, void *stream);
+
+/* xf_convective_rhs WITHOUT a caller-provided workspace, for callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it): the scratch of the residual evaluation (p, c, 1/rho, Gamma,
+ * chi_s per padded cell -- and the cell table of the viscous terms for a context with a transport table) lives in ONE
+ * file-scope `static __device__` array of XF_NOALLOC_SCRATCH_BYTES inside the library.  Every GPU that loads the
+ * library holds that array until the process exits.  Same arithmetic, same kernels and same result, bit for bit, as
+ * xf_convective_rhs; U, T and rhs are the caller's device arrays as there.
+ *   - calls no cudaMalloc / cudaFree or allocating library routine (the context was created earlier, by xf_create);
+ *   - returns XF_ETOOBIG, launching nothing, when xf_rhs_workspace_bytes(ctx) > XF_NOALLOC_SCRATCH_BYTES
+ *     (N = 10: up to 599 186 padded cells, e.g. 78^3);
+ *   - the array is shared by every context and every call on that GPU and keeps the last call's contents.  Nothing in
+ *     it has to start at zero: the primitives (and transport) kernel writes every field of every padded cell before a
+ *     sweep reads it.  Two calls that OVERLAP on the GPU (different streams, or different host threads on different
+ *     streams) race on it: serialise them on one stream or with events;
+ *   - xf_noalloc_prepare resolves the array's device address for the context's device (cudaGetSymbolAddress, once per
+ *     device, cached).  xf_convective_rhs_noalloc does the same on its first call for a device; call xf_noalloc_prepare
+ *     beforehand where even that one-time query must stay out of the loop (before a graph capture begins). */
+#define XF_NOALLOC_SCRATCH_BYTES (64u << 20)
+size_t xf_noalloc_scratch_bytes(void);            /* = XF_NOALLOC_SCRATCH_BYTES of the loaded library */
+int xf_noalloc_prepare(xf_ctx *ctx);
+int xf_convective_rhs_noalloc(xf_ctx *ctx, double *U, double *T, double *rhs, void *stream);
 
 /* Viscous / diffusive terms (context created with cfg.transport; Eq. 1-6; readings R19-R23):
  * F_v = (0, tau, tau.u + kappa grad T - sum_s h_s J_s, -J_s) with tau of Eq. 3, mu and kappa by Wilke's rule (Eq. 22) from

@@ -4,6 +4,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 
 #include <nvtx3/nvToolsExt.h>
@@ -14,6 +15,10 @@ int xf_sweep_x_init();
 int xf_sweep_y_init();
 int xf_sweep_z_init();
 int xf_probe_fp64_launch(int blocks, int threads, int iters, double *sink, cudaStream_t s);
+
+// Scratch of xf_convective_rhs_noalloc (include/xf.h): one array per GPU that loads the library, held until exit.  In
+// host code this NAME is a host-side stand-in, not a device address -- see noalloc_scratch() below.
+static __device__ __align__(256) double g_noalloc_scratch[XF_NOALLOC_SCRATCH_BYTES / sizeof(double)];
 
 struct xf_ctx {
   XfGrid G;
@@ -62,6 +67,23 @@ struct DeviceGuard {
     if (prev >= 0) cudaSetDevice(prev);
   }
 };
+
+// Device address of g_noalloc_scratch on `device`, which must be the CURRENT device: asked of the runtime once per
+// device and cached (the query allocates nothing; the array came with the module).
+constexpr int NOALLOC_MAX_DEVICES = 64;
+int noalloc_scratch(int device, double **out) {
+  static std::mutex mu;
+  static double *ptr[NOALLOC_MAX_DEVICES];
+  if (device < 0 || device >= NOALLOC_MAX_DEVICES) return XF_EINVAL;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!ptr[device]) {
+    void *p = nullptr;
+    if (cudaGetSymbolAddress(&p, g_noalloc_scratch) != cudaSuccess || !p) return XF_ECUDA;
+    ptr[device] = static_cast<double *>(p);
+  }
+  *out = ptr[device];
+  return XF_OK;
+}
 
 inline size_t field_bytes(const xf_ctx *c) { return sizeof(double) * (size_t)c->G.cells; }
 
@@ -753,6 +775,37 @@ int xf_probe_fp64_sustained(int device, double seconds, double *tflops, double *
   return XF_OK;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// The no-allocation entry point (include/xf.h: xf_convective_rhs_noalloc).  g_noalloc_scratch (file scope, below the
+// includes) is the HOST-side stand-in of the device array: host code never passes it to a kernel; it asks the runtime
+// for the array's address on the current device, once per device, and passes that.
+// ---------------------------------------------------------------------------------------------------------------
+size_t xf_noalloc_scratch_bytes(void) { return XF_NOALLOC_SCRATCH_BYTES; }
+
+int xf_noalloc_prepare(xf_ctx *c) {
+  if (!c) return XF_EINVAL;
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  double *ptr = nullptr;
+  return noalloc_scratch(c->device, &ptr);
+}
+
+int xf_convective_rhs_noalloc(xf_ctx *c, double *U, double *T, double *rhs, void *stream) {
+  if (!c || !U || !T || !rhs) return XF_EINVAL;
+  if (xf_rhs_workspace_bytes(c) > (size_t)XF_NOALLOC_SCRATCH_BYTES) return XF_ETOOBIG;
+  Range r("xf_convective_rhs_noalloc");
+  DeviceGuard guard(c->device);
+  if (!guard.ok) return XF_ECUDA;
+  double *scratch = nullptr;
+  const int rc = noalloc_scratch(c->device, &scratch);   // cached after the first call for this device
+  if (rc != XF_OK) return rc;
+  XfEpilogue E;
+  memset(&E, 0, sizeof(E));
+  E.mode = 0;
+  E.out = rhs;
+  return residual(c, U, T, scratch, rhs, E, static_cast<cudaStream_t>(stream));
+}
+
 const char *xf_strerror(int code) {
   switch (code) {
     case XF_OK: return "ok";
@@ -761,6 +814,7 @@ const char *xf_strerror(int code) {
     case XF_ENOMEM: return "out of device memory";
     case XF_ENONPHYSICAL: return "non-physical state on the device (NaN or rho, p, T <= 0)";
     case XF_ENOCONV: return "Newton iteration for T(e) did not converge";
+    case XF_ETOOBIG: return "problem exceeds the static scratch of the no-allocation entry point (XF_NOALLOC_SCRATCH_BYTES)";
     default: return "unknown error";
   }
 }

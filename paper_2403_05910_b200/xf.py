@@ -16,7 +16,7 @@ import numpy as np
 _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libxf.so"
 
-XF_OK, XF_EINVAL, XF_ECUDA, XF_ENOMEM, XF_ENONPHYSICAL, XF_ENOCONV = 0, -1, -2, -3, -4, -5
+XF_OK, XF_EINVAL, XF_ECUDA, XF_ENOMEM, XF_ENONPHYSICAL, XF_ENOCONV, XF_ETOOBIG = 0, -1, -2, -3, -4, -5, -6
 XF_BC_PERIODIC, XF_BC_TRANSMISSIVE, XF_BC_REFLECTIVE, XF_BC_DIRICHLET, XF_BC_EXCHANGE = 0, 1, 2, 3, 4
 XF_VISC_LLF, XF_VISC_ROE, XF_VISC_GLF = 0, 1, 2
 XF_RECON_WENO5, XF_RECON_WENOCU6, XF_RECON_WENO7 = 0, 1, 2
@@ -30,6 +30,7 @@ ABI_SYMBOLS = (
     "xf_unpack_halo", "xf_rk3_stage", "xf_set_mechanism", "xf_react",
     "xf_status", "xf_newton_mean_iterations", "xf_launch_count", "xf_convective_rhs_host", "xf_rk3_steps_host",
     "xf_probe_fp64_peak", "xf_probe_fp64_sustained", "xf_strerror", "xf_timing_enable", "xf_timing_read",
+    "xf_noalloc_scratch_bytes", "xf_noalloc_prepare", "xf_convective_rhs_noalloc",
 )
 KERNEL_KINDS = ("ghost_fill", "primitives", "sweep_x", "sweep_y", "sweep_z", "max_wavespeed", "transport",
                 "viscous", "react")  # XF_K_* of xf.h
@@ -74,6 +75,10 @@ def lib() -> C.CDLL:
         L.xf_fill_ghosts.argtypes = [ctx, dp, vp]
         L.xf_primitives.argtypes = [ctx, dp, dp, dp, dp, vp]
         L.xf_convective_rhs.argtypes = [ctx, dp, dp, dp, vp, vp]
+        L.xf_noalloc_scratch_bytes.argtypes = []
+        L.xf_noalloc_scratch_bytes.restype = C.c_size_t
+        L.xf_noalloc_prepare.argtypes = [ctx]
+        L.xf_convective_rhs_noalloc.argtypes = [ctx, dp, dp, dp, vp]
         L.xf_set_rhs_dt.argtypes = [ctx, C.c_double]
         L.xf_viscous_rhs.argtypes = [ctx, dp, dp, dp, vp, vp]
         ip = C.POINTER(C.c_int)
@@ -244,6 +249,14 @@ class Context:
         assert work.numel() * work.element_size() >= self.rhs_workspace_bytes
         _check(lib().xf_convective_rhs(self._h, _ptr(U), _ptr(T), _ptr(rhs), _ptr(work), _stream(stream)),
                "xf_convective_rhs")
+
+    def xf_noalloc_prepare(self) -> None:
+        _check(lib().xf_noalloc_prepare(self._h), "xf_noalloc_prepare")
+
+    def xf_convective_rhs_noalloc(self, U, T, rhs, stream=None) -> None:
+        """xf_convective_rhs on the library's static device scratch (include/xf.h): no workspace, no allocation."""
+        _check(lib().xf_convective_rhs_noalloc(self._h, _ptr(U), _ptr(T), _ptr(rhs), _stream(stream)),
+               "xf_convective_rhs_noalloc")
 
     def xf_set_mechanism(self, m) -> None:
         """m: an object with nu_r, nu_p [NR, N] (int), A, B, E [NR], third [NR], eff [NR, N], p_atm (workloads.Mechanism)"""
