@@ -16,8 +16,11 @@
  * degree-4 polynomials, 5th order on smooth data; uniform-flow preservation; exact Sod Riemann solution; design
  * order on an advected density wave; round-off conservation; interface equilibrium (equal gamma); mirror and
  * permutation symmetry; direction consistency; dense-inverse brute-force face flux.
+ * Roe's property U (F_b - F_a = A~ (U_b - U_a)) in the mass, tangential-momentum and species rows for a mixture and
+ * in all rows for one perfect gas fixes the sqrt(rho) weights of u~, Y~_s, H~ (tests/test_oracle_pins_definitions.py).
  * Parity unpinned: agreement with XFluids' own code output and with the paper's Fig. 15 curves (neither code,
- * numbers nor reference data are available).
+ * numbers nor reference data are available); the sqrt(rho) weighting of Gamma~ and chi~_s in xo_eigensystem (reading
+ * R5: a definition that neither PAPER.md:107 nor the mathematics fixes; written out in the same test file).
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -fPIC -shared (no -ffast-math).  OpenMP only on outermost loops of
  * independent per-cell / per-face work, so results do not depend on the thread count.

@@ -4,8 +4,11 @@
   INTERIOR cells only);
 * ``xo_rhs_cells`` (the sampled-cell checker of the full-size GPU parity test) against ``xo_rhs`` at every interior cell;
 * the Roe-type average of reading R5 -- the sqrt(rho) weighting of Gamma~, Y~_s, chi~_s -- written out from its
-  definition.  Nothing in PAPER.md:107 or in the mathematics fixes that weighting (L R = I holds for any average), so
-  this pin only guards the DEFINITION against slips; DESIGN.md section 3 lists R5 as "parity unpinned";
+  definition.  L R = I holds for any average; what the mathematics does fix is pinned by Roe's property U
+  (F_b - F_a = A~ (U_b - U_a)): the species and tangential-momentum rows for a three-species mixture (u~, v~, w~, Y~_s)
+  and every row for one perfect gas (H~, c~^2).  The weighting of Gamma~ and chi~_s is fixed by nothing in PAPER.md:107
+  or in the mathematics, so for those two the pin only guards the DEFINITION against slips; DESIGN.md section 3 lists
+  them as "parity unpinned";
 * beta_6 of ``xo_wenocu6`` against exact rational arithmetic on smooth data (the case that motivated evaluating it on
   first differences, reading R16).
 
@@ -157,6 +160,69 @@ def test_roe_average_weights_of_reading_R5_written_out(oracle_mod, d):
     assert abs(0.5 * (a["Gamma"] + b["Gamma"]) - Gt) > 1e-2 * Gt
     assert abs(0.5 * (a["Y"][0] + b["Y"][0]) - Yt[0]) > 1e-2
     assert abs(0.5 * (a["chi"][0] + b["chi"][0]) - chit[0]) > 1e-2 * abs(chit[0])
+
+
+# --------------------------------------------------------------------------------------------------------------
+# reading R5, the part the mathematics DOES fix: Roe's property U.  With A~ = R diag(lambda) L of the averaged state,
+# F(U_b) - F(U_a) = A~ (U_b - U_a) holds row by row exactly when the average is the sqrt(rho)-weighted one:
+#   * tangential-momentum rows  Delta(rho u v) = -u~ v~ Delta rho + v~ Delta(rho u) + u~ Delta(rho v)
+#   * species rows               Delta(rho u Y_s) = -u~ Y~_s Delta rho + Y~_s Delta(rho u) + u~ Delta(rho Y_s)
+#   for ANY equation of state (these rows of A~ hold only u~, v~, w~, Y~_s), and for one calorically perfect gas with
+#   a6 = 0 (chi = 0, Gamma = gamma - 1 constant) in ALL rows, which fixes H~ and c~^2 as well (Roe 1981).
+# An arithmetic mean of u, Y_s or H fails them at O(1).  What stays a definition is the weighting of Gamma~ and chi~_s.
+# --------------------------------------------------------------------------------------------------------------
+def _roe_matrix(o, Pa, Pb, d):
+    L, R, roe, st = o.eigensystem(Pa, Pb, d)
+    assert st == 0
+    Nv = L.shape[0]
+    un, c = roe[d], roe[5]
+    lam = np.full(Nv, un)                                       # fields: u - c, u (entropy, shear x 2, species), u + c
+    lam[0], lam[Nv - 1] = un - c, un + c
+    return R @ np.diag(lam) @ L
+
+
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_roe_property_U_fixes_the_weights_of_velocity_and_mass_fractions(oracle_mod, d):
+    W3 = np.array([28.0, 4.0, 44.0])
+    g3 = np.array([1.4, 5.0 / 3.0, 1.29])
+    a63 = np.array([-350.0, 900.0, 120.0])
+    o = oracle_mod.Oracle(4, 1, 1, 0.25, 1.0, 1.0, W3, _nasa7(g3, a63), RU, 0.0, 1e300)
+    Ua, a = _state(0.3, (40.0, -15.0, 22.0), 450.0, np.array([0.6, 0.15, 0.25]), W3, g3, a63)
+    Ub, b = _state(4.0, (-10.0, 35.0, 5.0), 1300.0, np.array([0.1, 0.7, 0.2]), W3, g3, a63)
+    Pa, Pb = o.cell_primitives(Ua, 400.0), o.cell_primitives(Ub, 1000.0)
+    A = _roe_matrix(o, Pa, Pb, d)
+    dU = Ub - Ua
+    dF = o.phys_flux(Ub, Pb, d) - o.phys_flux(Ua, Pa, d)
+    AdU = A @ dU
+    rows = [0] + [1 + q for q in range(3) if q != d] + [5, 6]   # mass, the two tangential momenta, both species
+    rowscale = np.abs(A) @ np.abs(dU)                            # each row against the size of its own terms
+    assert np.max(np.abs(AdU[rows] - dF[rows]) / rowscale[rows]) <= 1e-13
+    # written out: the species and tangential rows of A~ dU with sqrt(rho) weights equal the flux jump ...
+    wa, wb = np.sqrt(a["rho"]), np.sqrt(b["rho"])
+    ut = (wa * a["vel"] + wb * b["vel"]) / (wa + wb)
+    Yt = (wa * a["Y"] + wb * b["Y"]) / (wa + wb)
+    for s in range(2):
+        row = -ut[d] * Yt[s] * dU[0] + Yt[s] * dU[1 + d] + ut[d] * dU[5 + s]
+        assert abs(row - dF[5 + s]) <= 1e-13 * rowscale[5 + s]
+    # ... and with arithmetic means they do not (so the property distinguishes the two)
+    um, Ym = 0.5 * (a["vel"] + b["vel"]), 0.5 * (a["Y"] + b["Y"])
+    row = -um[d] * Ym[0] * dU[0] + Ym[0] * dU[1 + d] + um[d] * dU[5]
+    assert abs(row - dF[5]) > 1e-2 * rowscale[5]
+
+
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_roe_property_U_in_all_rows_for_one_perfect_gas(oracle_mod, d):
+    W1, g1, z1 = np.array([28.0]), np.array([1.4]), np.array([0.0])
+    o = oracle_mod.Oracle(4, 1, 1, 0.25, 1.0, 1.0, W1, _nasa7(g1, z1), RU, 0.0, 1e300)
+    Ua, a = _state(0.3, (40.0, -15.0, 22.0), 450.0, np.array([1.0]), W1, g1, z1)
+    Ub, b = _state(4.0, (-10.0, 35.0, 5.0), 1300.0, np.array([1.0]), W1, g1, z1)
+    Pa, Pb = o.cell_primitives(Ua, 400.0), o.cell_primitives(Ub, 1000.0)
+    A = _roe_matrix(o, Pa, Pb, d)
+    dF = o.phys_flux(Ub, Pb, d) - o.phys_flux(Ua, Pa, d)
+    assert np.max(np.abs(A @ (Ub - Ua) - dF)) <= 1e-12 * np.abs(dF).max()
+    # the energy row fails by O(1) if H~ were the arithmetic mean (c~^2 = (gamma - 1)(H~ - k~) would move with it)
+    L, R, roe, _ = o.eigensystem(Pa, Pb, d)
+    assert abs(roe[3] - 0.5 * (a["H"] + b["H"])) > 1e-2 * abs(roe[3])
 
 
 # --------------------------------------------------------------------------------------------------------------
