@@ -33,7 +33,11 @@ __device__ __forceinline__ double fit_eval(const double *a, double lnT) {   // E
 // rolled with the table in global memory 15.4 ms at 81 % of the L1 throughput (four memory operations per five fp64
 // ones in the pair loops); table in shared memory, the t side of Wilke's pair loop in registers with the s loop rolled,
 // and the symmetric 1/D_st pair loop unrolled with its denominators in registers: 10.9 ms at 92 registers.
-constexpr int TR_THREADS = 128;
+// Round 2, from the ncu source page (17 % of the warp samples sat on the species loads, a rolled loop of N - 1 DRAM round
+// trips; 10 % on the block's copy of the 13 KB table): every global operand of the cell is requested first and the
+// table copy overlaps it, 1 / W_s once per block, 256 threads per block (half as many table copies): 11.1 -> 9.35 ms.
+// Tried and dropped: persistent blocks with a grid-stride loop (the compiler then keeps 164 registers or spills: 12.6 ms).
+constexpr int TR_THREADS = 256;
 template <int N_T>
 __global__ void __launch_bounds__(TR_THREADS)
 transport_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const XfTransportDev *__restrict__ tr_glob,
@@ -44,29 +48,43 @@ transport_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const XfTr
   // with the table in global memory), then X, a, sq, isq: 4 arrays [N][TR_THREADS]; den reuses sq
   extern __shared__ double sh[];
   constexpr int TBL = (int)(sizeof(XfTransportDev) / sizeof(double));
-  for (int q = threadIdx.x; q < TBL; q += TR_THREADS) sh[q] = reinterpret_cast<const double *>(tr_glob)[q];
-  __syncthreads();
-  const XfTransportDev *tr = reinterpret_cast<const XfTransportDev *>(sh);
-  double *X = sh + TBL + threadIdx.x, *a = X + N * TR_THREADS, *sq = a + N * TR_THREADS, *isq = sq + N * TR_THREADS;
+  double *X = sh + TBL + XF_MAXN + threadIdx.x, *a = X + N * TR_THREADS, *sq = a + N * TR_THREADS, *isq = sq + N * TR_THREADS;
   double *den = sq;
 #define AT(arr, s) arr[(s) * TR_THREADS]
   const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= G.cells) return;
   const long long C = G.cells;
-  const double rho = U[idx], rinv = 1.0 / rho;
+  const bool live = idx < C;
+  // Every global operand of the cell is requested before the block's copy of the table: as a rolled loop the species
+  // loads were N - 1 DRAM round trips in a row (17 % of the warp samples), and the table copy another one (10 %).
+  double rho = 1.0, Tk = 300.0;
+  if (live) {
+    rho = U[idx];
+    Tk = T[idx];
+    if constexpr (N_T > 0) {
+#pragma unroll
+      for (int s = 0; s < N_T - 1; ++s) AT(X, s) = U[(5 + s) * C + idx];
+    }
+  }
+  for (int q = threadIdx.x; q < TBL; q += TR_THREADS) sh[q] = reinterpret_cast<const double *>(tr_glob)[q];
+  if (threadIdx.x < N) sh[TBL + threadIdx.x] = 1.0 / reinterpret_cast<const XfTransportDev *>(tr_glob)->W[threadIdx.x];
+  __syncthreads();
+  const XfTransportDev *tr = reinterpret_cast<const XfTransportDev *>(sh);
+  const double *iW = sh + TBL;                                     // 1 / W_s: N divisions per block, not per cell
+  if (!live) return;
+  const double rinv = 1.0 / rho;
 #pragma unroll
   for (int q = 0; q < 3; ++q) vtab[(VT_U + q) * C + idx] = U[(1 + q) * C + idx] * rinv;
   double sumY = 0.0, sumYW = 0.0, Rbar = 0.0;
   for (int s = 0; s < N; ++s) {
-    const double Y = s < N - 1 ? U[(5 + s) * C + idx] * rinv : 1.0 - sumY;   // closure, no clipping (reading R12)
+    const double Y = s < N - 1 ? (N_T > 0 ? AT(X, s) : U[(5 + s) * C + idx]) * rinv : 1.0 - sumY;   // closure, no clipping (reading R12)
     sumY += Y;
     vtab[(VT_Y + s) * C + idx] = Y;
-    const double x = Y / tr->W[s];
+    const double x = Y * iW[s];
     AT(X, s) = x;
     sumYW += x;
     Rbar = fma(Y, th.Rs[s], Rbar);
   }
-  const double Tk = T[idx], lnT = log(Tk);
+  const double lnT = log(Tk);
   const double p = rho * Rbar * Tk;   // Eq. 7
   const double isum = 1.0 / sumYW;
   double Wbar = 0.0;
@@ -380,9 +398,9 @@ int xf_launch_transport(const XfGrid &G, const XfThermo &Th, const XfTransportDe
                         double *vtab, cudaStream_t s) {
   const int threads = TR_THREADS;
   const unsigned blocks = (unsigned)((G.cells + threads - 1) / threads);
-  const size_t smem = sizeof(XfTransportDev) + sizeof(double) * 4 * (size_t)Th.N * TR_THREADS;   // N = 16: 13 + 64 KB
+  const size_t smem = sizeof(XfTransportDev) + sizeof(double) * (XF_MAXN + 4 * (size_t)Th.N * TR_THREADS);   // N = 16: 13 + 64 KB
 #define CALL(NT)                                                                                                   \
-  cudaFuncSetAttribute(transport_kernel<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(XfTransportDev) + sizeof(double) * 4 * XF_MAXN * TR_THREADS)); \
+  cudaFuncSetAttribute(transport_kernel<NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(XfTransportDev) + sizeof(double) * (XF_MAXN + 4 * XF_MAXN * TR_THREADS))); \
   transport_kernel<NT><<<blocks, threads, smem, s>>>(G, Th, tr_dev, U, T, vtab)
   XF_DISPATCH_N(Th.N, CALL)
 #undef CALL
