@@ -32,7 +32,7 @@ struct xf_ctx {
   double *lam_glob_dev;               // GLF: [3][3] global maxima of the current residual evaluation
   int visc, recon;                    // XF_VISC_*, XF_RECON_*
   XfTransportDev *tr_dev;             // transport fits (device), or nullptr: no viscous / diffusive terms
-  XfMechDev *mech_dev;                // reaction mechanism (device), or nullptr (xf_set_mechanism)
+  XfMechDev *mech;                // reaction mechanism: HOST copy, handed to the kernel by value (constant bank), or nullptr
   double a7[XF_MAXN], W[XF_MAXN], Ru; // kept for xf_set_mechanism
   int positivity;                     // positivity-preserving flux blending on (Eq. 17-20)
   double rhs_dt;                      // the step the limiter of a bare xf_convective_rhs guards (xf_set_rhs_dt)
@@ -373,7 +373,7 @@ int xf_destroy(xf_ctx *c) {
   cudaFree(c->S_dev);
   cudaFree(c->lam_glob_dev);
   cudaFree(c->tr_dev);
-  cudaFree(c->mech_dev);
+  delete c->mech;
   cudaFree(c->hU);
   cudaFree(c->hT);
   cudaFree(c->hR);
@@ -455,23 +455,23 @@ int xf_set_mechanism(xf_ctx *c, int n_reactions, const int *nu_r, const int *nu_
   for (int s = 0; s < N; ++s) {
     h->a7[s] = c->a7[s];
     h->W[s] = c->W[s];
+    h->iW[s] = 1.0 / c->W[s];
   }
   h->p_atm = p_atm;
   h->Ru = c->Ru;
-  bool ok = c->mech_dev || cudaMalloc(&c->mech_dev, sizeof(XfMechDev)) == cudaSuccess;
-  ok = ok && cudaMemcpy(c->mech_dev, h, sizeof(XfMechDev), cudaMemcpyHostToDevice) == cudaSuccess;
-  delete h;
-  return ok ? XF_OK : XF_ECUDA;
+  delete c->mech;
+  c->mech = h;
+  return XF_OK;
 }
 
 int xf_react(xf_ctx *c, double *U, double *T, double dt, int n_sub, int n_corr, void *stream) {
-  if (!c || !U || !T || !c->mech_dev || !(dt >= 0.0) || isinf(dt) || n_sub < 1 || n_corr < 1) return XF_EINVAL;
+  if (!c || !U || !T || !c->mech || !(dt >= 0.0) || isinf(dt) || n_sub < 1 || n_corr < 1) return XF_EINVAL;
   Range r("xf_react");
   DeviceGuard guard(c->device);
   if (!guard.ok) return XF_ECUDA;
   ++c->launches;
   Timed t(c, XF_K_REACT, static_cast<cudaStream_t>(stream));
-  return xf_launch_react(c->G, c->Th, c->mech_dev, U, T, dt, n_sub, n_corr, c->status_dev, static_cast<cudaStream_t>(stream));
+  return xf_launch_react(c->G, c->Th, *c->mech, U, T, dt, n_sub, n_corr, c->status_dev, static_cast<cudaStream_t>(stream));
 }
 
 int xf_fill_ghosts_dir(xf_ctx *c, double *U, int dir, void *stream) {

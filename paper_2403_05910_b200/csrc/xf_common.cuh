@@ -47,7 +47,7 @@ struct XfTransportDev {
   double p_ref;
 };
 
-// Reaction mechanism in compiled form, in DEVICE memory (xf_react.cu): per reaction the reactant and product species
+// Reaction mechanism in compiled form, a kernel parameter of xf_react.cu (constant bank: every access is warp-uniform): per reaction the reactant and product species
 // lists (a coefficient 2 is the species listed twice; at most three entries a side), the Arrhenius parameters of Eq. 11,
 // the third-body flag and efficiencies; a7 = the entropy constants of the NASA-7 table (Eq. 12).
 #define XF_MAXR XF_MAX_REACTIONS
@@ -56,7 +56,7 @@ struct XfMechDev {
   int n_r[XF_MAXR], n_p[XF_MAXR], re[XF_MAXR][3], pr[XF_MAXR][3], third[XF_MAXR];
   double A[XF_MAXR], B[XF_MAXR], E[XF_MAXR];
   double eff[XF_MAXR][XF_MAXN];
-  double a7[XF_MAXN], W[XF_MAXN];
+  double a7[XF_MAXN], W[XF_MAXN], iW[XF_MAXN];
   double p_atm, Ru;
 };
 
@@ -132,7 +132,7 @@ int xf_launch_viscous(const XfGrid &G, int N, const double *vtab, const double *
                       cudaStream_t s, long *launches);
 
 // reaction step (xf_react.cu): species of the interior cells advanced over dt at fixed rho, rho u, E; T in / out
-int xf_launch_react(const XfGrid &G, const XfThermo &Th, const XfMechDev *mech_dev, double *U, double *T, double dt,
+int xf_launch_react(const XfGrid &G, const XfThermo &Th, const XfMechDev &mech, double *U, double *T, double dt,
                     int n_sub, int n_corr, int *status, cudaStream_t s);
 
 // fp64 reciprocal: MUFU.RCP64H seed (relative error e <= 1e-6) refined as r (1 + e + e^2), which leaves e^3:

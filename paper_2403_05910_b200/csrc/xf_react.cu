@@ -4,13 +4,15 @@
 // over dt in n_sub sub-steps of one predictor and n_corr correctors, the temperature follows from the fixed internal
 // energy by the Newton iteration of Eq. 21 after every update.  Per-thread arrays (mass fractions, concentrations, rates)
 // live in shared memory as [species][thread] so that the reaction loop can index them by species number; the mechanism
-// sits in device memory in a compiled form (reactant / product species lists, at most three of each per reaction).
+// is a kernel parameter in a compiled form (reactant / product species lists, at most three of each per reaction): all
+// threads of a warp walk the same reaction, so every access to it is a uniform constant-bank load.
 // ALU-bound by construction (a handful of exponentials per reaction per rate evaluation); no code shared with oracle/.
 #include "xf_common.cuh"
 
 namespace {
 
 constexpr int RT = 64;   // threads per block
+static_assert(sizeof(XfMechDev) + sizeof(XfThermo) + sizeof(XfGrid) + 64 < 32 * 1024, "kernel parameters: 32 KB on sm_100a");
 
 __device__ __forceinline__ double qss_alpha(double r) {   // reading R26
   if (r < 0.1) {
@@ -52,12 +54,15 @@ __device__ bool newton_T(const XfThermo &th, const int N, const double *Y, const
 }
 
 // q[s], d[s] (production and destruction rates of Y_s, 1/time) at (rho, Y, T); conc and g are scratch  (Eq. 9-12)
-__device__ void rates(const XfThermo &th, const XfMechDev *__restrict__ m, const int N, const double rho, const double *Y,
+// The reaction loop accumulates MOLAR rates (sum of R_f, R_b per species); the factor W_s / rho of Eq. 9 is applied once
+// per species afterwards instead of once per reaction and species (those divisions were 11 % of the warp samples).
+__device__ void rates(const XfThermo &th, const XfMechDev &mm, const int N, const double rho, const double *Y,
                       const double T, double *conc, double *g, double *q, double *d) {
+  const XfMechDev *m = &mm;
   const double Tc = fmin(fmax(T, th.Tlo), th.Thi), lnTc = log(Tc), lnr = log(T / Tc), iT = 1.0 / T;
   for (int s = 0; s < N; ++s) {
     const double *a = th.a[s], *b = th.b[s];
-    conc[s * RT] = rho * Y[s * RT] / m->W[s];
+    conc[s * RT] = rho * Y[s * RT] * m->iW[s];
     const double cp = fma(Tc, fma(Tc, fma(Tc, fma(Tc, a[4], a[3]), a[2]), a[1]), a[0]);
     const double hp = fma(Tc, fma(Tc, fma(Tc, fma(Tc, b[3], b[2]), b[1]), b[0]), a[0]);
     const double hR = fma(cp, T - Tc, fma(Tc, hp, a[5]));
@@ -70,17 +75,28 @@ __device__ void rates(const XfThermo &th, const XfMechDev *__restrict__ m, const
   }
   const double lnT = log(T), iRT = 1.0 / (m->Ru * T), lnp = log(m->p_atm * iRT);
   for (int r = 0; r < m->NR; ++r) {
-    double dg = 0.0, Rf = 1.0, Rb = 1.0;
+    // three reactant and three product slots, the unused ones (index 0, a valid species) switched off by a warp-uniform
+    // predicate: fixed trip counts, so all index loads and shared-memory reads of a reaction are in flight together
+    // (as loops over n_r, n_p their control flow and dependent loads were 28 % of the warp samples)
     const int nr = m->n_r[r], np = m->n_p[r];
-    for (int k = 0; k < nr; ++k) {
-      const int s = m->re[r][k];
-      dg -= g[s * RT];
-      Rf *= conc[s * RT];
+    int sr[3], sp[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      sr[k] = m->re[r][k] * RT;
+      sp[k] = m->pr[r][k] * RT;
     }
-    for (int k = 0; k < np; ++k) {
-      const int s = m->pr[r][k];
-      dg += g[s * RT];
-      Rb *= conc[s * RT];
+    double dg = 0.0, Rf = 1.0, Rb = 1.0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const double gr = g[sr[k]], cr = conc[sr[k]], gp = g[sp[k]], cp = conc[sp[k]];
+      if (k < nr) {
+        dg -= gr;
+        Rf *= cr;
+      }
+      if (k < np) {
+        dg += gp;
+        Rb *= cp;
+      }
     }
     const double kf = m->A[r] * exp(fma(m->B[r], lnT, -m->E[r] * iRT));               // Eq. 11 (reading R24)
     const double kb = kf * exp(-fma((double)(np - nr), lnp, dg));                      // k_f / K_c, Eq. 12
@@ -91,23 +107,31 @@ __device__ void rates(const XfThermo &th, const XfMechDev *__restrict__ m, const
     }
     Rf *= tb * kf;
     Rb *= tb * kb;
-    for (int k = 0; k < nr; ++k) {                                                      // Eq. 9 split as Eq. 27 (R25)
-      const int s = m->re[r][k];
-      const double w = m->W[s] / rho;
-      d[s * RT] = fma(w, Rf, d[s * RT]);
-      q[s * RT] = fma(w, Rb, q[s * RT]);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {                                                       // Eq. 9 split as Eq. 27 (R25)
+      if (k < nr) {
+        d[sr[k]] += Rf;
+        q[sr[k]] += Rb;
+      }
     }
-    for (int k = 0; k < np; ++k) {
-      const int s = m->pr[r][k];
-      const double w = m->W[s] / rho;
-      q[s * RT] = fma(w, Rf, q[s * RT]);
-      d[s * RT] = fma(w, Rb, d[s * RT]);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      if (k < np) {
+        q[sp[k]] += Rf;
+        d[sp[k]] += Rb;
+      }
     }
+  }
+  const double rinv = 1.0 / rho;
+  for (int s = 0; s < N; ++s) {
+    const double w = m->W[s] * rinv;
+    q[s * RT] *= w;
+    d[s * RT] *= w;
   }
 }
 
 __global__ void __launch_bounds__(RT)
-react_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const XfMechDev *__restrict__ m, double *__restrict__ U,
+react_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const __grid_constant__ XfMechDev m, double *__restrict__ U,
              double *__restrict__ T, const double dt, const int n_sub, const int n_corr, int *__restrict__ status) {
   const int N = th.N;
   extern __shared__ double sh[];                                   // 8 arrays [N][RT]
@@ -181,7 +205,7 @@ react_kernel(const XfGrid G, const __grid_constant__ XfThermo th, const XfMechDe
 
 }  // namespace
 
-int xf_launch_react(const XfGrid &G, const XfThermo &Th, const XfMechDev *mech_dev, double *U, double *T, double dt,
+int xf_launch_react(const XfGrid &G, const XfThermo &Th, const XfMechDev &mech, double *U, double *T, double dt,
                     int n_sub, int n_corr, int *status, cudaStream_t s) {
   const long long ncell = (long long)G.n[0] * G.n[1] * G.n[2];
   const unsigned blocks = (unsigned)((ncell + RT - 1) / RT);
@@ -191,6 +215,6 @@ int xf_launch_react(const XfGrid &G, const XfThermo &Th, const XfMechDev *mech_d
     cudaFuncSetAttribute(react_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(double) * 8 * XF_MAXN * RT));
     attr_done = true;
   }
-  react_kernel<<<blocks, RT, smem, s>>>(G, Th, mech_dev, U, T, dt, n_sub, n_corr, status);
+  react_kernel<<<blocks, RT, smem, s>>>(G, Th, mech, U, T, dt, n_sub, n_corr, status);
   return cudaGetLastError() == cudaSuccess ? XF_OK : XF_ECUDA;
 }
