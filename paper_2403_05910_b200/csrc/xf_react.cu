@@ -102,8 +102,14 @@ __device__ void rates(const XfThermo &th, const XfMechDev &mm, const int N, cons
     const double kb = kf * exp(-fma((double)(np - nr), lnp, dg));                      // k_f / K_c, Eq. 12
     double tb = 1.0;
     if (m->third[r]) {
-      tb = 0.0;
-      for (int s = 0; s < N; ++s) tb = fma(m->eff[r][s], conc[s * RT], tb);
+      double t0 = 0.0, t1 = 0.0;                                  // two chains: the sum was one dependent FMA per species
+      int s = 0;
+      for (; s + 1 < N; s += 2) {
+        t0 = fma(m->eff[r][s], conc[s * RT], t0);
+        t1 = fma(m->eff[r][s + 1], conc[(s + 1) * RT], t1);
+      }
+      if (s < N) t0 = fma(m->eff[r][s], conc[s * RT], t0);
+      tb = t0 + t1;
     }
     Rf *= tb * kf;
     Rb *= tb * kb;
