@@ -176,6 +176,62 @@ def test_second_order_against_a_stiff_reference_and_what_stays_fixed(oracle_mod)
     assert np.max(np.abs(np.append(U2[5:], rho - U2[5:].sum()) / rho - ref)) < 2 * errs[1]
 
 
+def _alpha_ld(r):
+    """alpha of reading R26 from its closed form in extended precision (series below 1e-4), not the oracle's function"""
+    x = np.longdouble(r)
+    if r < 1e-4:
+        return float(0.5 + x / 12)
+    em = -np.expm1(-x)
+    return float((1 - em / x) / em)
+
+
+@pytest.mark.parametrize("n_corr", [1, 2])
+def test_predictor_corrector_step_written_out(oracle_mod, n_corr):
+    """One sub-step of Eq. 27-28 written out in numpy from independent pieces -- the numpy rates of this file, alpha from its
+    closed form in extended precision, T from e(T, Y) by a Newton iteration on workloads' forward table evaluation -- and
+    compared with xo_react_cell.  A second-order test cannot see a slip in the PREDICTOR's alpha (any alpha leaves the
+    predictor first order and the corrector second order): a mutation of its argument survived every other pin."""
+    table, mech, o, om = _setup(oracle_mod, rate=60.0)
+    Y0 = np.array([0.12, 0.35, 0.06, 0.02, 0.015, 0.01, 0.02, 0.005, 0.4])
+    rho, vel, Tstart, h = 1.3, (2.0, 0.5, -1.0), 1500.0, 2.5e-3
+    U, e = _cell(table, rho, vel, Tstart, Y0)
+
+    def T_of(Y, Tg):
+        T = Tg
+        for _ in range(60):
+            cv = float((Y * table.Rs * (table.cp_over_R(np.float64(T)) - 1.0)).sum())
+            T = T + (e - float(table.internal_energy(Y.reshape(-1, 1), np.array([T]))[0])) / cv
+        return T
+
+    T0 = T_of(Y0, 1400.0)
+    q0, d0, _, _ = _rates_numpy(table, mech, rho, Y0, T0)
+    p0 = d0 / Y0
+    assert (p0[:-1] * h).max() > 0.5 and (p0[:-1] * h).min() < 0.05     # alpha far from 1/2 for some species, near it for others
+    a0 = np.array([_alpha_ld(r) for r in p0 * h])
+    Yp = Y0 + h * (q0 - p0 * Y0) / (1 + a0 * p0 * h)                      # predictor
+    Yp[-1] = 1.0 - Yp[:-1].sum()
+    Tp = T0
+    for _ in range(n_corr):                                               # corrector(s), reading R27
+        Tp = T_of(Yp, Tp)
+        qp, dp, _, _ = _rates_numpy(table, mech, rho, Yp, Tp)
+        pb = 0.5 * (p0 + dp / Yp)
+        ab = np.array([_alpha_ld(r) for r in pb * h])
+        qb = ab * qp + (1 - ab) * q0
+        Yc = Y0 + h * (qb - pb * Y0) / (1 + ab * pb * h)
+        Yc[-1] = 1.0 - Yc[:-1].sum()
+        Yp = Yc
+    T1 = T_of(Yp, Tp)
+    st, U1, T1o = o.react_cell(om, U, 1400.0, h, 1, n_corr)
+    assert st == 0
+    Y1o = np.append(U1[5:], rho - U1[5:].sum()) / rho
+    assert np.max(np.abs(Y1o - Yp)) <= 2e-12 * Yp.max(), np.max(np.abs(Y1o - Yp))
+    assert abs(T1o - T1) <= 1e-11 * T1
+    assert np.max(np.abs(Yp - Y0)) > 0.01                                  # the step really moves the composition
+    # the predictor's alpha matters at this step size: with alpha = 1/2 in the predictor the result is visibly different
+    Yp_half = Y0 + h * (q0 - p0 * Y0) / (1 + 0.5 * p0 * h)
+    assert np.max(np.abs(Yp_half[:-1] - (Y0 + h * (q0 - p0 * Y0) / (1 + a0 * p0 * h))[:-1])) > 1e-6
+
+
 def test_field_call_touches_interior_species_only(oracle_mod):
     table, mech, _, om = _setup(oracle_mod)
     rng = np.random.default_rng(9)
