@@ -430,6 +430,44 @@ def test_P12_direction_consistency(oracle_mod):
             assert np.max(np.abs(r - ref) / np.abs(ref).max(axis=1, keepdims=True)) <= 1e-14
 
 
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_P12_steps_in_a_box_reproduce_the_pencil(oracle_mod, axis):
+    """RK3 STEPS (not only the residual) in a 3-D box: the shock tube laid along `axis` and replicated over 4 x 5 cells in
+    the two other (periodic) directions must stay uniform across them and follow the 1-D run (itself held by P7 and P12)
+    -- the stage combinations of Eq. 16 index every interior cell of a padded 3-D array, and a slip in that indexing
+    leaves conservation, symmetry and every 1-D pin intact (a mutation of it survived them all)."""
+    w1 = wl.config1_shock_tube(nx=40, axis=axis)
+    o1 = make_oracle(oracle_mod, w1)
+    U1, T1 = w1.U.copy(), w1.T_guess.copy()
+    dt = 0.4 / o1.max_wavespeed(U1, T1)
+    ext = [4, 5, 6]
+    ext[axis] = 40
+    reps = [1, 1, 1]
+    for a in range(3):
+        if a != axis:
+            reps[a] = ext[a]
+    tile = (1, reps[2], reps[1], reps[0])                       # U[v, k, j, i]
+    Ui = np.tile(w1.interior(w1.U), tile)
+    Ti = np.tile(w1.interior(w1.T_guess), tile[1:])
+    bc = [wl.BC_PERIODIC] * 6
+    bc[2 * axis] = bc[2 * axis + 1] = wl.BC_TRANSMISSIVE
+    d = [0.3, 0.7, 1.1]                                         # transverse spacings: arbitrary, they must not matter
+    d[axis] = [w1.dx, w1.dy, w1.dz][axis]
+    w3 = wl._finish("tube_in_a_box", ext[0], ext[1], ext[2], d[0], d[1], d[2], w1.table, bc, Ui, Ti,
+                    np.random.default_rng(0), guess_jitter=0.0)
+    o3 = make_oracle(oracle_mod, w3)
+    U3, T3 = w3.U.copy(), w3.T_guess.copy()
+    for _ in range(6):
+        assert o1.rk3_step(U1, T1, dt) == 0
+        assert o3.rk3_step(U3, T3, dt) == 0
+    a1 = w1.interior(U1)                                        # [Nv, 1|40, 1|40, 1|40]
+    a3 = w3.interior(U3)
+    assert np.abs(a1 - w1.interior(w1.U)).max() > 1e-2          # the tube has really moved
+    scale = np.abs(a1).reshape(a1.shape[0], -1).max(axis=1).reshape(-1, 1, 1, 1) + 1e-300
+    scale[1:4] = scale[1:4].max()
+    assert np.max(np.abs(a3 - a1) / scale) <= 1e-13             # broadcasting a1 over the replicated directions
+
+
 # ------------------------------------------------------------------ P13: brute-force dense cross-check of a face flux
 @pytest.mark.parametrize("d", [0, 1, 2])
 def test_P13_face_flux_dense_inverse(oracle_mod, d):
