@@ -232,12 +232,14 @@ def test_predictor_corrector_step_written_out(oracle_mod, n_corr):
     assert np.max(np.abs(Yp_half[:-1] - (Y0 + h * (q0 - p0 * Y0) / (1 + a0 * p0 * h))[:-1])) > 1e-6
 
 
-def test_field_call_touches_interior_species_only(oracle_mod):
+@pytest.mark.parametrize("nz", [1, 4])
+def test_field_call_touches_interior_species_only(oracle_mod, nz):
     table, mech, _, om = _setup(oracle_mod)
     rng = np.random.default_rng(9)
     nx, ny = 6, 5
-    o = oracle_mod.Oracle(nx, ny, 1, 0.1, 0.1, 1, table.W, table.nasa7, table.Ru, table.Tlo, table.Thi)
-    shape = (1, ny + 6, nx + 6)
+    o = oracle_mod.Oracle(nx, ny, nz, 0.1, 0.1, 0.1 if nz > 1 else 1, table.W, table.nasa7, table.Ru, table.Tlo, table.Thi)
+    gz = 3 if nz > 1 else 0
+    shape = (nz + 2 * gz, ny + 6, nx + 6)
     Y = rng.dirichlet(np.ones(9), size=shape).transpose(3, 0, 1, 2)
     T = rng.uniform(900, 1500, shape)
     rho = rng.uniform(0.5, 2, shape)
@@ -246,9 +248,11 @@ def test_field_call_touches_interior_species_only(oracle_mod):
     assert o.react(om, U, T, 1e-3, 2, 1) == 0
     assert np.array_equal(U[:5], U0[:5])
     mask = np.ones(shape, dtype=bool)
-    mask[:, 3:-3, 3:-3] = False
+    mask[gz:shape[0] - gz, 3:-3, 3:-3] = False
     assert np.array_equal(U[5:][:, mask], U0[5:][:, mask]) and np.array_equal(T[mask], T0[mask])
-    assert np.max(np.abs(U[5:, :, 3:-3, 3:-3] - U0[5:, :, 3:-3, 3:-3])) > 1e-4
-    k, j, i = 0, 4, 5                                            # one cell against the per-cell call
-    st, Uc, Tc = o.react_cell(om, U0[:, k, j, i], T0[k, j, i], 1e-3, 2, 1)
-    assert np.array_equal(Uc, U[:, k, j, i]) and Tc == T[k, j, i]
+    assert np.max(np.abs(U[5:, gz:shape[0] - gz, 3:-3, 3:-3] - U0[5:, gz:shape[0] - gz, 3:-3, 3:-3])) > 1e-4
+    for k in range(gz, gz + nz):                                 # EVERY interior cell against the per-cell call
+        for j in range(3, 3 + ny):
+            for i in range(3, 3 + nx):
+                st, Uc, Tc = o.react_cell(om, U0[:, k, j, i], T0[k, j, i], 1e-3, 2, 1)
+                assert np.array_equal(Uc, U[:, k, j, i]) and Tc == T[k, j, i], (k, j, i)
