@@ -518,6 +518,25 @@ def test_rhs_parity_viscosity_variants(oracle_mod, visc, shape, n, bc):
     g.close()
 
 
+@pytest.mark.parametrize("visc", [0, 1, 2])
+def test_rhs_parity_supersonic_flow_in_the_negative_directions(oracle_mod, visc):
+    """u_d + c < 0 in every cell (a frame moving at three sound speeds along +x, +y, +z): the maxima of Eq. 14 are of
+    ABSOLUTE wave speeds -- the corner the oracle pin test_glf_global_maxima_are_over_all_padded_cells holds"""
+    w = wl.random_smooth_box(26, 20, 18, nspecies=3, seed=2100)
+    cmax = 1.5 * float(np.sqrt(np.max(w.U[4] / w.U[0])))
+    for q in (1, 2, 3):
+        mom = w.U[q] - 3.0 * cmax * w.U[0]
+        w.U[4] += 0.5 * (mom ** 2 - w.U[q] ** 2) / w.U[0]
+        w.U[q] = mom
+    orc = oracle_mod.Oracle.from_workload(w, viscosity=visc)
+    ro = orc.rhs(w.U.copy(), w.T_guess.copy())
+    assert orc.last_status == 0
+    g = _gpu(w, viscosity=visc)
+    err = field_err(w.interior(g.rhs()), w.interior(ro))
+    assert err.max() < RHS_TOL, err
+    g.close()
+
+
 @pytest.mark.parametrize("visc", [1, 2])
 def test_shock_tube_and_bubble_steps_viscosity_variants(oracle_mod, visc):
     for w, steps in ((wl.config1_shock_tube(), 100), (wl.config3_shock_bubble_3d(32), 12)):

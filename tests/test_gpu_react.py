@@ -53,6 +53,42 @@ def test_react_parity(oracle_mod, shape, n_sub, n_corr, nreac):
     g.close()
 
 
+def test_react_parity_outside_the_fit_range(oracle_mod):
+    """half of the cells hotter than T_hi: the constant-c_p continuation of h_s and S_s in the rates and in the Newton
+    iteration (readings R3, R24) -- the corner the oracle pin test_rates_outside_the_fit_range_use_the_continuation holds
+    (cold cells below T_lo are left to that pin: the seeded exothermic mechanism leaves the range within one step)"""
+    from gpu_helpers import GpuRun
+
+    w, comp = _reacting_box((16, 12, 1), seed=91)
+    t = w.table
+    Ui = w.interior(w.U)
+    rho = Ui[0]
+    Y = np.concatenate([Ui[5:] / rho, (1.0 - (Ui[5:] / rho).sum(axis=0))[None]])
+    hot = np.broadcast_to(np.arange(16)[None, None, :] < 8, rho.shape)
+    Tnew = np.where(hot, 1.2 * t.Thi, w.interior(w.T_guess[None])[0])
+    e = t.internal_energy(Y.reshape(9, -1), Tnew.reshape(-1)).reshape(rho.shape)
+    k = 0.5 * (Ui[1] ** 2 + Ui[2] ** 2 + Ui[3] ** 2) / rho
+    Ui[4] = np.where(hot, rho * e + k, Ui[4])
+    w.interior(w.T_guess[None])[0][...] = np.where(hot, Tnew * 1.01, Tnew)
+    mech = wl.synthetic_mechanism(w.table, comp, 19, seed=19, rate=5.0)
+    om = oracle_mod.make_mechanism(mech)
+    orc = oracle_mod.Oracle.from_workload(w)
+    Uo, To = w.U.copy(), w.T_guess.copy()
+    assert orc.react(om, Uo, To, 2e-4, 2, 1) == 0
+    g = GpuRun(w)
+    g.ctx.xf_set_mechanism(mech)
+    g.ctx.xf_react(g.U, g.T, 2e-4, 2, 1)
+    assert g.ctx.xf_status() == 0
+    Ug, Tg = g.host_U(), g.host_T()
+    Toi = w.interior(To[None])[0]
+    assert Toi[..., :8].min() > t.Thi and Toi[..., 8:].max() < t.Thi            # the hot half is still above the range
+    den = np.abs(w.interior(Uo)[5:]).reshape(8, -1).max(axis=1)
+    err = np.abs(w.interior(Ug)[5:] - w.interior(Uo)[5:]).reshape(8, -1).max(axis=1) / den
+    assert err.max() < 1e-11, err
+    assert np.max(np.abs(w.interior(Tg[None])[0] - Toi) / Toi) < 1e-12
+    g.close()
+
+
 def test_strang_split_reacting_flow_steps(oracle_mod):
     """react(dt/2), convective SSP-RK3 step, react(dt/2), five times: the composed path against the
     oracle's composition of the same pieces"""

@@ -132,6 +132,37 @@ def test_single_reaction_by_hand_and_detailed_balance(oracle_mod):
 # ------------------------------------------------------------------------------------------------------------
 # the integrator (readings R26-R30)
 # ------------------------------------------------------------------------------------------------------------
+def test_rates_outside_the_fit_range_use_the_continuation(oracle_mod):
+    """T above T_hi / below T_lo (readings R3, R24): c_p frozen at the range end, h continued linearly and S with
+    c_p ln(T / T_c) -- written out here; the in-range pins never reach those terms (a mutation of the entropy
+    continuation survived them)."""
+    table, mech, o, om = _setup(oracle_mod)
+    a, W, Ru = table.nasa7, table.W, table.Ru
+    rng = np.random.default_rng(6)
+    for T in (table.Thi * 1.25, table.Tlo * 0.8):
+        Tc = min(max(T, table.Tlo), table.Thi)
+        Y = rng.dirichlet(np.ones(9))
+        rho = 0.7
+        cpR = a[:, 0] + a[:, 1] * Tc + a[:, 2] * Tc ** 2 + a[:, 3] * Tc ** 3 + a[:, 4] * Tc ** 4
+        hR = (a[:, 0] * Tc + a[:, 1] * Tc ** 2 / 2 + a[:, 2] * Tc ** 3 / 3 + a[:, 3] * Tc ** 4 / 4 + a[:, 4] * Tc ** 5 / 5
+              + a[:, 5]) + cpR * (T - Tc)                         # h_s / R_s [K]
+        SR = (a[:, 0] * np.log(Tc) + a[:, 1] * Tc + a[:, 2] * Tc ** 2 / 2 + a[:, 3] * Tc ** 3 / 3 + a[:, 4] * Tc ** 4 / 4
+              + a[:, 6]) + cpR * np.log(T / Tc)
+        conc = rho * Y / W
+        nu = mech.nu_p - mech.nu_r
+        kf = mech.A * T ** mech.B * np.exp(-mech.E / (Ru * T))
+        Kc = (mech.p_atm / (Ru * T)) ** nu.sum(axis=1) * np.exp(nu @ (SR - hR / T))
+        tb = np.where(mech.third == 1, mech.eff @ conc, 1.0)
+        Rf = tb * kf * np.prod(conc[None, :] ** mech.nu_r, axis=1)
+        Rb = tb * kf / Kc * np.prod(conc[None, :] ** mech.nu_p, axis=1)
+        qn = W / rho * (mech.nu_p.T @ Rf + mech.nu_r.T @ Rb)
+        dn = W / rho * (mech.nu_r.T @ Rf + mech.nu_p.T @ Rb)
+        q, d = o.reaction_rates(om, rho, Y, T)
+        assert np.allclose(q, qn, rtol=1e-11, atol=1e-13 * np.abs(qn).max())
+        assert np.allclose(d, dn, rtol=1e-11, atol=1e-13 * np.abs(dn).max())
+        assert np.abs(cpR * np.log(T / Tc)).max() > 0.5            # the continuation term is not small here
+
+
 def _reference_solution(table, mech, rho, e, Y0, t_end):
     """scipy's implicit solver on the numpy restatement of dY/dt = q - d with T from e(T, Y) by bisection-free Newton"""
     def T_of(Y, Tg):

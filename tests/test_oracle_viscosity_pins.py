@@ -60,6 +60,13 @@ def test_glf_global_maxima_are_over_all_padded_cells(oracle_mod):
     w = wl.random_smooth_box(10, 9, 1, nspecies=2, seed=9, bc=(1, 1, 2, 2, 0, 0))
     o = _oracle(oracle_mod, w, GLF)
     U, T = w.U.copy(), w.T_guess.copy()
+    # a frame moving at three sound speeds in +x and +y: every cell flows supersonically in the NEGATIVE directions, so
+    # u + c < 0 and max |u + c| differs from max (u + c) (the maxima are of absolute values)
+    cmax = 1.5 * float(np.sqrt(np.max(U[4] / U[0])))
+    for q in (1, 2):
+        mom = U[q] - 3.0 * cmax * U[0]
+        U[4] += 0.5 * (mom ** 2 - U[q] ** 2) / U[0]
+        U[q] = mom
     rhs = o.rhs(U, T)                                         # fills ghosts, converges T
     p, c = np.zeros_like(T), np.zeros_like(T)
     oracle_mod.Oracle.from_workload(w).primitives(U, T.copy(), p, c)

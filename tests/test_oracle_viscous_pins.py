@@ -45,7 +45,7 @@ def _coords(o, n, h):
 # ------------------------------------------------------------------------------------------------------------
 def test_fits_are_polynomials_in_ln_T_and_D_scales_with_inverse_pressure(oracle_mod):
     table = wl.synthetic_nasa7_table((28.0, 4.0, 40.0), Ru=0.1, rng=np.random.default_rng(0))
-    tr = wl.synthetic_transport(table, 3)
+    tr = wl.synthetic_transport(table, 3, p_ref=2.5)           # p_ref != 1: D_st(T, p) = D_st(T, p_ref) p_ref / p (reading R19)
     o = oracle_mod.Oracle(8, 1, 1, 0.1, 1, 1, table.W, table.nasa7, table.Ru, table.Tlo, table.Thi)
     ot = oracle_mod.make_transport(tr)
     for T in (250.0, 700.0, 2500.0):
