@@ -92,6 +92,26 @@ def test_P1_newton_inside_range_inverts_table(oracle_mod):
         assert P.iters <= 8 and P.status == 0
 
 
+def test_field_primitives_agree_with_the_cell_call_and_count_iterations(oracle_mod):
+    """xo_primitives (the field call: every padded cell) against xo_cell_primitives cell by cell, and its debug counter:
+    the MEAN Newton iteration count over the padded cells."""
+    w = wl.random_smooth_box(6, 5, 4, nspecies=3, seed=107)
+    o = make_oracle(oracle_mod, w)
+    U, T = w.U.copy(), w.T_guess.copy()
+    o.fill_ghosts(U)
+    p, c = np.zeros_like(T), np.zeros_like(T)
+    st, mean_it = o.primitives(U, T, p, c)
+    assert st == 0
+    its = []
+    for k in range(T.shape[0]):
+        for j in range(T.shape[1]):
+            for i in range(T.shape[2]):
+                P = o.cell_primitives(U[:, k, j, i], w.T_guess[k, j, i])
+                its.append(P.iters)
+                assert P.T == T[k, j, i] and P.p == p[k, j, i] and P.c == c[k, j, i]
+    assert abs(mean_it - np.mean(its)) <= 1e-12 and 1.0 <= mean_it <= 10.0
+
+
 # ------------------------------------------------------------------ P2: thermodynamic identities
 def test_P2_sound_speed_identity_and_monotone_e(oracle_mod):
     rng = np.random.default_rng(201)
