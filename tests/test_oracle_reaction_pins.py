@@ -216,14 +216,18 @@ def _alpha_ld(r):
     return float((1 - em / x) / em)
 
 
+@pytest.mark.parametrize("absent", [False, True])
 @pytest.mark.parametrize("n_corr", [1, 2])
-def test_predictor_corrector_step_written_out(oracle_mod, n_corr):
+def test_predictor_corrector_step_written_out(oracle_mod, n_corr, absent):
     """One sub-step of Eq. 27-28 written out in numpy from independent pieces -- the numpy rates of this file, alpha from its
     closed form in extended precision, T from e(T, Y) by a Newton iteration on workloads' forward table evaluation -- and
     compared with xo_react_cell.  A second-order test cannot see a slip in the PREDICTOR's alpha (any alpha leaves the
     predictor first order and the corrector second order): a mutation of its argument survived every other pin."""
     table, mech, o, om = _setup(oracle_mod, rate=60.0)
     Y0 = np.array([0.12, 0.35, 0.06, 0.02, 0.015, 0.01, 0.02, 0.005, 0.4])
+    if absent:                                                  # a species that is not there: p_s = 0 where Y_s <= 0 (reading R25)
+        Y0[8] += Y0[3]
+        Y0[3] = 0.0
     rho, vel, Tstart, h = 1.3, (2.0, 0.5, -1.0), 1500.0, 2.5e-3
     U, e = _cell(table, rho, vel, Tstart, Y0)
 
@@ -236,7 +240,8 @@ def test_predictor_corrector_step_written_out(oracle_mod, n_corr):
 
     T0 = T_of(Y0, 1400.0)
     q0, d0, _, _ = _rates_numpy(table, mech, rho, Y0, T0)
-    p0 = d0 / Y0
+    with np.errstate(divide="ignore", invalid="ignore"):
+        p0 = np.where(Y0 > 0.0, d0 / Y0, 0.0)
     assert (p0[:-1] * h).max() > 0.5 and (p0[:-1] * h).min() < 0.05     # alpha far from 1/2 for some species, near it for others
     a0 = np.array([_alpha_ld(r) for r in p0 * h])
     Yp = Y0 + h * (q0 - p0 * Y0) / (1 + a0 * p0 * h)                      # predictor
@@ -245,7 +250,8 @@ def test_predictor_corrector_step_written_out(oracle_mod, n_corr):
     for _ in range(n_corr):                                               # corrector(s), reading R27
         Tp = T_of(Yp, Tp)
         qp, dp, _, _ = _rates_numpy(table, mech, rho, Yp, Tp)
-        pb = 0.5 * (p0 + dp / Yp)
+        with np.errstate(divide="ignore", invalid="ignore"):
+            pb = 0.5 * (p0 + np.where(Yp > 0.0, dp / Yp, 0.0))
         ab = np.array([_alpha_ld(r) for r in pb * h])
         qb = ab * qp + (1 - ab) * q0
         Yc = Y0 + h * (qb - pb * Y0) / (1 + ab * pb * h)
@@ -261,6 +267,27 @@ def test_predictor_corrector_step_written_out(oracle_mod, n_corr):
     # the predictor's alpha matters at this step size: with alpha = 1/2 in the predictor the result is visibly different
     Yp_half = Y0 + h * (q0 - p0 * Y0) / (1 + 0.5 * p0 * h)
     assert np.max(np.abs(Yp_half[:-1] - (Y0 + h * (q0 - p0 * Y0) / (1 + a0 * p0 * h))[:-1])) > 1e-6
+
+
+def test_a_species_outside_the_mechanism_that_is_absent_stays_absent(oracle_mod):
+    """Y_s = 0 and no reaction touches s: q_s = d_s = 0 through predictor AND corrector, where p_s = d_s / Y_s is 0 by the
+    guard of reading R25 (0/0 otherwise); the species stays exactly absent and everything else finite."""
+    table, mech, o, om = _setup(oracle_mod, n_reactions=3, seed=2)
+    used = (mech.nu_r + mech.nu_p).sum(axis=0)
+    idle = [s for s in range(8) if used[s] == 0]
+    assert idle, "the seeded three-reaction mechanism leaves some species out"
+    s0 = idle[-1]
+    assert s0 > 0                                                # not the first species: a guard that looked at Y_0 instead must show
+    Y0 = np.full(9, 0.1)
+    Y0[8] = 0.2
+    Y0[8] += Y0[s0]
+    Y0[s0] = 0.0
+    U, e = _cell(table, 1.1, (1.0, 0.0, 0.0), 1400.0, Y0)
+    for n_corr in (1, 3):
+        st, U1, T1 = o.react_cell(om, U, 1300.0, 1e-3, 2, n_corr)
+        assert st == 0 and np.all(np.isfinite(U1)) and np.isfinite(T1)
+        assert U1[5 + s0] == 0.0
+        assert np.max(np.abs(U1[5:] - U[5:])) > 1e-6             # the others do react
 
 
 @pytest.mark.parametrize("nz", [1, 4])
