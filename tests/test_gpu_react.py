@@ -89,6 +89,36 @@ def test_react_parity_outside_the_fit_range(oracle_mod):
     g.close()
 
 
+def test_react_parity_with_absent_species(oracle_mod):
+    """one species absent from every cell, another from half of them: p_s = d_s / Y_s is 0 where Y_s <= 0 (reading R25)"""
+    from gpu_helpers import GpuRun
+
+    w, comp = _reacting_box((14, 11, 1), seed=93)
+    Ui = w.interior(w.U)
+    Ui[5 + 7] += Ui[5 + 2]                                       # move species 2's mass to species 7: rho unchanged
+    Ui[5 + 2] = 0.0
+    half = np.broadcast_to(np.arange(14)[None, None, :] < 7, Ui[0].shape)
+    Ui[5 + 7] += np.where(half, Ui[5 + 4], 0.0)
+    Ui[5 + 4] = np.where(half, 0.0, Ui[5 + 4])
+    mech = wl.synthetic_mechanism(w.table, comp, 19, seed=19, rate=5.0)
+    om = oracle_mod.make_mechanism(mech)
+    orc = oracle_mod.Oracle.from_workload(w)
+    Uo, To = w.U.copy(), w.T_guess.copy()
+    assert orc.react(om, Uo, To, 3e-4, 2, 2) == 0
+    g = GpuRun(w)
+    g.ctx.xf_set_mechanism(mech)
+    g.ctx.xf_react(g.U, g.T, 3e-4, 2, 2)
+    assert g.ctx.xf_status() == 0
+    Ug, Tg = g.host_U(), g.host_T()
+    assert np.all(np.isfinite(Ug)) and np.all(np.isfinite(Tg))
+    den = np.abs(w.interior(Uo)[5:]).reshape(8, -1).max(axis=1)
+    err = np.abs(w.interior(Ug)[5:] - w.interior(Uo)[5:]).reshape(8, -1).max(axis=1) / den
+    assert err.max() < 1e-11, err
+    Toi = w.interior(To[None])[0]
+    assert np.max(np.abs(w.interior(Tg[None])[0] - Toi) / Toi) < 1e-12
+    g.close()
+
+
 def test_strang_split_reacting_flow_steps(oracle_mod):
     """react(dt/2), convective SSP-RK3 step, react(dt/2), five times: the composed path against the
     oracle's composition of the same pieces"""
